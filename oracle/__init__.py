@@ -1,0 +1,177 @@
+"""CPU oracle (TEST INFRASTRUCTURE ONLY) -- ctypes face of wilson_clover_oracle.cpp.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It never imports paper_1109_2935_b200 and shares no
+code with the CUDA path.  All arrays are numpy complex128, C-contiguous, in the
+canonical layouts of include/lqcd.h:
+
+    gauge   U[mu][t][z][y][x][3][3]      spinor  psi[t][z][y][x][4][3]
+    clover  T[t][z][y][x][12][12]        (row = spin*3 + colour)
+
+What each function computes and the passage of the paper it follows is stated in
+wilson_clover_oracle.cpp.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "wilson_clover_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+BICGSTAB, GCR_DD = 0, 1
+
+
+def build(force=False):
+    """Compile the oracle with g++ (OpenMP).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.orc_num_threads.restype = ctypes.c_int
+        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_invert"):
+            getattr(_lib, name).restype = ctypes.c_int
+    return _lib
+
+
+def _c(a):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    return a
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i4(v):
+    return (ctypes.c_int * 4)(*[int(t) for t in v])
+
+
+def _blk(block):
+    return None if block is None else _i4(block)
+
+
+def num_threads():
+    return lib().orc_num_threads()
+
+
+def dims_of(psi):
+    """(X,Y,Z,T) of a canonical spinor psi[t][z][y][x][4][3]."""
+    T, Z, Y, X = psi.shape[:4]
+    return (X, Y, Z, T)
+
+
+def gamma(mu):
+    """gamma_mu for mu=0..3 (x,y,z,t), gamma5 for mu=4, as a 4x4 complex array."""
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().orc_gamma(ctypes.c_int(mu), _p(out))
+    return out
+
+
+def dslash(psi, U, bc, dagger=False, block=None):
+    psi, U = _c(psi), _c(U)
+    out = np.empty_like(psi)
+    lib().orc_dslash(_p(out), _p(psi), _p(U), _i4(dims_of(psi)), _i4(bc), ctypes.c_int(int(dagger)), _blk(block))
+    return out
+
+
+def clover_term(U, c_sw):
+    U = _c(U)
+    _, T, Z, Y, X = U.shape[:5]
+    out = np.empty((T, Z, Y, X, 12, 12), dtype=np.complex128)
+    lib().orc_clover_term(_p(out), _p(U), _i4((X, Y, Z, T)), ctypes.c_double(c_sw))
+    return out
+
+
+def clover_apply(psi, Tcl, kappa, inverse=False, parity=-1):
+    psi, Tcl = _c(psi), _c(Tcl)
+    out = np.empty_like(psi)
+    lib().orc_clover_apply(_p(out), _p(psi), _p(Tcl), _i4(dims_of(psi)), ctypes.c_double(kappa),
+                           ctypes.c_int(int(inverse)), ctypes.c_int(parity))
+    return out
+
+
+def M(psi, U, Tcl, bc, kappa, dagger=False, block=None):
+    psi, U, Tcl = _c(psi), _c(U), _c(Tcl)
+    out = np.empty_like(psi)
+    lib().orc_M(_p(out), _p(psi), _p(U), _p(Tcl), _i4(dims_of(psi)), _i4(bc), ctypes.c_double(kappa),
+                ctypes.c_int(int(dagger)), _blk(block))
+    return out
+
+
+def matpc(psi, U, Tcl, bc, kappa, parity, dagger=False, block=None):
+    psi, U, Tcl = _c(psi), _c(U), _c(Tcl)
+    out = np.empty_like(psi)
+    lib().orc_matpc(_p(out), _p(psi), _p(U), _p(Tcl), _i4(dims_of(psi)), _i4(bc), ctypes.c_double(kappa),
+                    ctypes.c_int(parity), ctypes.c_int(int(dagger)), _blk(block))
+    return out
+
+
+def prepare_source(b, U, Tcl, bc, kappa, parity):
+    b, U, Tcl = _c(b), _c(U), _c(Tcl)
+    out = np.empty_like(b)
+    lib().orc_prepare_source(_p(out), _p(b), _p(U), _p(Tcl), _i4(dims_of(b)), _i4(bc), ctypes.c_double(kappa),
+                             ctypes.c_int(parity))
+    return out
+
+
+def reconstruct(xp, b, U, Tcl, bc, kappa, parity):
+    x = _c(xp).copy()
+    b, U, Tcl = _c(b), _c(U), _c(Tcl)
+    lib().orc_reconstruct(_p(x), _p(b), _p(U), _p(Tcl), _i4(dims_of(b)), _i4(bc), ctypes.c_double(kappa),
+                          ctypes.c_int(parity))
+    return x
+
+
+def schwarz(r, U, Tcl, bc, kappa, parity, block, n_mr=10, omega_mr=1.0):
+    r, U, Tcl = _c(r), _c(U), _c(Tcl)
+    out = np.empty_like(r)
+    lib().orc_schwarz(_p(out), _p(r), _p(U), _p(Tcl), _i4(dims_of(r)), _i4(bc), ctypes.c_double(kappa),
+                      ctypes.c_int(parity), _blk(block), ctypes.c_int(n_mr), ctypes.c_double(omega_mr))
+    return out
+
+
+def bicgstab_pc(bhat, U, Tcl, bc, kappa, parity, stop, maxit=10000, x0=None):
+    """Solve Mhat x = bhat on one parity; stop = absolute residual norm.  Returns (x, info)."""
+    bhat, U, Tcl = _c(bhat), _c(U), _c(Tcl)
+    x = np.zeros_like(bhat) if x0 is None else _c(x0).copy()
+    it, rn = ctypes.c_int(0), ctypes.c_double(0)
+    st = lib().orc_bicgstab_pc(_p(x), _p(bhat), _p(U), _p(Tcl), _i4(dims_of(bhat)), _i4(bc), ctypes.c_double(kappa),
+                               ctypes.c_int(parity), ctypes.c_double(stop), ctypes.c_int(maxit),
+                               ctypes.byref(it), ctypes.byref(rn))
+    return x, dict(status=st, iterations=it.value, residual_norm=rn.value)
+
+
+def gcr_pc(bhat, U, Tcl, bc, kappa, parity, stop, maxit=10000, kmax=16, delta=0.1, precond=True,
+           block=None, n_mr=10, omega_mr=1.0, x0=None):
+    bhat, U, Tcl = _c(bhat), _c(U), _c(Tcl)
+    x = np.zeros_like(bhat) if x0 is None else _c(x0).copy()
+    it, rs, rn = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_double(0)
+    st = lib().orc_gcr_pc(_p(x), _p(bhat), _p(U), _p(Tcl), _i4(dims_of(bhat)), _i4(bc), ctypes.c_double(kappa),
+                          ctypes.c_int(parity), ctypes.c_double(stop), ctypes.c_int(maxit), ctypes.c_int(kmax),
+                          ctypes.c_double(delta), ctypes.c_int(int(precond)), _blk(block), ctypes.c_int(n_mr),
+                          ctypes.c_double(omega_mr), ctypes.byref(it), ctypes.byref(rs), ctypes.byref(rn))
+    return x, dict(status=st, iterations=it.value, restarts=rs.value, residual_norm=rn.value)
+
+
+def invert(b, U, Tcl, bc, kappa, parity=0, tol=1e-12, maxit=10000, solver=BICGSTAB, kmax=16, delta=0.1,
+           block=None, n_mr=10, omega_mr=1.0):
+    """Full-lattice solve of M x = b (Eq. 1).  Returns (x, info)."""
+    b, U, Tcl = _c(b), _c(U), _c(Tcl)
+    x = np.zeros_like(b)
+    it, tr = ctypes.c_int(0), ctypes.c_double(0)
+    st = lib().orc_invert(_p(x), _p(b), _p(U), _p(Tcl), _i4(dims_of(b)), _i4(bc), ctypes.c_double(kappa),
+                          ctypes.c_int(parity), ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.c_int(solver),
+                          ctypes.c_int(kmax), ctypes.c_double(delta), _blk(block), ctypes.c_int(n_mr),
+                          ctypes.c_double(omega_mr), ctypes.byref(it), ctypes.byref(tr))
+    return x, dict(status=st, iterations=it.value, true_residual=tr.value)
