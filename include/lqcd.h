@@ -1,0 +1,176 @@
+/* lqcd.h -- C ABI of the B200-native Wilson-clover library (liblqcd_b200.so).
+ *
+ * The library computes what the solvers of arXiv:1109.2935 ("Scaling Lattice QCD beyond
+ * 100 GPUs", Babich et al., SC11) spend their time in.  Citations are lines of the paper
+ * text plus section / equation; "R<n>" are the readings listed in DESIGN.md
+ * for points on which the paper is silent.
+ *
+ *   problem           M x = b                                    PAPER.md:88-92  Sec. 2.1 Eq. 1
+ *   operator          M = A(kappa) - kappa D,  A = 1 + kappa T   PAPER.md:98-108 Sec. 2.2 Eq. 2 (R1-R4)
+ *   even-odd          Mhat = A_pp - kappa^2 D A^-1 D             PAPER.md:128    Sec. 3.1     (R6)
+ *   solvers           mixed-precision BiCGstab
+ *                     GCR-DD (Algorithm 1) + additive Schwarz/MR PAPER.md:146, :248-292 Sec. 8.1
+ *
+ * Conventions
+ *   - Unless a function says "host", every field pointer is a DEVICE pointer owned by the
+ *     caller (e.g. a PyTorch tensor).  The library never frees or reallocates caller memory.
+ *     The library owns the context, its packed gauge / clover copies and solver workspace;
+ *     lqcd_destroy frees them.
+ *   - `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  Calls are
+ *     stream-ordered and asynchronous, except lqcd_invert and the *_host calls, which
+ *     synchronise the stream before returning.
+ *   - Every function returns 0 (LQCD_OK) or a negative error code; nothing is printed, no
+ *     exception crosses the ABI, nothing aborts.  lqcd_last_error gives the text.
+ *   - A context is used from one host thread at a time.
+ *
+ * Canonical (external) layouts, C-contiguous complex128 (interleaved re, im):
+ *   gauge   U[mu][t][z][y][x][row][col]  mu = 0:x 1:y 2:z 3:t.  U_mu(x) multiplies psi(x+mu)
+ *           in Eq. 2.  Links carry NO boundary signs.
+ *   spinor  psi[t][z][y][x][spin][colour]   DeGrand-Rossi chiral gamma basis (R2):
+ *           gamma5 = diag(1,1,-1,-1).
+ * Packed (internal) layouts are private: even-odd checkerboarded structure-of-arrays, one
+ * parity per field; their size is queried with lqcd_field_bytes.  A packed field of one
+ * precision is only meaningful to calls with the same `prec`.
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx;
+
+/* error codes */
+#define LQCD_OK          0
+#define LQCD_EINVAL     (-1)   /* bad argument: null pointer, odd extent, bad enum, block not dividing dims */
+#define LQCD_ESTATE     (-2)   /* call order: dslash before load_gauge, matpc before build_clover, c_sw mismatch */
+#define LQCD_ENOMEM     (-3)
+#define LQCD_ECUDA      (-4)   /* a CUDA call failed; text in lqcd_last_error */
+#define LQCD_ENOCONV    (-5)   /* max_iter reached */
+#define LQCD_EBREAKDOWN (-6)   /* BiCGstab rho/omega breakdown or NaN */
+
+/* storage precisions.  HALF = int16 fixed point with one fp32 norm per site
+ * (PAPER.md:164 (c): "custom 16-bit fixed-point storage format"; R9); arithmetic in fp32. */
+#define LQCD_PREC_DOUBLE 0
+#define LQCD_PREC_SINGLE 1
+#define LQCD_PREC_HALF   2
+
+/* gauge-link compression (PAPER.md:164 (a): 18 -> 12 or 8 reals per link) */
+#define LQCD_RECON_18 18
+#define LQCD_RECON_12 12
+#define LQCD_RECON_8   8
+
+#define LQCD_SOLVER_BICGSTAB 0
+#define LQCD_SOLVER_GCR_DD   1
+
+#define LQCD_FIELD_SPINOR_PARITY 0
+
+/* Create a context for a lattice dims = (X,Y,Z,T), all even and >= 2, with per-direction
+ * boundary condition boundary[mu] = +1 periodic / -1 antiperiodic (R5).  `device` is the
+ * CUDA device ordinal.  Host pointers. */
+int lqcd_create(lqcd_ctx** ctx, const int dims[4], const int boundary[4], int device);
+int lqcd_destroy(lqcd_ctx* ctx);
+const char* lqcd_last_error(const lqcd_ctx* ctx);
+
+/* Load the gauge field (canonical layout, device pointer, 4*V*9 complex128).  Packs the
+ * checkerboarded fp64 / recon-18 copy immediately; other precision x compression copies are
+ * derived from it on first use.  Invalidates a previously built clover term. */
+int lqcd_load_gauge(lqcd_ctx* ctx, const void* U_canonical, void* stream);
+
+/* Build the clover term T_x = c_sw * sum_{mu<nu} (i sigma_munu) (x) F_munu(x) with the
+ * four-leaf field strength (fn.1 :138; R4), kappa-independent, stored as
+ * two Hermitian 6x6 chiral blocks = 72 reals per site. */
+int lqcd_build_clover(lqcd_ctx* ctx, double c_sw, void* stream);
+
+/* Bytes of one packed field of `kind` in precision `prec`. */
+size_t lqcd_field_bytes(const lqcd_ctx* ctx, int kind, int prec);
+
+/* canonical (full lattice, complex128) <-> packed (one parity, `prec`).  pack reads only the
+ * sites of `parity`; unpack writes only those sites and leaves the others untouched. */
+int lqcd_pack_spinor(lqcd_ctx* ctx, void* packed, const void* canonical, int parity, int prec, void* stream);
+int lqcd_unpack_spinor(lqcd_ctx* ctx, void* canonical, const void* packed, int parity, int prec, void* stream);
+
+/* out_p = D_{p,pbar} in_pbar : the hopping term of Eq. 2, no kappa, no
+ * clover; `in` is a packed field of parity 1-parity_out, `out` of parity parity_out;
+ * dagger != 0 applies D^dagger.  Nominal 1320 flop per output site.  out must not alias in. */
+int lqcd_dslash(lqcd_ctx* ctx, void* out, const void* in, int parity_out, int dagger,
+                int prec, int recon, void* stream);
+
+/* out = A in (inverse == 0) or A^-1 in, A = 1 + kappa T on sites of `parity`.  504 flop/site. */
+int lqcd_clover(lqcd_ctx* ctx, void* out, const void* in, int parity, int inverse,
+                double kappa, int prec, void* stream);
+
+/* out = Mhat in on `parity` (R6): two fused launches
+ *   tmp = A^-1_{pbar pbar} D_{pbar p} in ;  out = A_pp in - kappa^2 D_{p pbar} tmp.
+ * 3696 flop per site.  out must not alias in. */
+int lqcd_matpc(lqcd_ctx* ctx, void* out, const void* in, int parity, int dagger,
+               double kappa, int prec, int recon, void* stream);
+
+/* Schwarz preconditioner K (R7): out = K in on `parity`, n_mr
+ * minimum-residual steps on the Dirichlet-cut Mhat_D with one alpha per block.  in/out are
+ * packed fields (natural layout) of precision `prec_io`; the MR iteration itself runs in
+ * `prec` on block-major copies. */
+int lqcd_schwarz(lqcd_ctx* ctx, void* out, const void* in, int parity, double kappa,
+                 const int block[4], int n_mr, double omega_mr, int prec, int recon,
+                 int prec_io, void* stream);
+
+typedef struct {
+  double kappa;
+  double c_sw;            /* must equal the value given to lqcd_build_clover */
+  double tol;             /* stop on ||b - M x|| <= tol * ||b||  (full system) */
+  double delta;           /* BiCGstab: reliable-update trigger; GCR: early restart (Alg. 1) */
+  int    max_iter;
+  int    solver;          /* LQCD_SOLVER_* */
+  int    prec_outer, prec_sloppy, prec_precond;
+  int    recon_outer, recon_sloppy, recon_precond;
+  int    parity;          /* parity on which the Schur system is solved */
+  int    gcr_kmax;        /* restart length (16) */
+  int    schwarz_block[4];/* e.g. 12,12,12,24; extents even, dividing dims */
+  int    mr_steps;        /* 10 */
+  double mr_omega;        /* 1.0 */
+  int    use_initial_guess;
+  int    precondition;    /* GCR: 1 = Schwarz/MR preconditioner, 0 = plain GCR */
+} lqcd_invert_params;
+
+typedef struct {
+  int    status;          /* LQCD_OK, LQCD_ENOCONV, LQCD_EBREAKDOWN */
+  int    iterations;      /* BiCGstab iterations / GCR outer iterations */
+  int    restarts;        /* reliable updates (BiCGstab) or restarts (GCR) */
+  int    matpc_sloppy, matpc_outer, matpc_precond;   /* operator applications by precision */
+  double true_residual;   /* ||bhat - Mhat x_p|| / ||b|| in fp64 = ||b - M x|| / ||b|| */
+  double iterated_residual;
+  double seconds;         /* device time of the whole call (CUDA events) */
+  double gflop;           /* nominal flops executed (operators 3696/site + BLAS-1) / 1e9 */
+} lqcd_invert_result;
+
+/* Solve M x = b on the full lattice (Eq. 1): source preparation, parity solve of the Schur
+ * system, reconstruction of the other parity.  x and b are canonical full-lattice DEVICE
+ * arrays.  Synchronises `stream`. */
+int lqcd_invert(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical,
+                const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
+
+/* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */
+/* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned or pageable).
+ * out = D in on both parities (op == 0) or out_p = Mhat in_p on `parity`, rest zero (op == 1),
+ * computed in (prec, recon).  Synchronises `stream`. */
+int lqcd_apply_host(lqcd_ctx* ctx, void* out_host, const void* in_host, int op, int parity, int dagger,
+                    double kappa, int prec, int recon, void* stream);
+int lqcd_invert_host(lqcd_ctx* ctx, void* x_host, const void* b_host,
+                     const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
+
+/* ---- fused BLAS-1 on packed fields, exported for tests and the bench ---- */
+/* y += a*x ; returns ||y||^2 in *norm2_host after a stream sync (host pointer). */
+int lqcd_axpy_norm(lqcd_ctx* ctx, double a, const void* x, void* y, int prec, double* norm2_host, void* stream);
+/* <x,y> = sum conj(x) y -> dot_host[0..1] (re, im). */
+int lqcd_cdot(lqcd_ctx* ctx, const void* x, const void* y, int prec, double* dot_host, void* stream);
+
+/* number of kernel launches issued by this context since creation (bench: gpu_launches) */
+long long lqcd_launch_count(const lqcd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

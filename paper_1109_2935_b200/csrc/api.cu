@@ -1,0 +1,313 @@
+// api.cu -- C ABI entry points of include/lqcd.h: context, field management, operators.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include "ops.h"
+
+using namespace lq;
+
+namespace lq {
+
+int fail(lqcd_ctx* c, int code, const char* what, cudaError_t e) {
+  if (c) {
+    c->err = what;
+    if (e != cudaSuccess) { c->err += ": "; c->err += cudaGetErrorString(e); }
+  }
+  return code;
+}
+
+static Geom make_geom(const int* X, const int* bc, int nb) {
+  Geom g;
+  for (int m = 0; m < 4; ++m) { g.X[m] = X[m]; g.bc[m] = bc[m]; }
+  g.Xh = X[0] / 2;
+  g.vh = X[0] * X[1] * X[2] * X[3] / 2;
+  g.nb = nb;
+  g.ns = (long long)nb * g.vh;
+  return g;
+}
+
+int dev_alloc(lqcd_ctx* c, void** p, size_t bytes) {
+  cudaError_t e = cudaMalloc(p, bytes);
+  if (e != cudaSuccess) { *p = nullptr; return fail(c, LQCD_ENOMEM, "cudaMalloc", e); }
+  return LQCD_OK;
+}
+
+static void free_p(char*& p) { if (p) cudaFree(p); p = nullptr; }
+
+static void drop_clover_copies(lqcd_ctx* c) {
+  for (int i = 0; i < 3; ++i) { free_p(c->clov[i]); free_p(c->clovinv[i]); free_p(c->bclov[i]); free_p(c->bclovinv[i]); }
+  c->kappa = NAN;
+}
+static void drop_block_copies(lqcd_ctx* c) {
+  for (int i = 0; i < 3; ++i) {
+    for (int r = 0; r < 3; ++r) free_p(c->bgauge[i][r]);
+    free_p(c->bclov[i]); free_p(c->bclovinv[i]); free_p(c->btmp[i]);
+  }
+  c->have_blocks = false;
+}
+static void drop_gauge_copies(lqcd_ctx* c) {
+  for (int i = 0; i < 3; ++i) for (int r = 0; r < 3; ++r) { free_p(c->gauge[i][r]); free_p(c->bgauge[i][r]); }
+}
+
+int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, cudaStream_t s) {
+  const int ri = recon_index(recon);
+  if (prec < 0 || prec > 2 || ri < 0) return fail(c, LQCD_EINVAL, "bad precision / recon");
+  if (!c->have_gauge) return fail(c, LQCD_ESTATE, "gauge field not loaded");
+  if (blocked && !c->have_blocks) return fail(c, LQCD_ESTATE, "no Schwarz blocking set");
+  char*& slot = blocked ? c->bgauge[prec][ri] : c->gauge[prec][ri];
+  if (!slot) {
+    int rc = dev_alloc(c, (void**)&slot, gauge_bytes(prec, recon, c->nat.ns));
+    if (rc) return rc;
+    cudaError_t e = run_convert_gauge(prec, recon, slot, c->g64, c->bm, blocked ? 1 : 0, s);
+    c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "convert_gauge", e);
+  }
+  *out = slot;
+  return LQCD_OK;
+}
+
+int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A, const char** Ainv, cudaStream_t s) {
+  if (prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "bad precision");
+  if (!c->have_clover) return fail(c, LQCD_ESTATE, "clover term not built");
+  if (blocked && !c->have_blocks) return fail(c, LQCD_ESTATE, "no Schwarz blocking set");
+  if (!(c->kappa == kappa)) { drop_clover_copies(c); c->kappa = kappa; }
+  char*& a = blocked ? c->bclov[prec] : c->clov[prec];
+  char*& ai = blocked ? c->bclovinv[prec] : c->clovinv[prec];
+  if (!a) {
+    int rc = dev_alloc(c, (void**)&a, clover_bytes(prec, c->nat.ns));
+    if (rc) return rc;
+    rc = dev_alloc(c, (void**)&ai, clover_bytes(prec, c->nat.ns));
+    if (rc) return rc;
+    cudaError_t e = run_clover_make(prec, a, ai, c->T72, c->bm, blocked ? 1 : 0, kappa, s);
+    c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_make", e);
+  }
+  *A = a; *Ainv = ai;
+  return LQCD_OK;
+}
+
+int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out) {
+  char*& t = blocked ? c->btmp[prec] : c->tmp[prec];
+  if (!t) { int rc = dev_alloc(c, (void**)&t, spinor_bytes(prec, c->nat.ns)); if (rc) return rc; }
+  *out = t;
+  return LQCD_OK;
+}
+
+int set_blocks(lqcd_ctx* c, const int* blk) {
+  if (!blk) return fail(c, LQCD_EINVAL, "null block");
+  for (int m = 0; m < 4; ++m)
+    if (blk[m] < 2 || (blk[m] & 1) || c->dims[m] % blk[m]) return fail(c, LQCD_EINVAL, "Schwarz block extents must be even and divide the lattice");
+  if (c->have_blocks && !memcmp(blk, c->bm.blk.X, 4 * sizeof(int))) return LQCD_OK;
+  drop_block_copies(c);
+  int nb = 1, bcb[4];
+  for (int m = 0; m < 4; ++m) {
+    c->bm.nbd[m] = c->dims[m] / blk[m];
+    nb *= c->bm.nbd[m];
+    bcb[m] = (c->bm.nbd[m] == 1) ? c->bc[m] : 0;    // unpartitioned direction keeps its wrap (R7)
+  }
+  c->bm.nat = c->nat;
+  c->bm.blk = make_geom(blk, bcb, nb);
+  c->have_blocks = true;
+  const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * 4;
+  if (need > c->boxdots_doubles) {
+    if (c->boxdots) cudaFree(c->boxdots);
+    c->boxdots = nullptr; c->boxdots_doubles = 0;
+    int rc = dev_alloc(c, (void**)&c->boxdots, need * sizeof(double));
+    if (rc) return rc;
+    c->boxdots_doubles = need;
+  }
+  return LQCD_OK;
+}
+
+// out = [C] ([A] y + a * D in) : one fused launch (dslash.cuh)
+int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
+              int epi, double a, double kappa, bool blocked, cudaStream_t s) {
+  DslashArgs d;
+  memset(&d, 0, sizeof(d));
+  d.g = blocked ? c->bm.blk : c->nat;
+  d.out = out; d.in = in; d.y = y; d.a = a; d.parity = parity_out; d.dagger = dagger;
+  int rc = get_gauge(c, prec, recon, blocked, &d.gauge, s);
+  if (rc) return rc;
+  if (epi != EPI_NONE && epi != EPI_XPAY) {
+    const char *A, *Ai;
+    rc = get_clover(c, prec, kappa, blocked, &A, &Ai, s);
+    if (rc) return rc;
+    d.clov_y = A; d.clov_out = Ai;
+  }
+  d.dots = c->boxdots;
+  cudaError_t e;
+  switch (prec) {
+    case 0: e = launch_dslash<PrecD>(d, recon, epi, s); break;
+    case 1: e = launch_dslash<PrecS>(d, recon, epi, s); break;
+    case 2: e = launch_dslash<PrecH>(d, recon, epi, s); break;
+    default: return fail(c, LQCD_EINVAL, "bad precision");
+  }
+  c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dslash launch", e);
+  return LQCD_OK;
+}
+
+// out = Mhat in  (R6):  tmp = A^-1 D in ;  out = A in - kappa^2 D tmp
+int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
+             bool blocked, bool dots, cudaStream_t s) {
+  char* tmp;
+  int rc = get_tmp(c, prec, blocked, &tmp);
+  if (rc) return rc;
+  rc = op_dslash(c, tmp, in, nullptr, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, blocked, s);
+  if (rc) return rc;
+  return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, dots ? EPI_CLOVX_XPAY_DOTS : EPI_CLOVX_XPAY,
+                   -kappa * kappa, kappa, blocked, s);
+}
+
+}  // namespace lq
+
+// ================================================================================================
+extern "C" {
+
+int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int device) {
+  if (!out || !dims || !boundary) return LQCD_EINVAL;
+  *out = nullptr;
+  for (int m = 0; m < 4; ++m) {
+    if (dims[m] < 2 || (dims[m] & 1)) return LQCD_EINVAL;
+    if (boundary[m] != 1 && boundary[m] != -1) return LQCD_EINVAL;
+  }
+  if ((long long)dims[0] * dims[1] * dims[2] * dims[3] / 2 > 0x7fffffffLL) return LQCD_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LQCD_ECUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return LQCD_ECUDA;
+  lqcd_ctx* c = new (std::nothrow) lqcd_ctx();
+  if (!c) return LQCD_ENOMEM;
+  for (int m = 0; m < 4; ++m) { c->dims[m] = dims[m]; c->bc[m] = boundary[m]; }
+  c->device = device;
+  c->V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
+  c->Vh = c->V / 2;
+  c->nat = make_geom(dims, boundary, 1);
+  c->bm.nat = c->nat; c->bm.blk = c->nat; c->bm.nbd[0] = c->bm.nbd[1] = c->bm.nbd[2] = c->bm.nbd[3] = 1;
+  c->launches = 0;
+  c->have_gauge = c->have_blocks = c->have_clover = false;
+  c->g64 = nullptr; c->T72 = nullptr; c->kappa = NAN; c->c_sw = NAN;
+  memset(c->gauge, 0, sizeof(c->gauge)); memset(c->bgauge, 0, sizeof(c->bgauge));
+  memset(c->clov, 0, sizeof(c->clov)); memset(c->clovinv, 0, sizeof(c->clovinv));
+  memset(c->bclov, 0, sizeof(c->bclov)); memset(c->bclovinv, 0, sizeof(c->bclovinv));
+  memset(c->tmp, 0, sizeof(c->tmp)); memset(c->btmp, 0, sizeof(c->btmp));
+  c->S = nullptr; c->partials = nullptr; c->counters = nullptr; c->boxdots = nullptr; c->hS = nullptr;
+  c->boxdots_doubles = 0;
+  cudaDeviceProp prop;
+  cudaGetDeviceProperties(&prop, device);
+  c->n_sm = prop.multiProcessorCount;
+  c->partials_doubles = (size_t)c->n_sm * 8 * 16 + 4096;
+  bool ok = cudaMalloc((void**)&c->S, S_TOTAL * sizeof(double)) == cudaSuccess &&
+            cudaMalloc((void**)&c->partials, c->partials_doubles * sizeof(double)) == cudaSuccess &&
+            cudaMalloc((void**)&c->counters, 4096 * sizeof(unsigned)) == cudaSuccess &&
+            cudaMallocHost((void**)&c->hS, S_TOTAL * sizeof(double)) == cudaSuccess;
+  if (ok) ok = cudaMemset(c->S, 0, S_TOTAL * sizeof(double)) == cudaSuccess &&
+               cudaMemset(c->counters, 0, 4096 * sizeof(unsigned)) == cudaSuccess;
+  if (!ok) { lqcd_destroy(c); return LQCD_ENOMEM; }
+  *out = c;
+  return LQCD_OK;
+}
+
+int lqcd_destroy(lqcd_ctx* c) {
+  if (!c) return LQCD_EINVAL;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  drop_gauge_copies(c); drop_clover_copies(c); drop_block_copies(c);
+  for (int i = 0; i < 3; ++i) free_p(c->tmp[i]);
+  if (c->g64) cudaFree(c->g64);
+  if (c->T72) cudaFree(c->T72);
+  if (c->S) cudaFree(c->S);
+  if (c->partials) cudaFree(c->partials);
+  if (c->counters) cudaFree(c->counters);
+  if (c->boxdots) cudaFree(c->boxdots);
+  if (c->hS) cudaFreeHost(c->hS);
+  for (void* p : c->pool) cudaFree(p);
+  delete c;
+  return LQCD_OK;
+}
+
+const char* lqcd_last_error(const lqcd_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+long long lqcd_launch_count(const lqcd_ctx* c) { return c ? c->launches : 0; }
+
+int lqcd_load_gauge(lqcd_ctx* c, const void* U, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!U) return fail(c, LQCD_EINVAL, "null gauge pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaSetDevice(c->device);
+  drop_gauge_copies(c); drop_clover_copies(c);
+  c->have_clover = false;
+  if (!c->g64) { int rc = dev_alloc(c, (void**)&c->g64, gauge_bytes(0, 18, c->nat.ns)); if (rc) return rc; }
+  cudaError_t e = run_pack_gauge(c->g64, (const double*)U, c->nat, s);
+  c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack_gauge", e);
+  c->have_gauge = true;
+  return LQCD_OK;
+}
+
+int lqcd_build_clover(lqcd_ctx* c, double c_sw, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!c->have_gauge) return fail(c, LQCD_ESTATE, "build_clover before load_gauge");
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaSetDevice(c->device);
+  drop_clover_copies(c);
+  if (!c->T72) { int rc = dev_alloc(c, (void**)&c->T72, (size_t)c->nat.ns * 2 * 576); if (rc) return rc; }
+  cudaError_t e = run_clover_term(c->T72, c->g64, c->nat, c_sw, s);
+  c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_term", e);
+  c->c_sw = c_sw;
+  c->have_clover = true;
+  return LQCD_OK;
+}
+
+size_t lqcd_field_bytes(const lqcd_ctx* c, int kind, int prec) {
+  if (!c || kind != LQCD_FIELD_SPINOR_PARITY || prec < 0 || prec > 2) return 0;
+  return spinor_bytes(prec, c->nat.ns);
+}
+
+int lqcd_pack_spinor(lqcd_ctx* c, void* packed, const void* canonical, int parity, int prec, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!packed || !canonical || (parity | 1) != 1 || prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "pack_spinor arguments");
+  cudaSetDevice(c->device);
+  cudaError_t e = run_pack_spinor(prec, (char*)packed, (const double*)canonical, c->nat, parity, 0, (cudaStream_t)stream);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "pack_spinor", e);
+}
+
+int lqcd_unpack_spinor(lqcd_ctx* c, void* canonical, const void* packed, int parity, int prec, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!packed || !canonical || (parity | 1) != 1 || prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "unpack_spinor arguments");
+  cudaSetDevice(c->device);
+  cudaError_t e = run_pack_spinor(prec, (char*)packed, (const double*)canonical, c->nat, parity, 1, (cudaStream_t)stream);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "unpack_spinor", e);
+}
+
+int lqcd_dslash(lqcd_ctx* c, void* out, const void* in, int parity_out, int dagger, int prec, int recon, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity_out | 1) != 1) return fail(c, LQCD_EINVAL, "dslash arguments");
+  cudaSetDevice(c->device);
+  return op_dslash(c, (char*)out, (const char*)in, nullptr, parity_out, dagger ? 1 : 0, prec, recon, EPI_NONE, 0.0, 0.0,
+                   false, (cudaStream_t)stream);
+}
+
+int lqcd_clover(lqcd_ctx* c, void* out, const void* in, int parity, int inverse, double kappa, int prec, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || (parity | 1) != 1) return fail(c, LQCD_EINVAL, "clover arguments");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  const char *A, *Ai;
+  int rc = get_clover(c, prec, kappa, false, &A, &Ai, s);
+  if (rc) return rc;
+  cudaError_t e = run_clover_apply(prec, (char*)out, (const char*)in, inverse ? Ai : A, c->nat, parity, s);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "clover_apply", e);
+}
+
+int lqcd_matpc(lqcd_ctx* c, void* out, const void* in, int parity, int dagger, double kappa, int prec, int recon, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity | 1) != 1) return fail(c, LQCD_EINVAL, "matpc arguments");
+  cudaSetDevice(c->device);
+  return op_matpc(c, (char*)out, (const char*)in, parity, dagger ? 1 : 0, kappa, prec, recon, false, false, (cudaStream_t)stream);
+}
+
+}  // extern "C"

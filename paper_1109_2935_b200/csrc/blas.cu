@@ -1,0 +1,207 @@
+// blas.cu -- launchers for the fused BLAS-1 passes (blas_ops.cuh), the multi-vector GCR
+// orthogonalisation kernels (Algorithm 1) and the mixed-precision
+// convert / accumulate kernels used at reliable updates and GCR restarts.
+#include "blas_ops.cuh"
+#include "host.h"
+
+namespace lq {
+
+template <class Op>
+cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s) {
+  int gx = (a.vh + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK;
+  if (gx > max_ctas) gx = max_ctas;
+  if (gx < 1) gx = 1;
+  dim3 grid(gx, a.nb), block(LQ_BLAS_BLOCK);
+  switch (prec) {
+    case 0: blas_kernel<PrecD, Op><<<grid, block, 0, s>>>(a); break;
+    case 1: blas_kernel<PrecS, Op><<<grid, block, 0, s>>>(a); break;
+    case 2: blas_kernel<PrecH, Op><<<grid, block, 0, s>>>(a); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+#define LQ_INST(OP) template cudaError_t run_blas<OP>(int, const BlasArgs&, int, cudaStream_t);
+LQ_INST(OpZero) LQ_INST(OpNorm2) LQ_INST(OpCdot) LQ_INST(OpAxpyNorm) LQ_INST(OpXmyNorm)
+LQ_INST(OpBicgInit) LQ_INST(OpBicgP) LQ_INST(OpBicgAlpha) LQ_INST(OpBicgS) LQ_INST(OpBicgOmega) LQ_INST(OpBicgXR)
+LQ_INST(OpGcrScale)
+typedef OpMrUpdate<true, false> OpMrFirst;
+typedef OpMrUpdate<false, false> OpMrMid;
+typedef OpMrUpdate<false, true> OpMrLast;
+typedef OpMrUpdate<true, true> OpMrOnly;
+LQ_INST(OpMrFirst) LQ_INST(OpMrMid) LQ_INST(OpMrLast) LQ_INST(OpMrOnly)
+#undef LQ_INST
+
+// ---------------------------------------------------------------- GCR multi-vector kernels
+// beta_{i,k} = <z_i, z_k> for i in [i0, i0+n), n <= 8, one pass over z_k and the n vectors.
+template <class P>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_dots_kernel(const MultiArgs m) {
+  typedef typename P::real R;
+  const BlasArgs& a = m.b;
+  double red[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) red[k] = 0;
+  for (int cb = blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x; cb < a.vh; cb += gridDim.x * LQ_BLAS_BLOCK) {
+    R zk[24];
+    load_site<P, 24>(zk, m.z[m.k], a.ns, cb);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      if (j < m.n) {
+        R zi[24];
+        load_site<P, 24>(zi, m.z[m.i0 + j], a.ns, cb);
+        site_cdot(zi, zk, red[2 * j], red[2 * j + 1]);
+      }
+    }
+  }
+  reduce_and_finalize<16>(red, a, 0, [&](const double* s) {
+    for (int j = 0; j < m.n; ++j) {
+      double* b = a.S + S_GCR_BETA + 2 * ((m.i0 + j) * LQ_GCR_KMAX + m.k);
+      b[0] = s[2 * j]; b[1] = s[2 * j + 1];
+    }
+  });
+}
+
+// z_k -= sum_{i<k} beta_{i,k} z_i ; then zz = ||z_k||^2, zr = <z_k, rhat> ;
+// last CTA: gamma_k = sqrt(zz), alpha_k = zr / gamma_k  (Algorithm 1)
+template <class P>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_orth_kernel(const MultiArgs m) {
+  typedef typename P::real R;
+  const BlasArgs& a = m.b;
+  double red[3] = {0, 0, 0};
+  for (int cb = blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x; cb < a.vh; cb += gridDim.x * LQ_BLAS_BLOCK) {
+    R zk[24], r[24];
+    load_site<P, 24>(zk, m.z[m.k], a.ns, cb);
+    for (int i = 0; i < m.k; ++i) {
+      R zi[24];
+      load_site<P, 24>(zi, m.z[i], a.ns, cb);
+      const double* b = a.S + S_GCR_BETA + 2 * (i * LQ_GCR_KMAX + m.k);
+      site_caxpy<R>((R)(-b[0]), (R)(-b[1]), zi, zk);
+    }
+    if (m.k > 0) store_site<P, 24>(zk, (char*)m.z[m.k], a.ns, cb);
+    load_site<P, 24>(r, a.v[0], a.ns, cb);
+    site_norm2(zk, red[0]);
+    site_cdot(zk, r, red[1], red[2]);
+  }
+  reduce_and_finalize<3>(red, a, 0, [&](const double* s) {
+    double* S = a.S;
+    const double gamma = sqrt(s[0]);
+    S[S_GCR_ZZ] = s[0];
+    S[S_GCR_GAMMA] = gamma;
+    S[S_GCR_ALPHA] = s[1] / gamma; S[S_GCR_ALPHA + 1] = s[2] / gamma;
+    S[S_GCR_GAMMAS + m.k] = gamma;
+    S[S_GCR_ALPHAS + 2 * m.k] = s[1] / gamma; S[S_GCR_ALPHAS + 2 * m.k + 1] = s[2] / gamma;
+  });
+}
+
+cudaError_t run_gcr_dots(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s) {
+  int gx = (m.b.vh + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK;
+  if (gx > max_ctas) gx = max_ctas;
+  dim3 grid(gx), block(LQ_BLAS_BLOCK);
+  switch (prec) {
+    case 0: gcr_dots_kernel<PrecD><<<grid, block, 0, s>>>(m); break;
+    case 1: gcr_dots_kernel<PrecS><<<grid, block, 0, s>>>(m); break;
+    case 2: gcr_dots_kernel<PrecH><<<grid, block, 0, s>>>(m); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s) {
+  int gx = (m.b.vh + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK;
+  if (gx > max_ctas) gx = max_ctas;
+  dim3 grid(gx), block(LQ_BLAS_BLOCK);
+  switch (prec) {
+    case 0: gcr_orth_kernel<PrecD><<<grid, block, 0, s>>>(m); break;
+    case 1: gcr_orth_kernel<PrecS><<<grid, block, 0, s>>>(m); break;
+    case 2: gcr_orth_kernel<PrecH><<<grid, block, 0, s>>>(m); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------- mixed precision
+// dst (PB) = src (PA), optionally permuting between the natural layout and the block-major
+// layout of the Schwarz preconditioner (dir: 0 none, 1 natural -> blocks, 2 blocks -> natural).
+template <class PA, class PB>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) convert_kernel(char* dst, const char* src, const BlockMap bm, int dir, int parity) {
+  const long long i = (long long)blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x;
+  if (i >= bm.nat.ns) return;
+  long long is = i, id = i;
+  if (dir != 0) {
+    const int box = (int)(i / bm.blk.vh), lcb = (int)(i % bm.blk.vh);
+    const long long n = block_to_natural(bm, box, lcb, parity);
+    if (dir == 1) { is = n; id = i; } else { is = i; id = n; }
+  }
+  typename PA::real va[24];
+  load_site<PA, 24>(va, src, bm.nat.ns, is);
+  typename PB::real vb[24];
+#pragma unroll
+  for (int k = 0; k < 24; ++k) vb[k] = (typename PB::real)va[k];
+  store_site<PB, 24>(vb, dst, bm.nat.ns, id);
+}
+
+// y (PH) += sum_{i<n} chi_i * x_i (PL)   (implicit solution update; and
+// x += x_lo at a reliable update with n = 1, chi = 1)
+template <class PH_, class PL_>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, const MultiArgs m) {
+  const long long i = (long long)blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x;
+  if (i >= m.b.ns) return;
+  typename PH_::real acc[24];
+  load_site<PH_, 24>(acc, y, m.b.ns, i);
+  for (int j = 0; j < m.n; ++j) {
+    typename PL_::real x[24];
+    load_site<PL_, 24>(x, m.z[j], m.b.ns, i);
+    const typename PH_::real cr = (typename PH_::real)m.chi[2 * j], ci = (typename PH_::real)m.chi[2 * j + 1];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+      const typename PH_::real xr = (typename PH_::real)x[2 * k], xi = (typename PH_::real)x[2 * k + 1];
+      acc[2 * k] += cr * xr - ci * xi;
+      acc[2 * k + 1] += cr * xi + ci * xr;
+    }
+  }
+  store_site<PH_, 24>(acc, y, m.b.ns, i);
+}
+
+template <class PA>
+static cudaError_t convert_b(int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s) {
+  dim3 grid((unsigned)((bm.nat.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK)), block(LQ_BLAS_BLOCK);
+  switch (pb) {
+    case 0: convert_kernel<PA, PrecD><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
+    case 1: convert_kernel<PA, PrecS><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
+    case 2: convert_kernel<PA, PrecH><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s) {
+  switch (pa) {
+    case 0: return convert_b<PrecD>(pb, dst, src, bm, dir, parity, s);
+    case 1: return convert_b<PrecS>(pb, dst, src, bm, dir, parity, s);
+    case 2: return convert_b<PrecH>(pb, dst, src, bm, dir, parity, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <class PH_>
+static cudaError_t accumulate_b(int pl, char* y, const MultiArgs& m, cudaStream_t s) {
+  dim3 grid((unsigned)((m.b.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK)), block(LQ_BLAS_BLOCK);
+  switch (pl) {
+    case 0: accumulate_kernel<PH_, PrecD><<<grid, block, 0, s>>>(y, m); break;
+    case 1: accumulate_kernel<PH_, PrecS><<<grid, block, 0, s>>>(y, m); break;
+    case 2: accumulate_kernel<PH_, PrecH><<<grid, block, 0, s>>>(y, m); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStream_t s) {
+  switch (ph) {
+    case 0: return accumulate_b<PrecD>(pl, y, m, s);
+    case 1: return accumulate_b<PrecS>(pl, y, m, s);
+    case 2: return accumulate_b<PrecH>(pl, y, m, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace lq

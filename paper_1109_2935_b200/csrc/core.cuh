@@ -1,0 +1,233 @@
+// core.cuh -- packed field records, precision traits, SU(3) link reconstruction.
+//
+// Data layout in HBM: every field is an even-odd checkerboarded
+// structure of arrays.  A record of N reals of storage type T (N*sizeof(T) bytes per site)
+// is split into 16-byte chunks (then one 8- and/or one 4-byte chunk); chunk k of all sites is
+// one contiguous plane, so a warp reading chunk k of 32 consecutive sites issues one fully
+// coalesced 512-byte (int4) request.  (PAPER.md:164, :180-186 and Figs. 2,3 describe the
+// same idea for Fermi with float2/float4 textures; the chunking here is sized for 128-bit
+// loads on sm_100a.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lq {
+
+// Geometry of one launch: a batch of `nb` independent 4-d boxes of extents X (one box = the
+// whole lattice for the global operator; one box = one Schwarz block for the Dirichlet
+// operator).  bc[mu]: +1 periodic, -1 antiperiodic, 0 open (hop dropped).
+struct Geom {
+  int X[4];
+  int Xh;          // X[0]/2
+  int bc[4];
+  int vh;          // sites of one parity in one box
+  int nb;          // boxes in the batch
+  long long ns;    // nb*vh = plane stride of every packed field
+};
+
+struct PrecD { typedef double store_t; typedef double real; static constexpr bool HALF = false; static constexpr int ID = 0; };
+struct PrecS { typedef float  store_t; typedef float  real; static constexpr bool HALF = false; static constexpr int ID = 1; };
+struct PrecH { typedef short  store_t; typedef float  real; static constexpr bool HALF = true;  static constexpr int ID = 2; };
+
+#define LQ_DEV __device__ __forceinline__
+
+template <typename V> LQ_DEV V ld_nc(const V* p) { return __ldg(p); }
+
+// ---------------------------------------------------------------- packed records
+template <typename T, int N>
+struct Rec {
+  static constexpr int BYTES = N * (int)sizeof(T);
+  static constexpr int N16 = BYTES / 16;
+  static constexpr int N8 = (BYTES % 16) / 8;
+  static constexpr int N4 = (BYTES % 8) / 4;
+  static constexpr int E16 = 16 / (int)sizeof(T), E8 = 8 / (int)sizeof(T), E4 = 4 / (int)sizeof(T);
+  static_assert(BYTES % 4 == 0, "record must be a multiple of 4 bytes");
+
+  LQ_DEV static void load(T* __restrict__ v, const char* __restrict__ base, long long ns, long long i) {
+#pragma unroll
+    for (int k = 0; k < N16; ++k) {
+      int4 t = ld_nc(reinterpret_cast<const int4*>(base + 16ll * k * ns) + i);
+      *reinterpret_cast<int4*>(v + k * E16) = t;
+    }
+    if (N8) {
+      int2 t = ld_nc(reinterpret_cast<const int2*>(base + 16ll * N16 * ns) + i);
+      *reinterpret_cast<int2*>(v + N16 * E16) = t;
+    }
+    if (N4) {
+      int t = ld_nc(reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i);
+      *reinterpret_cast<int*>(v + N16 * E16 + N8 * E8) = t;
+    }
+  }
+  LQ_DEV static void store(const T* __restrict__ v, char* __restrict__ base, long long ns, long long i) {
+#pragma unroll
+    for (int k = 0; k < N16; ++k)
+      reinterpret_cast<int4*>(base + 16ll * k * ns)[i] = *reinterpret_cast<const int4*>(v + k * E16);
+    if (N8) reinterpret_cast<int2*>(base + 16ll * N16 * ns)[i] = *reinterpret_cast<const int2*>(v + N16 * E16);
+    if (N4) reinterpret_cast<int*>(base + (16ll * N16 + 8ll * N8) * ns)[i] = *reinterpret_cast<const int*>(v + N16 * E16 + N8 * E8);
+  }
+};
+
+// bytes per site of a packed field of N reals (+ one fp32 norm per site in half precision)
+template <class P> __host__ __device__ constexpr int site_bytes(int n, bool with_norm) {
+  return n * (int)sizeof(typename P::store_t) + ((P::HALF && with_norm) ? 4 : 0);
+}
+
+#define LQ_FIXED_MAX 32767.0f
+#define LQ_FIXED_INV (1.0f / 32767.0f)
+
+// ---------------------------------------------------------------- site vectors with a norm (spinor: 24, clover: 72)
+// R9: half = int16 q_i = rint(v_i * 32767 / n), n = max_i |v_i| (fp32) per site; decode v_i = q_i * n/32767.
+template <class P, int N>
+LQ_DEV void load_site(typename P::real* __restrict__ v, const char* __restrict__ f, long long ns, long long i) {
+  if constexpr (!P::HALF) {
+    Rec<typename P::store_t, N>::load(v, f, ns, i);
+  } else {
+    alignas(16) short q[N];
+    Rec<short, N>::load(q, f, ns, i);
+    const float n = ld_nc(reinterpret_cast<const float*>(f + (long long)(2 * N) * ns) + i) * LQ_FIXED_INV;
+#pragma unroll
+    for (int k = 0; k < N; ++k) v[k] = (float)q[k] * n;
+  }
+}
+
+template <class P, int N>
+LQ_DEV void store_site(const typename P::real* __restrict__ v, char* __restrict__ f, long long ns, long long i) {
+  if constexpr (!P::HALF) {
+    Rec<typename P::store_t, N>::store(v, f, ns, i);
+  } else {
+    float m = 0.f;
+#pragma unroll
+    for (int k = 0; k < N; ++k) m = fmaxf(m, fabsf(v[k]));
+    const float sc = (m > 0.f) ? (LQ_FIXED_MAX / m) : 0.f;
+    alignas(16) short q[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) q[k] = (short)__float2int_rn(v[k] * sc);
+    Rec<short, N>::store(q, f, ns, i);
+    reinterpret_cast<float*>(f + (long long)(2 * N) * ns)[i] = m;
+  }
+}
+
+// ---------------------------------------------------------------- complex helpers on (re,im) pairs
+template <typename R> struct cx { R re, im; };
+template <typename R> LQ_DEV cx<R> cmul(cx<R> a, cx<R> b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+template <typename R> LQ_DEV cx<R> cmulc(cx<R> a, cx<R> b) { /* conj(a)*b */ return {a.re * b.re + a.im * b.im, a.re * b.im - a.im * b.re}; }
+template <typename R> LQ_DEV cx<R> conj_(cx<R> a) { return {a.re, -a.im}; }
+
+LQ_DEV void sincos_(float x, float* s, float* c) { __sincosf(x, s, c); }
+LQ_DEV void sincos_(double x, double* s, double* c) { sincos(x, s, c); }
+LQ_DEV float rsqrt_(float x) { return rsqrtf(x); }
+LQ_DEV double rsqrt_(double x) { return rsqrt(x); }
+LQ_DEV float sqrt_(float x) { return sqrtf(x); }
+LQ_DEV double sqrt_(double x) { return sqrt(x); }
+
+// ---------------------------------------------------------------- gauge links (PAPER.md:164 (a); R10)
+// u[18] = row-major 3x3 complex.  RECON 18: as stored.  12: rows 0,1 stored, row2 = conj(row0 x row1).
+// 8: a2,a3,b1,arg(a1),arg(c1) stored (the parametrisation of ref. [3] of the paper).
+template <class P, int RECON>
+LQ_DEV void load_link(typename P::real* __restrict__ u, const char* __restrict__ g, long long ns, long long i) {
+  typedef typename P::real R;
+  typedef typename P::store_t S;
+  alignas(16) S raw[RECON];
+  Rec<S, RECON>::load(raw, g, ns, i);
+  R v[RECON];
+  if constexpr (P::HALF) {
+#pragma unroll
+    for (int k = 0; k < RECON; ++k) v[k] = (float)raw[k] * LQ_FIXED_INV;
+    if constexpr (RECON == 8) { v[6] *= 3.14159265358979323846f; v[7] *= 3.14159265358979323846f; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < RECON; ++k) v[k] = raw[k];
+  }
+  if constexpr (RECON == 18) {
+#pragma unroll
+    for (int k = 0; k < 18; ++k) u[k] = v[k];
+  } else if constexpr (RECON == 12) {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) u[k] = v[k];
+  } else {
+    const cx<R> a2 = {v[0], v[1]}, a3 = {v[2], v[3]}, b1 = {v[4], v[5]};
+    const R N = a2.re * a2.re + a2.im * a2.im + a3.re * a3.re + a3.im * a3.im;
+    R s1, c1, s2, c2;
+    sincos_(v[6], &s1, &c1);
+    sincos_(v[7], &s2, &c2);
+    const R a1m2 = fmax(R(0), R(1) - N);
+    const R a1m = sqrt_(a1m2);
+    const cx<R> a1 = {a1m * c1, a1m * s1};
+    const R c1m = sqrt_(fmax(R(0), R(1) - a1m2 - b1.re * b1.re - b1.im * b1.im));
+    const cx<R> cc1 = {c1m * c2, c1m * s2};
+    const R iN = R(1) / N;
+    const cx<R> p = cmulc(a1, b1);        // conj(a1) b1
+    const cx<R> q = cmulc(a1, cc1);       // conj(a1) c1
+    // b2 = -(p a2 + conj(c1) conj(a3))/N ; b3 = (-p a3 + conj(c1) conj(a2))/N
+    // c2 = (-q a2 + conj(b1) conj(a3))/N ; c3 = -(q a3 + conj(b1) conj(a2))/N
+    const cx<R> pa2 = cmul(p, a2), pa3 = cmul(p, a3), qa2 = cmul(q, a2), qa3 = cmul(q, a3);
+    const cx<R> c1a3 = conj_(cmul(cc1, a3)), c1a2 = conj_(cmul(cc1, a2));
+    const cx<R> b1a3 = conj_(cmul(b1, a3)), b1a2 = conj_(cmul(b1, a2));
+    u[0] = a1.re; u[1] = a1.im; u[2] = a2.re; u[3] = a2.im; u[4] = a3.re; u[5] = a3.im;
+    u[6] = b1.re; u[7] = b1.im;
+    u[8] = -(pa2.re + c1a3.re) * iN;  u[9] = -(pa2.im + c1a3.im) * iN;
+    u[10] = (c1a2.re - pa3.re) * iN;  u[11] = (c1a2.im - pa3.im) * iN;
+    u[12] = cc1.re; u[13] = cc1.im;
+    u[14] = (b1a3.re - qa2.re) * iN;  u[15] = (b1a3.im - qa2.im) * iN;
+    u[16] = -(qa3.re + b1a2.re) * iN; u[17] = -(qa3.im + b1a2.im) * iN;
+  }
+  if constexpr (RECON == 12) {
+    // row2 = conj(row0 x row1)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int j = (c + 1) % 3, k = (c + 2) % 3;
+      const R re = (u[2 * j] * u[6 + 2 * k] - u[2 * j + 1] * u[6 + 2 * k + 1]) - (u[2 * k] * u[6 + 2 * j] - u[2 * k + 1] * u[6 + 2 * j + 1]);
+      const R im = (u[2 * j] * u[6 + 2 * k + 1] + u[2 * j + 1] * u[6 + 2 * k]) - (u[2 * k] * u[6 + 2 * j + 1] + u[2 * k + 1] * u[6 + 2 * j]);
+      u[12 + 2 * c] = re;
+      u[12 + 2 * c + 1] = -im;
+    }
+  }
+}
+
+// Encode a full fp64 link into the stored RECON form (setup path, fp64 arithmetic).
+template <int RECON>
+LQ_DEV void compress_link(const double* __restrict__ u, double* __restrict__ v) {
+  if constexpr (RECON == 18) {
+#pragma unroll
+    for (int k = 0; k < 18; ++k) v[k] = u[k];
+  } else if constexpr (RECON == 12) {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) v[k] = u[k];
+  } else {
+    v[0] = u[2]; v[1] = u[3]; v[2] = u[4]; v[3] = u[5]; v[4] = u[6]; v[5] = u[7];
+    v[6] = atan2(u[1], u[0]);
+    v[7] = atan2(u[13], u[12]);
+  }
+}
+
+// convert RECON stored reals (fp64 values) into storage type of precision P
+template <class P, int RECON>
+LQ_DEV void quantize_link(const double* __restrict__ v, typename P::store_t* __restrict__ q) {
+  if constexpr (!P::HALF) {
+#pragma unroll
+    for (int k = 0; k < RECON; ++k) q[k] = (typename P::store_t)v[k];
+  } else {
+#pragma unroll
+    for (int k = 0; k < RECON; ++k) {
+      double x = v[k];
+      if (RECON == 8 && k >= 6) x *= (1.0 / 3.14159265358979323846);
+      x = fmin(1.0, fmax(-1.0, x));
+      q[k] = (short)__double2int_rn(x * 32767.0);
+    }
+  }
+}
+
+// ---------------------------------------------------------------- index arithmetic
+// Checkerboard index of one box: cb = xh + Xh*(y + Y*(z + Z*t)),  x = 2*xh + ((y+z+t+parity)&1).
+LQ_DEV void cb_to_coords(const Geom& g, int cb, int parity, int c[4]) {
+  int xh = cb % g.Xh; int r = cb / g.Xh;
+  c[1] = r % g.X[1]; r /= g.X[1];
+  c[2] = r % g.X[2];
+  c[3] = r / g.X[2];
+  c[0] = 2 * xh + ((c[1] + c[2] + c[3] + parity) & 1);
+}
+LQ_DEV int coords_to_cb(const Geom& g, const int c[4]) {
+  return (c[0] >> 1) + g.Xh * (c[1] + g.X[1] * (c[2] + g.X[2] * c[3]));
+}
+
+}  // namespace lq

@@ -1,0 +1,275 @@
+// dslash.cuh -- the Wilson-clover hopping term with fused clover / xpay epilogues.
+//
+// Computes, for every site x of parity p of every box in the batch (Eq. 2;
+// readings R1,R2,R5 in DESIGN.md):
+//
+//   r(x) = sum_mu [ s+ (1 -/+ g_mu) U_mu(x) in(x+mu) + s- (1 +/- g_mu) U_mu(x-mu)^dag in(x-mu) ]
+//
+// (upper signs: D, lower signs: D^dagger), then the epilogue
+//
+//   XPAY    : r = y + a*r           (CLOVX: y := A_x y first)       -> Mhat second half, source prep
+//   CLOVOUT : r = C_x r             (C = A^-1 of the output parity)  -> Mhat first half, reconstruction
+//   DOTS    : per-box partial sums of <r,y> and <r,r>               -> fused MR reductions
+//
+// One thread per output site (PAPER.md:164, :200-202 K1): 8 neighbour spinors + 8 links are
+// loaded with 128-bit coalesced loads; the 8-fold reuse of each input spinor is served by L2
+// (126 MB on B200).  CUDA-core FMA only: 3x3 complex matvecs
+// are not a dense contraction.  Spin projection uses the rank-2 structure of (1 +- g_mu) in
+// the chiral basis: 12 reals per hop go through the SU(3) multiply instead of 24.
+#pragma once
+#include "core.cuh"
+
+namespace lq {
+
+struct DslashArgs {
+  Geom g;
+  char* out;            // packed spinor, output parity
+  const char* in;       // packed spinor, input parity
+  const char* y;        // XPAY operand (output parity) or nullptr
+  const char* gauge;    // packed links, [parity][mu] records of RECON reals
+  const char* clov_y;   // A of the output parity (CLOVX)
+  const char* clov_out; // A^-1 of the output parity (CLOVOUT)
+  double a;             // xpay coefficient
+  double* dots;         // DOTS: [box][chunk][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
+  int parity;           // output parity
+  int dagger;
+};
+
+// multiply by a compile-time unit: C = 0: 1, 1: i, 2: -1, 3: -i
+template <int C, typename R> LQ_DEV cx<R> unit_mul(cx<R> z) {
+  if (C == 0) return z;
+  if (C == 1) return {-z.im, z.re};
+  if (C == 2) return {-z.re, -z.im};
+  return {z.im, -z.re};
+}
+
+// (gamma_mu psi)_0 = c0 psi_{j0}, (gamma_mu psi)_1 = c1 psi_{j1} in the DeGrand-Rossi basis (R2)
+template <int MU> struct GammaRow;
+template <> struct GammaRow<0> { static constexpr int j0 = 3, c0 = 1, j1 = 2, c1 = 1; };   // gamma_x
+template <> struct GammaRow<1> { static constexpr int j0 = 3, c0 = 2, j1 = 2, c1 = 0; };   // gamma_y
+template <> struct GammaRow<2> { static constexpr int j0 = 2, c0 = 1, j1 = 3, c1 = 3; };   // gamma_z
+template <> struct GammaRow<3> { static constexpr int j0 = 2, c0 = 0, j1 = 3, c1 = 0; };   // gamma_t
+
+// One hop: acc += sgn * (1 + sigma*gamma_MU) W psi,  W = U (FWD) or U^dagger (!FWD).
+template <int MU, bool FWD, typename R>
+LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restrict__ u, R sigma, R sgn) {
+  typedef GammaRow<MU> G;
+  // project: h0 = psi_0 + sigma*c0*psi_j0, h1 = psi_1 + sigma*c1*psi_j1   (3 colours each)
+  cx<R> h[2][3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const cx<R> p0 = {psi[2 * c], psi[2 * c + 1]};
+    const cx<R> p1 = {psi[6 + 2 * c], psi[6 + 2 * c + 1]};
+    const cx<R> q0 = unit_mul<G::c0>(cx<R>{psi[6 * G::j0 + 2 * c], psi[6 * G::j0 + 2 * c + 1]});
+    const cx<R> q1 = unit_mul<G::c1>(cx<R>{psi[6 * G::j1 + 2 * c], psi[6 * G::j1 + 2 * c + 1]});
+    h[0][c] = {p0.re + sigma * q0.re, p0.im + sigma * q0.im};
+    h[1][c] = {p1.re + sigma * q1.re, p1.im + sigma * q1.im};
+  }
+  // colour multiply
+  cx<R> w[2][3];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+      R re = 0, im = 0;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        if (FWD) {                       // U[r][k] * h[k]
+          const R ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
+          re += ur * h[s][k].re - ui * h[s][k].im;
+          im += ur * h[s][k].im + ui * h[s][k].re;
+        } else {                         // conj(U[k][r]) * h[k]
+          const R ur = u[6 * k + 2 * r], ui = u[6 * k + 2 * r + 1];
+          re += ur * h[s][k].re + ui * h[s][k].im;
+          im += ur * h[s][k].im - ui * h[s][k].re;
+        }
+      }
+      w[s][r] = {re, im};
+    }
+  }
+  // reconstruct: r_0 = w0, r_1 = w1, r_j0 = sigma*conj(c0)*w0, r_j1 = sigma*conj(c1)*w1
+  const R ss = sgn * sigma;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    acc[2 * c] += sgn * w[0][c].re;      acc[2 * c + 1] += sgn * w[0][c].im;
+    acc[6 + 2 * c] += sgn * w[1][c].re;  acc[6 + 2 * c + 1] += sgn * w[1][c].im;
+    const cx<R> t0 = unit_mul<(4 - G::c0) % 4>(w[0][c]);
+    const cx<R> t1 = unit_mul<(4 - G::c1) % 4>(w[1][c]);
+    acc[6 * G::j0 + 2 * c] += ss * t0.re; acc[6 * G::j0 + 2 * c + 1] += ss * t0.im;
+    acc[6 * G::j1 + 2 * c] += ss * t1.re; acc[6 * G::j1 + 2 * c + 1] += ss * t1.im;
+  }
+}
+
+// out = C in for one site: two Hermitian 6x6 blocks, 36 reals each: 6 diagonal then the 15
+// lower-triangle entries (i>j) at 6 + 2*(i(i-1)/2 + j).  504 flop (PAPER.md:138 fn.1: 72 reals).
+template <typename R>
+LQ_DEV void clover_mul(R* __restrict__ out, const R* __restrict__ in, const R* __restrict__ cl) {
+#pragma unroll
+  for (int ch = 0; ch < 2; ++ch) {
+    const R* c = cl + 36 * ch;
+    const R* x = in + 12 * ch;
+    R* o = out + 12 * ch;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      R re = c[i] * x[2 * i], im = c[i] * x[2 * i + 1];
+#pragma unroll
+      for (int j = 0; j < 6; ++j) {
+        if (j < i) {
+          const R lr = c[6 + 2 * (i * (i - 1) / 2 + j)], li = c[6 + 2 * (i * (i - 1) / 2 + j) + 1];
+          re += lr * x[2 * j] - li * x[2 * j + 1];
+          im += lr * x[2 * j + 1] + li * x[2 * j];
+        } else if (j > i) {
+          const R lr = c[6 + 2 * (j * (j - 1) / 2 + i)], li = c[6 + 2 * (j * (j - 1) / 2 + i) + 1];
+          re += lr * x[2 * j] + li * x[2 * j + 1];
+          im += lr * x[2 * j + 1] - li * x[2 * j];
+        }
+      }
+      o[2 * i] = re; o[2 * i + 1] = im;
+    }
+  }
+}
+
+// deterministic CTA reduction of NV doubles; result valid in thread 0
+template <int NV, int BLOCK>
+LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
+#pragma unroll
+  for (int k = 0; k < NV; ++k) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < NV; ++k) smem[k * (BLOCK / 32) + wid] = v[k];
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+      double s = 0;
+#pragma unroll
+      for (int w = 0; w < BLOCK / 32; ++w) s += smem[k * (BLOCK / 32) + w];
+      v[k] = s;
+    }
+  }
+}
+
+#define LQ_DSLASH_BLOCK 128
+
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+__global__ void __launch_bounds__(LQ_DSLASH_BLOCK)
+dslash_kernel(const DslashArgs a) {
+  typedef typename P::real R;
+  const Geom& g = a.g;
+  const int cb = blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
+  const int box = blockIdx.y;
+  const bool active = cb < g.vh;
+  double red[3] = {0, 0, 0};
+  if (active) {
+    const long long base = (long long)box * g.vh;
+    const long long idx = base + cb;
+    const int p = a.parity;
+    int c[4];
+    cb_to_coords(g, cb, p, c);
+    const int xh = c[0] >> 1;
+    const int rp = c[0] & 1;                 // row parity: x = 2*xh + rp
+    const long long link_bytes = (long long)RECON * sizeof(typename P::store_t) * g.ns;
+    const char* g_out = a.gauge + (long long)(p * 4) * link_bytes;        // links living on output-parity sites
+    const char* g_in = a.gauge + (long long)((1 - p) * 4) * link_bytes;   // links living on input-parity sites
+    const R sig_f = a.dagger ? R(1) : R(-1);  // forward hop: (1 - g) for D, (1 + g) for D^dagger
+    R acc[24];
+#pragma unroll
+    for (int k = 0; k < 24; ++k) acc[k] = 0;
+
+    // neighbour checkerboard indices
+    int nf[4], nbk[4];
+    {
+      const int xf = rp ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh;
+      const int xb = rp ? xh : (xh == 0 ? g.Xh - 1 : xh - 1);
+      nf[0] = cb - xh + xf;
+      nbk[0] = cb - xh + xb;
+      const int sy = g.Xh, sz = g.Xh * g.X[1], st = g.Xh * g.X[1] * g.X[2];
+      nf[1] = (c[1] + 1 == g.X[1]) ? cb - (g.X[1] - 1) * sy : cb + sy;
+      nbk[1] = (c[1] == 0) ? cb + (g.X[1] - 1) * sy : cb - sy;
+      nf[2] = (c[2] + 1 == g.X[2]) ? cb - (g.X[2] - 1) * sz : cb + sz;
+      nbk[2] = (c[2] == 0) ? cb + (g.X[2] - 1) * sz : cb - sz;
+      nf[3] = (c[3] + 1 == g.X[3]) ? cb - (g.X[3] - 1) * st : cb + st;
+      nbk[3] = (c[3] == 0) ? cb + (g.X[3] - 1) * st : cb - st;
+    }
+
+#define LQ_HOP(MU)                                                                              \
+    {                                                                                           \
+      const R sf = (c[MU] + 1 == g.X[MU]) ? (R)g.bc[MU] : R(1);                                 \
+      if (sf != R(0)) {                                                                         \
+        R u[18], psi[24];                                                                       \
+        load_link<P, RECON>(u, g_out + MU * link_bytes, g.ns, idx);                             \
+        load_site<P, 24>(psi, a.in, g.ns, base + nf[MU]);                                       \
+        hop<MU, true, R>(acc, psi, u, sig_f, sf);                                               \
+      }                                                                                         \
+      const R sb = (c[MU] == 0) ? (R)g.bc[MU] : R(1);                                           \
+      if (sb != R(0)) {                                                                         \
+        R u[18], psi[24];                                                                       \
+        load_link<P, RECON>(u, g_in + MU * link_bytes, g.ns, base + nbk[MU]);                   \
+        load_site<P, 24>(psi, a.in, g.ns, base + nbk[MU]);                                      \
+        hop<MU, false, R>(acc, psi, u, -sig_f, sb);                                             \
+      }                                                                                         \
+    }
+    LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3)
+#undef LQ_HOP
+
+    R yv[24];
+    if constexpr (XPAY) {
+      load_site<P, 24>(yv, a.y, g.ns, idx);
+      const R coef = (R)a.a;
+      if constexpr (CLOVX) {
+        R cl[72], ay[24];
+        load_site<P, 72>(cl, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
+        clover_mul<R>(ay, yv, cl);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) acc[k] = ay[k] + coef * acc[k];
+      } else {
+#pragma unroll
+        for (int k = 0; k < 24; ++k) acc[k] = yv[k] + coef * acc[k];
+      }
+    }
+    if constexpr (CLOVOUT) {
+      R cl[72], t[24];
+      load_site<P, 72>(cl, a.clov_out + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
+      clover_mul<R>(t, acc, cl);
+#pragma unroll
+      for (int k = 0; k < 24; ++k) acc[k] = t[k];
+    }
+    store_site<P, 24>(acc, a.out, g.ns, idx);
+    if constexpr (DOTS) {
+      // <r,y> = sum conj(r) y, <r,r>
+#pragma unroll
+      for (int k = 0; k < 12; ++k) {
+        red[0] += (double)(acc[2 * k] * yv[2 * k] + acc[2 * k + 1] * yv[2 * k + 1]);
+        red[1] += (double)(acc[2 * k] * yv[2 * k + 1] - acc[2 * k + 1] * yv[2 * k]);
+        red[2] += (double)(acc[2 * k] * acc[2 * k] + acc[2 * k + 1] * acc[2 * k + 1]);
+      }
+    }
+  }
+  if constexpr (DOTS) {
+    __shared__ double sm[3 * (LQ_DSLASH_BLOCK / 32)];
+    cta_reduce<3, LQ_DSLASH_BLOCK>(red, sm);
+    if (threadIdx.x == 0) {
+      double* d = a.dots + ((long long)box * gridDim.x + blockIdx.x) * 4;
+      d[0] = red[0]; d[1] = red[1]; d[2] = red[2]; d[3] = 0;
+    }
+  }
+}
+
+// Epilogue selector used by the host dispatch
+enum DslashEpi {
+  EPI_NONE = 0,       // out = D in
+  EPI_CLOVOUT = 1,    // out = C (D in)
+  EPI_CLOVX_XPAY = 2, // out = A y + a D in
+  EPI_XPAY = 3,       // out = y + a D in
+  EPI_XPAY_CLOVOUT = 4, // out = C (y + a D in)
+  EPI_CLOVX_XPAY_DOTS = 5  // EPI_CLOVX_XPAY + per-box <out,y>, <out,out>
+};
+
+template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);
+
+}  // namespace lq

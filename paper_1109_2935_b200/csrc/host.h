@@ -1,0 +1,96 @@
+// host.h -- internal declarations shared by the translation units of liblqcd_b200.so:
+// the context, the block-major (Schwarz) index map, and the launch wrappers.
+#pragma once
+#include <string>
+#include <vector>
+#include "core.cuh"
+#include "blas.cuh"
+#include "../../include/lqcd.h"
+
+namespace lq {
+
+// Natural layout <-> block-major layout.  The Schwarz preconditioner sees
+// the lattice as nbd[0]*nbd[1]*nbd[2]*nbd[3] independent boxes of extents blk.X with open
+// (Dirichlet) boundaries; box b = bx + nbd0*(by + nbd1*(bz + nbd2*bt)) occupies the contiguous
+// index range [b*blk.vh, (b+1)*blk.vh) of every block-major field.  Block extents are even,
+// so the parity of a site inside its box equals its global parity.
+struct BlockMap {
+  Geom nat;     // whole lattice, nb = 1
+  Geom blk;     // one box, nb = number of boxes, ns = nat.ns
+  int nbd[4];
+};
+
+LQ_DEV long long block_to_natural(const BlockMap& bm, int box, int lcb, int parity) {
+  int lc[4];
+  cb_to_coords(bm.blk, lcb, parity, lc);
+  int b = box, gc[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { gc[m] = (b % bm.nbd[m]) * bm.blk.X[m] + lc[m]; b /= bm.nbd[m]; }
+  return coords_to_cb(bm.nat, gc);
+}
+
+struct MultiArgs {
+  BlasArgs b;
+  const char* z[LQ_GCR_KMAX];
+  double chi[2 * LQ_GCR_KMAX];
+  int k, i0, n;
+};
+
+cudaError_t run_gcr_dots(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
+cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
+cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s);
+cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStream_t s);
+
+// setup kernels (pack.cu, clover.cu)
+cudaError_t run_pack_gauge(double* g64, const double* U_canonical, const Geom& nat, cudaStream_t s);
+cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s);
+cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s);
+cudaError_t run_clover_term(double* T72, const double* g64, const Geom& nat, double c_sw, cudaStream_t s);
+cudaError_t run_clover_make(int prec, char* A, char* Ainv, const double* T72, const BlockMap& bm, int blocked, double kappa, cudaStream_t s);
+cudaError_t run_clover_apply(int prec, char* out, const char* in, const char* clov, const Geom& g, int parity, cudaStream_t s);
+
+inline size_t spinor_bytes(int prec, long long ns) { return (size_t)ns * (prec == 0 ? 192 : prec == 1 ? 96 : 52); }
+inline size_t clover_bytes(int prec, long long ns) { return (size_t)ns * 2 * (prec == 0 ? 576 : prec == 1 ? 288 : 148); }
+inline size_t gauge_bytes(int prec, int recon, long long ns) { return (size_t)ns * 8 * recon * (prec == 0 ? 8 : prec == 1 ? 4 : 2); }
+inline int recon_index(int recon) { return recon == 18 ? 0 : recon == 12 ? 1 : recon == 8 ? 2 : -1; }
+
+}  // namespace lq
+
+// ------------------------------------------------------------------------------------------------
+struct lqcd_ctx {
+  int dims[4], bc[4], device;
+  long long V, Vh;
+  std::string err;
+  lq::Geom nat;
+  int n_sm;
+  long long launches;
+
+  // gauge: fp64 recon-18 natural master copy + derived copies [prec][recon index]
+  bool have_gauge;
+  double* g64;
+  char* gauge[3][3];
+  // Schwarz blocking currently materialised
+  bool have_blocks;
+  lq::BlockMap bm;
+  char* bgauge[3][3];
+  // clover
+  bool have_clover;
+  double c_sw;
+  double* T72;            // kappa-independent term, fp64, natural, [parity][72 reals planes]
+  double kappa;           // kappa of the materialised A / A^-1 copies (NaN = none)
+  char* clov[3];          // A      [prec]  natural  (both parities)
+  char* clovinv[3];       // A^-1
+  char* bclov[3];         // block-major copies
+  char* bclovinv[3];
+  // workspace
+  char* tmp[3];           // matpc temporary, natural layout, per precision
+  char* btmp[3];          // block-major temporary
+  double* S;              // device scalars (lq::S_TOTAL doubles)
+  double* partials;       // reduction partials
+  size_t partials_doubles;
+  unsigned* counters;
+  double* boxdots;        // MR per-box partial dots
+  size_t boxdots_doubles;
+  double* hS;             // pinned host mirror of S
+  std::vector<void*> pool; // solver workspace allocations released at the end of lqcd_invert
+};

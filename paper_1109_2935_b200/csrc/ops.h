@@ -1,0 +1,20 @@
+// ops.h -- internal host-side operator layer shared by api.cu and solver.cu.
+#pragma once
+#include "host.h"
+
+namespace lq {
+
+int fail(lqcd_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess);
+int dev_alloc(lqcd_ctx* c, void** p, size_t bytes);
+int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, cudaStream_t s);
+int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A, const char** Ainv, cudaStream_t s);
+int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out);
+int set_blocks(lqcd_ctx* c, const int* blk);
+int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
+              int epi, double a, double kappa, bool blocked, cudaStream_t s);
+int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
+             bool blocked, bool dots, cudaStream_t s);
+
+template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);
+
+}  // namespace lq

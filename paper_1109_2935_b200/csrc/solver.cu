@@ -1,0 +1,415 @@
+// solver.cu -- the solvers the operator runs inside:
+//   * mixed-precision BiCGstab with reliable updates  (reading R11)
+//   * additive-Schwarz preconditioner K = n_MR minimum-residual steps on the Dirichlet-cut
+//     Mhat_D, one alpha per block                      (reading R7)
+//   * GCR-DD, Algorithm 1                               (reading R8)
+// The host loop only launches kernels; all Krylov scalars live on the device (blas_ops.cuh).
+// One scalar (||r||^2) is read back per iteration for the convergence / restart decision.
+#include <cmath>
+#include <complex>
+#include <cstring>
+#include "blas_ops.cuh"
+#include "ops.h"
+
+using namespace lq;
+
+namespace {
+
+typedef OpMrUpdate<true, false> OpMrFirst;
+typedef OpMrUpdate<false, false> OpMrMid;
+typedef OpMrUpdate<false, true> OpMrLast;
+typedef OpMrUpdate<true, true> OpMrOnly;
+
+struct Work {                      // solver workspace, freed when it goes out of scope
+  lqcd_ctx* c;
+  std::vector<void*> ptrs;
+  explicit Work(lqcd_ctx* c_) : c(c_) {}
+  ~Work() { for (void* p : ptrs) cudaFree(p); }
+  int get(char** out, size_t bytes) {
+    void* p = nullptr;
+    int rc = dev_alloc(c, &p, bytes);
+    if (rc) return rc;
+    ptrs.push_back(p);
+    *out = (char*)p;
+    return LQCD_OK;
+  }
+};
+
+BlasArgs mk(lqcd_ctx* c, bool blocked, char* v0 = nullptr, char* v1 = nullptr, char* v2 = nullptr, char* v3 = nullptr, char* v4 = nullptr) {
+  BlasArgs a;
+  memset(&a, 0, sizeof(a));
+  a.v[0] = v0; a.v[1] = v1; a.v[2] = v2; a.v[3] = v3; a.v[4] = v4;
+  const Geom& g = blocked ? c->bm.blk : c->nat;
+  a.ns = g.ns; a.vh = g.vh; a.nb = g.nb;
+  a.S = c->S; a.partials = c->partials; a.counters = c->counters;
+  a.boxdots = c->boxdots;
+  a.nchunk = (g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK;
+  return a;
+}
+
+template <class Op>
+int blas(lqcd_ctx* c, int prec, const BlasArgs& a, cudaStream_t s) {
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "blas launch", e);
+}
+
+int read_S(lqcd_ctx* c, int off, int n, cudaStream_t s) {
+  cudaError_t e = cudaMemcpyAsync(c->hS + off, c->S + off, n * sizeof(double), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "scalar read-back", e);
+}
+
+int convert(lqcd_ctx* c, int pa, int pb, char* dst, const char* src, int dir, int parity, cudaStream_t s) {
+  cudaError_t e = run_convert(pa, pb, dst, src, c->bm, dir, parity, s);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "convert", e);
+}
+
+int norm2(lqcd_ctx* c, int prec, char* v, double* out, cudaStream_t s) {
+  BlasArgs a = mk(c, false, v);
+  int rc = blas<OpNorm2>(c, prec, a, s);
+  if (rc) return rc;
+  rc = read_S(c, S_OUT, 1, s);
+  *out = c->hS[S_OUT];
+  return rc;
+}
+
+// r = b - Mhat x in precision prec; returns ||r||
+int residual(lqcd_ctx* c, char* r, const char* b, const char* x, int parity, double kappa, int prec, int recon,
+             double* rn, cudaStream_t s) {
+  int rc = op_matpc(c, r, x, parity, 0, kappa, prec, recon, false, false, s);
+  if (rc) return rc;
+  BlasArgs a = mk(c, false, const_cast<char*>(b), r);
+  rc = blas<OpXmyNorm>(c, prec, a, s);
+  if (rc) return rc;
+  rc = read_S(c, S_OUT, 1, s);
+  *rn = sqrt(c->hS[S_OUT]);
+  return rc;
+}
+
+struct Counts { long long mat_sloppy = 0, mat_outer = 0, mat_precond = 0; double blas_flop_sites = 0; };
+
+}  // namespace
+
+namespace lq {
+
+// out = K in  (reading R7).  in/out: natural layout, precision prec_io.  rho, w, xk: block-major
+// workspace in precision prec (allocated by the caller).
+int schwarz_apply(lqcd_ctx* c, char* out, const char* in, int parity, double kappa, int n_mr, double omega,
+                  int prec, int recon, int prec_io, char* rho, char* w, char* xk, cudaStream_t s) {
+  int rc = convert(c, prec_io, prec, rho, in, 1, parity, s);
+  if (rc) return rc;
+  for (int step = 0; step < n_mr; ++step) {
+    rc = op_matpc(c, w, rho, parity, 0, kappa, prec, recon, true, true, s);
+    if (rc) return rc;
+    BlasArgs a = mk(c, true, xk, rho, w);
+    a.c[0] = omega;
+    const bool first = step == 0, last = step == n_mr - 1;
+    if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
+    else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
+    else if (last) rc = blas<OpMrLast>(c, prec, a, s);
+    else rc = blas<OpMrMid>(c, prec, a, s);
+    if (rc) return rc;
+  }
+  return convert(c, prec, prec_io, out, xk, 2, parity, s);
+}
+
+}  // namespace lq
+
+namespace {
+
+// ---------------------------------------------------------------- BiCGstab with reliable updates
+int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
+                   lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
+  const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
+  const long long ns = c->nat.ns;
+  Work wk(c);
+  char *r_hi, *xl, *rl, *rt, *pv, *v, *t;
+  int rc;
+  if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
+  char** lo[] = {&xl, &rl, &rt, &pv, &v, &t};
+  for (char** q : lo) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
+  double rn;
+  if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
+  cnt.mat_outer++;
+  res->iterations = 0; res->restarts = 0;
+  const double delta = p.delta > 0 ? p.delta : 0.1;
+  int status = LQCD_OK;
+  if (rn > stop) {
+    if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+    if ((rc = convert(c, ps, ps, rt, rl, 0, par, s))) return rc;
+    for (char* z : {xl, pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+    { BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc; }
+    double maxr = rn;
+    int it = 0;
+    while (true) {
+      if (it >= p.max_iter) { status = LQCD_ENOCONV; break; }
+      { BlasArgs a = mk(c, false, pv, rl, v); if ((rc = blas<OpBicgP>(c, ps, a, s))) return rc; }
+      if ((rc = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      { BlasArgs a = mk(c, false, rt, v); if ((rc = blas<OpBicgAlpha>(c, ps, a, s))) return rc; }
+      { BlasArgs a = mk(c, false, rl, v); if ((rc = blas<OpBicgS>(c, ps, a, s))) return rc; }
+      if ((rc = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      { BlasArgs a = mk(c, false, t, rl); if ((rc = blas<OpBicgOmega>(c, ps, a, s))) return rc; }
+      { BlasArgs a = mk(c, false, xl, pv, rl, t, rt); if ((rc = blas<OpBicgXR>(c, ps, a, s))) return rc; }
+      cnt.mat_sloppy += 2; cnt.blas_flop_sites += 1056; ++it;
+      if ((rc = read_S(c, S_RR, 2, s))) return rc;
+      const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
+      if (!(rr == rr) || flag != 0.0) { status = LQCD_EBREAKDOWN; }
+      const double rln = sqrt(rr);
+      if (rln > maxr) maxr = rln;
+      if (status == LQCD_EBREAKDOWN || rln <= stop || rln < delta * maxr) {
+        // reliable update: fold x_l into x, recompute the true residual in the outer precision
+        MultiArgs m; memset(&m, 0, sizeof(m));
+        m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
+        cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+        { BlasArgs a = mk(c, false, xl); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+        if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
+        cnt.mat_outer++; res->restarts++;
+        if (rn <= stop) { status = LQCD_OK; break; }
+        if (status == LQCD_EBREAKDOWN) {
+          // restart the recurrence from the true residual
+          status = LQCD_OK;
+          if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+          if ((rc = convert(c, ps, ps, rt, rl, 0, par, s))) return rc;
+          for (char* z : {pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+          BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
+          if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
+        } else {
+          if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+          BlasArgs a = mk(c, false, rt, rl); a.i0 = 1; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
+        }
+        maxr = rn;
+      }
+    }
+    res->iterations = it;
+  }
+  res->iterated_residual = rn;
+  return status;
+}
+
+// ---------------------------------------------------------------- GCR-DD (Algorithm 1)
+int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
+              lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
+  const int po = p.prec_outer, ps = p.prec_sloppy, pp = p.prec_precond, par = p.parity;
+  const long long ns = c->nat.ns;
+  const int kmax = p.gcr_kmax > 0 ? p.gcr_kmax : 16;
+  if (kmax > LQ_GCR_KMAX) return fail(c, LQCD_EINVAL, "gcr_kmax too large");
+  const double delta = p.delta > 0 ? p.delta : 0.1;
+  Work wk(c);
+  int rc;
+  char *r0, *rh, *rho = nullptr, *w = nullptr, *xk = nullptr;
+  std::vector<char*> ph(kmax), zh(kmax);
+  if ((rc = wk.get(&r0, spinor_bytes(po, ns)))) return rc;
+  if ((rc = wk.get(&rh, spinor_bytes(ps, ns)))) return rc;
+  for (int i = 0; i < kmax; ++i) {
+    if ((rc = wk.get(&ph[i], spinor_bytes(ps, ns)))) return rc;
+    if ((rc = wk.get(&zh[i], spinor_bytes(ps, ns)))) return rc;
+  }
+  if (p.precondition) {
+    if ((rc = set_blocks(c, p.schwarz_block))) return rc;
+    for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, ns)))) return rc;
+  }
+  double r0n;
+  if ((rc = residual(c, r0, b, x, par, p.kappa, po, p.recon_outer, &r0n, s))) return rc;
+  cnt.mat_outer++;
+  int total = 0, status = LQCD_OK;
+  res->restarts = 0;
+  while (r0n > stop) {
+    if (total >= p.max_iter) { status = LQCD_ENOCONV; break; }
+    if (!(r0n == r0n)) { status = LQCD_EBREAKDOWN; break; }
+    if ((rc = convert(c, po, ps, rh, r0, 0, par, s))) return rc;
+    int k = 0;
+    while (true) {
+      // p_k = K rhat
+      if (p.precondition) {
+        if ((rc = schwarz_apply(c, ph[k], rh, par, p.kappa, p.mr_steps, p.mr_omega, pp, p.recon_precond, ps, rho, w, xk, s))) return rc;
+        cnt.mat_precond += p.mr_steps; cnt.blas_flop_sites += p.mr_steps * (12.0 * 16 + 12.0 * 12);
+      } else if ((rc = convert(c, ps, ps, ph[k], rh, 0, par, s))) return rc;
+      // z_k = Mhat p_k
+      if ((rc = op_matpc(c, zh[k], ph[k], par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      cnt.mat_sloppy++;
+      // orthogonalise (one batched pass: classical Gram-Schmidt), normalise, update rhat
+      MultiArgs m; memset(&m, 0, sizeof(m));
+      m.b = mk(c, false, rh);
+      for (int i = 0; i <= k; ++i) m.z[i] = zh[i];
+      m.k = k;
+      for (int i0 = 0; i0 < k; i0 += 8) {
+        m.i0 = i0; m.n = (k - i0 < 8) ? k - i0 : 8;
+        cudaError_t e = run_gcr_dots(ps, m, c->n_sm * 8, s); c->launches++;
+        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "gcr dots", e);
+      }
+      { cudaError_t e = run_gcr_orth(ps, m, c->n_sm * 8, s); c->launches++;
+        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "gcr orth", e); }
+      { BlasArgs a = mk(c, false, zh[k], rh); if ((rc = blas<OpGcrScale>(c, ps, a, s))) return rc; }
+      cnt.blas_flop_sites += 12.0 * (16.0 * k + 12 + 14);
+      ++k; ++total;
+      if ((rc = read_S(c, S_RR, 1, s))) return rc;
+      const double rhn = sqrt(c->hS[S_RR]);
+      if (k == kmax || rhn / r0n < delta || rhn < stop || total >= p.max_iter || !(rhn == rhn)) break;
+    }
+    // implicit solution update: back-substitution for chi, then x += sum chi_i p_i
+    if ((rc = read_S(c, S_GCR_BETA, S_TOTAL - S_GCR_BETA, s))) return rc;
+    std::complex<double> chi[LQ_GCR_KMAX];
+    for (int l = k - 1; l >= 0; --l) {
+      std::complex<double> tacc(c->hS[S_GCR_ALPHAS + 2 * l], c->hS[S_GCR_ALPHAS + 2 * l + 1]);
+      for (int i = l + 1; i < k; ++i)
+        tacc -= std::complex<double>(c->hS[S_GCR_BETA + 2 * (l * LQ_GCR_KMAX + i)], c->hS[S_GCR_BETA + 2 * (l * LQ_GCR_KMAX + i) + 1]) * chi[i];
+      chi[l] = tacc / c->hS[S_GCR_GAMMAS + l];
+    }
+    MultiArgs m; memset(&m, 0, sizeof(m));
+    m.b = mk(c, false);
+    for (int i = 0; i < k; ++i) { m.z[i] = ph[i]; m.chi[2 * i] = chi[i].real(); m.chi[2 * i + 1] = chi[i].imag(); }
+    m.n = k;
+    cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+    if ((rc = residual(c, r0, b, x, par, p.kappa, po, p.recon_outer, &r0n, s))) return rc;
+    cnt.mat_outer++; res->restarts++;
+  }
+  res->iterations = total;
+  res->iterated_residual = r0n;
+  return status;
+}
+
+int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
+  if (!p) return fail(c, LQCD_EINVAL, "null params");
+  if (!c->have_gauge || !c->have_clover) return fail(c, LQCD_ESTATE, "invert before load_gauge / build_clover");
+  if (!(p->c_sw == c->c_sw)) return fail(c, LQCD_ESTATE, "params.c_sw differs from the built clover term");
+  if ((p->parity | 1) != 1) return fail(c, LQCD_EINVAL, "parity");
+  for (int pr : {p->prec_outer, p->prec_sloppy, p->prec_precond}) if (pr < 0 || pr > 2) return fail(c, LQCD_EINVAL, "precision");
+  for (int r : {p->recon_outer, p->recon_sloppy, p->recon_precond}) if (recon_index(r) < 0) return fail(c, LQCD_EINVAL, "recon");
+  if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "solver");
+  if (!(p->tol > 0) || p->max_iter < 1) return fail(c, LQCD_EINVAL, "tol / max_iter");
+  if (p->solver == LQCD_SOLVER_GCR_DD && p->precondition && p->mr_steps < 1) return fail(c, LQCD_EINVAL, "mr_steps");
+  return LQCD_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+int lqcd_schwarz(lqcd_ctx* c, void* out, const void* in, int parity, double kappa, const int block[4], int n_mr,
+                 double omega_mr, int prec, int recon, int prec_io, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || (parity | 1) != 1 || n_mr < 1 || prec < 0 || prec > 2 || prec_io < 0 || prec_io > 2)
+    return fail(c, LQCD_EINVAL, "schwarz arguments");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = set_blocks(c, block);
+  if (rc) return rc;
+  Work wk(c);
+  char *rho, *w, *xk;
+  for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->nat.ns)))) return rc;
+  rc = schwarz_apply(c, (char*)out, (const char*)in, parity, kappa, n_mr, omega_mr, prec, recon, prec_io, rho, w, xk, s);
+  cudaStreamSynchronize(s);          // workspace is freed on return
+  return rc;
+}
+
+int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_params* p, lqcd_invert_result* res, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!x_can || !b_can || !res) return fail(c, LQCD_EINVAL, "invert arguments");
+  int rc = check_params(c, p);
+  if (rc) return rc;
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  memset(res, 0, sizeof(*res));
+  const int po = p->prec_outer, par = p->parity;
+  const long long ns = c->nat.ns;
+  Work wk(c);
+  char *bp, *bq, *xp, *xq, *t1;
+  for (char** q : {&bp, &bq, &xp, &xq, &t1}) if ((rc = wk.get(q, spinor_bytes(po, ns)))) return rc;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  cudaEventRecord(e0, s);
+  Counts cnt;
+  // pack b; ||b||
+  cudaError_t e = run_pack_spinor(po, bp, (const double*)b_can, c->nat, par, 0, s); c->launches++;
+  if (e == cudaSuccess) { e = run_pack_spinor(po, bq, (const double*)b_can, c->nat, 1 - par, 0, s); c->launches++; }
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack", e);
+  double n1, n2;
+  if ((rc = norm2(c, po, bp, &n1, s))) return rc;
+  if ((rc = norm2(c, po, bq, &n2, s))) return rc;
+  const double bnorm = sqrt(n1 + n2);
+  if (bnorm == 0.0) {
+    cudaMemsetAsync(x_can, 0, (size_t)c->V * 24 * sizeof(double), s);
+    cudaStreamSynchronize(s);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    res->status = LQCD_OK;
+    return LQCD_OK;
+  }
+  // source preparation: bhat_p = b_p + kappa D A^-1 b_pbar   (R6)
+  const char *A, *Ai;
+  if ((rc = get_clover(c, po, p->kappa, false, &A, &Ai, s))) return rc;
+  e = run_clover_apply(po, t1, bq, Ai, c->nat, 1 - par, s); c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_apply", e);
+  if ((rc = op_dslash(c, xq /* holds bhat */, t1, bp, par, 0, po, p->recon_outer, EPI_XPAY, p->kappa, p->kappa, false, s))) return rc;
+  char* bhat = xq;
+  // initial guess
+  if (p->use_initial_guess) {
+    e = run_pack_spinor(po, xp, (const double*)x_can, c->nat, par, 0, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack", e);
+  } else {
+    BlasArgs a = mk(c, false, xp);
+    if ((rc = blas<OpZero>(c, po, a, s))) return rc;
+  }
+  const double stop = p->tol * bnorm;
+  int status;
+  if (p->solver == LQCD_SOLVER_BICGSTAB) status = solve_bicgstab(c, xp, bhat, *p, stop, res, cnt, s);
+  else status = solve_gcr(c, xp, bhat, *p, stop, res, cnt, s);
+  if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) { cudaEventDestroy(e0); cudaEventDestroy(e1); return status; }
+  // true residual of the Schur system in the outer precision = ||b - M x|| (R6)
+  double rn;
+  if ((rc = residual(c, t1, bhat, xp, par, p->kappa, po, p->recon_outer, &rn, s))) return rc;
+  cnt.mat_outer++;
+  res->true_residual = rn / bnorm;
+  res->iterated_residual /= bnorm;
+  // reconstruction: x_pbar = A^-1 (b_pbar + kappa D x_p)
+  if ((rc = op_dslash(c, t1, xp, bq, 1 - par, 0, po, p->recon_outer, EPI_XPAY_CLOVOUT, p->kappa, p->kappa, false, s))) return rc;
+  e = run_pack_spinor(po, xp, (const double*)x_can, c->nat, par, 1, s); c->launches++;
+  if (e == cudaSuccess) { e = run_pack_spinor(po, t1, (const double*)x_can, c->nat, 1 - par, 1, s); c->launches++; }
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "unpack", e);
+  cudaEventRecord(e1, s);
+  e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "invert", e);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  res->seconds = ms * 1e-3;
+  res->status = status;
+  res->matpc_sloppy = (int)cnt.mat_sloppy; res->matpc_outer = (int)cnt.mat_outer; res->matpc_precond = (int)cnt.mat_precond;
+  res->gflop = ((double)(cnt.mat_sloppy + cnt.mat_outer + cnt.mat_precond) * 3696.0 + cnt.blas_flop_sites) * (double)c->Vh * 1e-9;
+  if (status == LQCD_ENOCONV) return fail(c, status, "max_iter reached");
+  if (status == LQCD_EBREAKDOWN) return fail(c, status, "solver breakdown");
+  return LQCD_OK;
+}
+
+int lqcd_axpy_norm(lqcd_ctx* c, double a_, const void* x, void* y, int prec, double* norm2_host, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!x || !y || !norm2_host || prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "axpy_norm arguments");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  BlasArgs a = mk(c, false, (char*)x, (char*)y);
+  a.c[0] = a_;
+  int rc = blas<OpAxpyNorm>(c, prec, a, s);
+  if (rc) return rc;
+  rc = read_S(c, S_OUT, 1, s);
+  *norm2_host = c->hS[S_OUT];
+  return rc;
+}
+
+int lqcd_cdot(lqcd_ctx* c, const void* x, const void* y, int prec, double* dot_host, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!x || !y || !dot_host || prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "cdot arguments");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  BlasArgs a = mk(c, false, (char*)x, (char*)y);
+  int rc = blas<OpCdot>(c, prec, a, s);
+  if (rc) return rc;
+  rc = read_S(c, S_OUT, 2, s);
+  dot_host[0] = c->hS[S_OUT]; dot_host[1] = c->hS[S_OUT + 1];
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,202 @@
+"""GPU-vs-oracle parity (-m gpu): every call goes through the C ABI (include/lqcd.h) via the
+ctypes binding and is compared element by element with oracle/ on the same seeded inputs.
+
+Tolerances (relative L2 per operator application) are BASELINE.json's north_star:
+fp64 1e-13, fp32 1e-5, half 5e-3; solves: true residual <= 1e-10, solution within 1e-8.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1109_2935_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+BC = (1, 1, 1, -1)
+TOL = {0: 1e-13, 1: 1e-5, 2: 5e-3}
+
+
+def _rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+class Case:
+    """One lattice + gauge field loaded into a GPU context, with the oracle's clover term."""
+
+    def __init__(self, dims, eps, c_sw=1.0, bc=BC, gauge_seed=1):
+        from paper_1109_2935_b200 import lqcd
+        self.lqcd = lqcd
+        self.dims, self.bc, self.c_sw = dims, bc, c_sw
+        self.U = inputs.random_gauge(dims, eps, gauge_seed)
+        self.ctx = lqcd.Context(dims, bc, 0)
+        self.ctx.load_gauge(torch.from_numpy(self.U).cuda())
+        self.ctx.build_clover(c_sw)
+        self.T = oracle.clover_term(self.U, c_sw)
+        self.par = inputs.parity_mask(dims)
+
+    def mask(self, p):
+        return (self.par == p)[..., None, None]
+
+    def gpu_parity_op(self, fn, psi, p_in, p_out, prec):
+        """pack parity p_in of psi, run fn(out, in), unpack to a zero-initialised canonical array."""
+        ctx = self.ctx
+        d = torch.from_numpy(np.ascontiguousarray(psi)).cuda()
+        fin = ctx.pack_spinor(d, p_in, prec)
+        fout = ctx.new_field(prec)
+        fn(fout, fin)
+        res = torch.zeros_like(d)
+        ctx.unpack_spinor(res, fout, p_out, prec)
+        torch.cuda.synchronize()
+        return res.cpu().numpy()
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    return Case((4, 4, 4, 4), 0.5)
+
+
+@pytest.fixture(scope="module")
+def ragged():
+    # Vh = 6*4*10*8/2 = 960 = 7.5 CTAs of 128 threads: several tiles and a ragged tail
+    return Case((6, 4, 10, 8), 0.3, bc=(-1, 1, 1, -1))
+
+
+def test_pack_unpack_roundtrip(ragged):
+    c = ragged
+    psi = inputs.gaussian_spinor(c.dims, 2)
+    for prec, tol in ((0, 0.0), (1, 1e-7), (2, 3e-5)):
+        for p in (0, 1):
+            got = c.gpu_parity_op(lambda o, i: o.copy_(i), psi, p, p, prec)
+            want = psi * c.mask(p)
+            if tol == 0.0:
+                assert np.array_equal(got, want)
+            else:
+                assert _rel(got, want) <= tol
+            assert np.max(np.abs(got[c.par != p])) == 0.0
+
+
+@pytest.mark.parametrize("recon", [18, 12, 8])
+@pytest.mark.parametrize("dagger", [False, True])
+@pytest.mark.parametrize("parity", [0, 1])
+def test_cfg1_dslash_fp64(cfg1, parity, dagger, recon):
+    c = cfg1
+    psi = inputs.gaussian_spinor(c.dims, 2)
+    want = oracle.dslash(psi * c.mask(1 - parity), c.U, c.bc, dagger=dagger) * c.mask(parity)
+    got = c.gpu_parity_op(lambda o, i: c.ctx.dslash(o, i, parity, dagger, 0, recon), psi, 1 - parity, parity, 0)
+    assert _rel(got, want) <= (1e-13 if recon != 8 else 1e-11)   # recon-8 amplifies rounding by 1/N
+
+
+@pytest.mark.parametrize("dagger", [False, True])
+@pytest.mark.parametrize("parity", [0, 1])
+def test_cfg1_matpc_and_clover_fp64(cfg1, parity, dagger):
+    c = cfg1
+    kappa = 0.12
+    psi = inputs.gaussian_spinor(c.dims, 2)
+    want = oracle.matpc(psi, c.U, c.T, c.bc, kappa, parity, dagger=dagger)
+    got = c.gpu_parity_op(lambda o, i: c.ctx.matpc(o, i, parity, dagger, kappa, 0, 18), psi, parity, parity, 0)
+    assert _rel(got, want) <= 1e-13
+    for inverse in (False, True):
+        want = oracle.clover_apply(psi, c.T, kappa, inverse=inverse, parity=parity)
+        got = c.gpu_parity_op(lambda o, i: c.ctx.clover(o, i, parity, inverse, kappa, 0), psi, parity, parity, 0)
+        assert _rel(got, want) <= 1e-13
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+def test_ragged_all_precisions(ragged, prec, recon):
+    c = ragged
+    kappa = 0.124
+    psi = inputs.gaussian_spinor(c.dims, 3)
+    tol = TOL[prec] if not (prec == 0 and recon == 8) else 1e-11
+    for parity in (0, 1):
+        for dagger in (False, True):
+            want = oracle.dslash(psi * c.mask(1 - parity), c.U, c.bc, dagger=dagger) * c.mask(parity)
+            got = c.gpu_parity_op(lambda o, i: c.ctx.dslash(o, i, parity, dagger, prec, recon), psi, 1 - parity, parity, prec)
+            assert _rel(got, want) <= tol, ("dslash", parity, dagger)
+            assert np.max(np.abs(got[c.par != parity])) == 0.0
+            want = oracle.matpc(psi, c.U, c.T, c.bc, kappa, parity, dagger=dagger)
+            got = c.gpu_parity_op(lambda o, i: c.ctx.matpc(o, i, parity, dagger, kappa, prec, recon), psi, parity, parity, prec)
+            assert _rel(got, want) <= tol, ("matpc", parity, dagger)
+        for inverse in (False, True):
+            want = oracle.clover_apply(psi, c.T, kappa, inverse=inverse, parity=parity)
+            got = c.gpu_parity_op(lambda o, i: c.ctx.clover(o, i, parity, inverse, kappa, prec), psi, parity, parity, prec)
+            assert _rel(got, want) <= TOL[prec], ("clover", parity, inverse)
+
+
+def test_free_field_plane_wave_on_gpu():
+    """U = 1 (recon-18/12; recon-8 is singular at U = 1): closed form M(p)."""
+    dims, bc, kappa = (8, 4, 4, 6), (1, 1, 1, -1), 0.12
+    c = Case(dims, 0.0)
+    assert np.allclose(c.U, inputs.unit_gauge(dims))
+    X, Y, Z, T = dims
+    n = np.array([1, 0, 3, 2])
+    p = 2 * np.pi * (n + np.where(np.array(bc) < 0, 0.5, 0.0)) / np.array(dims)
+    t, z, y, x = np.meshgrid(np.arange(T), np.arange(Z), np.arange(Y), np.arange(X), indexing="ij")
+    phase = np.exp(1j * (p[0] * x + p[1] * y + p[2] * z + p[3] * t))
+    u = np.random.default_rng(5).standard_normal((4, 3)) + 0j
+    psi = phase[..., None, None] * u
+    g = [oracle.gamma(m) for m in range(4)]
+    Dp = sum((np.eye(4) - g[m]) * np.exp(1j * p[m]) + (np.eye(4) + g[m]) * np.exp(-1j * p[m]) for m in range(4))
+    want = phase[..., None, None] * (Dp @ u)
+    for recon in (18, 12):
+        for parity in (0, 1):
+            got = c.gpu_parity_op(lambda o, i: c.ctx.dslash(o, i, parity, False, 0, recon), psi, 1 - parity, parity, 0)
+            assert _rel(got, want * c.mask(parity)) <= 1e-13
+
+
+def test_cfg2_fp32_recon12():
+    """BASELINE.json config 2: 16^3x32, fp32 storage, recon-12, eps = 0.3."""
+    c = Case((16, 16, 16, 32), 0.3)
+    psi = inputs.gaussian_spinor(c.dims, 2)
+    for parity in (0, 1):
+        for dagger in (False, True):
+            want = oracle.dslash(psi * c.mask(1 - parity), c.U, c.bc, dagger=dagger) * c.mask(parity)
+            got = c.gpu_parity_op(lambda o, i: c.ctx.dslash(o, i, parity, dagger, 1, 12), psi, 1 - parity, parity, 1)
+            assert _rel(got, want) <= 1e-5
+        want = oracle.clover_apply(psi, c.T, 0.124, parity=parity)
+        got = c.gpu_parity_op(lambda o, i: c.ctx.clover(o, i, parity, False, 0.124, 1), psi, parity, parity, 1)
+        assert _rel(got, want) <= 1e-5
+    # half precision on the same lattice
+    want = oracle.matpc(psi, c.U, c.T, c.bc, 0.124, 0)
+    got = c.gpu_parity_op(lambda o, i: c.ctx.matpc(o, i, 0, False, 0.124, 2, 12), psi, 0, 0, 2)
+    assert _rel(got, want) <= 5e-3
+
+
+def test_blas_reductions(ragged):
+    c = ragged
+    x = inputs.gaussian_spinor(c.dims, 11)
+    y = inputs.gaussian_spinor(c.dims, 12)
+    for prec, tol in ((0, 1e-14), (1, 1e-6), (2, 2e-4)):
+        fx = c.ctx.pack_spinor(torch.from_numpy(x).cuda(), 0, prec)
+        fy = c.ctx.pack_spinor(torch.from_numpy(y).cuda(), 0, prec)
+        xm, ym = x * c.mask(0), y * c.mask(0)
+        d = c.ctx.cdot(fx, fy, prec)
+        assert abs(d - np.vdot(xm.ravel(), ym.ravel())) <= tol * np.linalg.norm(xm) * np.linalg.norm(ym)
+        n2 = c.ctx.axpy_norm(0.37, fx, fy, prec)
+        want = ym + 0.37 * xm
+        assert abs(n2 - np.linalg.norm(want) ** 2) <= 10 * tol * np.linalg.norm(want) ** 2
+        res = torch.zeros(x.shape, dtype=torch.complex128, device="cuda")
+        c.ctx.unpack_spinor(res, fy, 0, prec)
+        assert _rel(res.cpu().numpy(), want) <= max(tol, 1e-15) * 10
+        # bit-reproducible reductions
+        assert c.ctx.cdot(fx, fy, prec) == c.ctx.cdot(fx, fy, prec)
+
+
+def test_error_codes(cfg1):
+    from paper_1109_2935_b200 import lqcd
+    with pytest.raises(lqcd.LqcdError):
+        lqcd.Context((3, 4, 4, 4), BC, 0)                       # odd extent
+    ctx = lqcd.Context((4, 4, 4, 4), BC, 0)
+    f = ctx.new_field(0)
+    g = ctx.new_field(0)
+    with pytest.raises(lqcd.LqcdError) as e:
+        ctx.dslash(f, g, 0, False, 0, 18)                       # before load_gauge
+    assert e.value.code == lqcd.ESTATE
+    with pytest.raises(lqcd.LqcdError) as e:
+        cfg1.ctx.dslash(f, g, 0, False, 0, 10)                  # bad recon
+    assert e.value.code == lqcd.EINVAL
+    with pytest.raises(lqcd.LqcdError) as e:
+        cfg1.ctx.dslash(f, f, 0, False, 0, 18)                  # aliasing
+    assert e.value.code == lqcd.EINVAL
+    ctx.close()

@@ -1,0 +1,132 @@
+"""GPU solver parity (-m gpu): lqcd_invert / lqcd_schwarz through the C ABI against the oracle.
+
+Iterates and iteration counts differ between precisions and implementations (several correct
+answers); what is unique is compared: the solution x = M^-1 b (<= 1e-8 relative) and the true
+residual ||b - M x||/||b|| recomputed by the ORACLE's operator (<= 1e-10).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1109_2935_b200 import inputs
+from test_gpu_parity import Case, _rel, BC
+
+pytestmark = pytest.mark.gpu
+
+
+def _solve(c, b, params):
+    x = torch.zeros(b.shape, dtype=torch.complex128, device="cuda")
+    info = c.ctx.invert(x, torch.from_numpy(b).cuda(), params)
+    torch.cuda.synchronize()
+    return x.cpu().numpy(), info
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    return Case((4, 4, 4, 4), 0.5)
+
+
+@pytest.fixture(scope="module")
+def mid():
+    return Case((8, 8, 8, 16), 0.2)
+
+
+def test_cfg1_bicgstab_fp64(cfg1):
+    """BASELINE.json config 1: 4^4, kappa = 0.12, c_sw = 1, BiCGstab to 1e-12."""
+    c = cfg1
+    lq = c.lqcd
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, 0.12, parity=0, tol=1e-12)
+    assert io["status"] == 0
+    for parity in (0, 1):
+        p = c.ctx.make_params(0.12, 1.0, 1e-12, solver=lq.SOLVER_BICGSTAB, prec=(0, 0, 0), recon=(18, 18, 18), parity=parity)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-12
+        res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, 0.12)) / np.linalg.norm(b)
+        assert res <= 2e-12
+        assert _rel(x, xo) <= 1e-10
+
+
+@pytest.mark.parametrize("sloppy,recon", [(1, 12), (2, 12), (1, 8), (2, 18)])
+def test_mixed_precision_bicgstab(mid, sloppy, recon):
+    c = mid
+    lq = c.lqcd
+    kappa = 0.124
+    b = inputs.gaussian_spinor(c.dims, 2)
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB, prec=(0, sloppy, sloppy), recon=(18, recon, recon))
+    x, info = _solve(c, b, p)
+    assert info["status"] == 0 and info["true_residual"] <= 1e-10
+    assert info["restarts"] >= 1
+    res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+    assert res <= 1.05e-10
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    assert _rel(x, xo) <= 1e-8
+
+
+def test_schwarz_matches_oracle(mid):
+    c = mid
+    kappa, blk = 0.124, (4, 4, 4, 8)
+    r = inputs.gaussian_spinor(c.dims, 4)
+    for parity in (0, 1):
+        # Dirichlet operator alone, through K with one MR step: K r = alpha_b r per block
+        want1 = oracle.schwarz(r, c.U, c.T, c.bc, kappa, parity, blk, n_mr=1)
+        want5 = oracle.schwarz(r, c.U, c.T, c.bc, kappa, parity, blk, n_mr=5)
+        for prec, t1, t5 in ((0, 1e-12, 1e-11), (1, 1e-5, 5e-5), (2, 5e-3, 2e-2)):
+            got1 = c.gpu_parity_op(lambda o, i: c.ctx.schwarz(o, i, parity, kappa, blk, 1, 1.0, prec, 12, 0), r, parity, parity, 0)
+            got5 = c.gpu_parity_op(lambda o, i: c.ctx.schwarz(o, i, parity, kappa, blk, 5, 1.0, prec, 12, 0), r, parity, parity, 0)
+            assert _rel(got1, want1) <= t1, (parity, prec)
+            assert _rel(got5, want5) <= t5, (parity, prec)
+    # support on one block stays exactly inside it (bitwise zero elsewhere), even in half precision
+    T_, Z_, Y_, X_ = r.shape[:4]
+    t, z, y, x = np.meshgrid(np.arange(T_), np.arange(Z_), np.arange(Y_), np.arange(X_), indexing="ij")
+    inside = (x // 4 == 1) & (y // 4 == 0) & (z // 4 == 1) & (t // 8 == 1)
+    src = r * inside[..., None, None]
+    got = c.gpu_parity_op(lambda o, i: c.ctx.schwarz(o, i, 0, kappa, blk, 4, 1.0, 2, 12, 1), src, 0, 0, 1)
+    assert np.max(np.abs(got[~inside])) == 0.0
+    assert np.max(np.abs(got[inside])) > 0.0
+
+
+@pytest.mark.parametrize("sloppy,precond", [(0, 0), (1, 2), (2, 2)])
+def test_gcr_dd(mid, sloppy, precond):
+    c = mid
+    lq = c.lqcd
+    kappa = 0.124
+    b = inputs.gaussian_spinor(c.dims, 2)
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, prec=(0, sloppy, precond), recon=(18, 12, 12),
+                          gcr_kmax=16, schwarz_block=(4, 4, 4, 8), mr_steps=10, delta=0.1)
+    x, info = _solve(c, b, p)
+    assert info["status"] == 0 and info["true_residual"] <= 1e-10
+    res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+    assert res <= 1.05e-10
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    assert _rel(x, xo) <= 1e-8
+    # unpreconditioned GCR needs more outer iterations than GCR-DD
+    if sloppy == 0:
+        p2 = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, prec=(0, 0, 0), recon=(18, 18, 18),
+                               gcr_kmax=16, precondition=False)
+        x2, info2 = _solve(c, b, p2)
+        assert info2["true_residual"] <= 1e-10 and _rel(x2, xo) <= 1e-8
+        assert info["iterations"] < info2["iterations"]
+        # fp64 GCR-DD follows Algorithm 1 like the oracle: same number of outer iterations (+-1)
+        xo2, io2 = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-10, solver=oracle.GCR_DD, kmax=16,
+                                 delta=0.1, block=(4, 4, 4, 8), n_mr=10)
+        assert abs(io2["iterations"] - info["iterations"]) <= 1
+
+
+def test_invert_host_and_apply_host(cfg1):
+    c = cfg1
+    lq = c.lqcd
+    b = inputs.gaussian_spinor(c.dims, 2)
+    bh = torch.from_numpy(b).pin_memory()
+    xh = torch.zeros_like(bh).pin_memory()
+    p = c.ctx.make_params(0.12, 1.0, 1e-12, prec=(0, 1, 1), recon=(18, 12, 12))
+    info = c.ctx.invert_host(xh, bh, p)
+    assert info["true_residual"] <= 1e-12
+    res = np.linalg.norm(b - oracle.M(xh.numpy(), c.U, c.T, c.bc, 0.12)) / np.linalg.norm(b)
+    assert res <= 2e-12
+    out = torch.zeros_like(bh).pin_memory()
+    c.ctx.apply_host(out, bh, 0, 0, False, 0.12, 0, 18)
+    assert _rel(out.numpy(), oracle.dslash(b, c.U, c.bc)) <= 1e-13
+    c.ctx.apply_host(out, bh, 1, 1, True, 0.12, 0, 12)
+    assert _rel(out.numpy(), oracle.matpc(b, c.U, c.T, c.bc, 0.12, 1, dagger=True)) <= 1e-13
