@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- Wilson-clover Dslash GFLOP/s and HBM GB/s at 32^3x64 on B200 (BASELINE.json).
+
+A "step" is one application of the Wilson-clover hopping term D to a full-lattice spinor
+(both parities = two launches of the Dslash kernel), fp32 storage / recon-12 links, on the
+synthetic config-3 lattice (32^3x64, eps = 0.3).  `value` is nominal GFLOP/s at 1320 flop per
+site (Eq. 2; convention of BASELINE.json) with all inputs resident in HBM.  `e2e` is
+the same metric through lqcd_apply_host: host canonical spinor -> H2D -> pack -> D -> unpack
+-> D2H inside the timed region.  `extra` holds the precision x compression sweep for Dslash
+and Mhat, the fused BLAS-1 rates and the solver times (configs 4, and 5 with --full).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--full] [--quick]
+
+N > 1 (torchrun): replicas only: every rank runs the same workload on its own
+GPU, no collective on the data path; value = sum over ranks / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+DIMS = (32, 32, 32, 64)
+BC = (1, 1, 1, -1)
+EPS, KAPPA, CSW = 0.3, 0.124, 1.0
+FLOP_DSLASH, FLOP_MATPC = 1320, 3696
+# algorithmic (compulsory) bytes per output site of one parity: 2 spinors + 8 links
+SPINOR_B = {0: 192, 1: 96, 2: 52}
+LINK_B = {0: 8, 1: 4, 2: 2}
+CLOVER_B = {0: 576, 1: 288, 2: 148}
+
+
+def dslash_bytes(prec, recon):
+    return 2 * SPINOR_B[prec] + 8 * recon * LINK_B[prec]
+
+
+def matpc_bytes(prec, recon):
+    return 5 * SPINOR_B[prec] + 16 * recon * LINK_B[prec] + 2 * CLOVER_B[prec]
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 2 + k and r[2 + k].startswith("Active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def time_region(fn, reps):
+    """CUDA-event time (ms) of reps calls of fn on torch's current stream (the stream the
+    library launches on)."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def oracle_dslash_rate(n_apps, dims=DIMS, eps=EPS):
+    """The oracle, as it stands, on the host cores: full-lattice D applications."""
+    import numpy as np
+    import oracle
+    from paper_1109_2935_b200 import inputs
+    U = inputs.random_gauge_torch(dims, eps, 1).numpy()
+    psi = inputs.gaussian_spinor_torch(dims, 2).numpy()
+    oracle.num_threads()                      # loads (and if needed builds) the library outside the timed region
+    t0 = time.time()
+    for _ in range(n_apps):
+        out = oracle.dslash(psi, U, BC)
+    dt = time.time() - t0
+    V = int(np.prod(dims))
+    return FLOP_DSLASH * V * n_apps / dt / 1e9, dt, oracle.num_threads(), out
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    V = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3]
+    import oracle
+    from paper_1109_2935_b200 import inputs
+    U = inputs.random_gauge_torch(DIMS, EPS, 1).numpy()
+    psi = inputs.gaussian_spinor_torch(DIMS, 2).numpy()
+    for _ in range(min(args.warmup, 1)):
+        oracle.dslash(psi, U, BC)
+    t0 = time.time()
+    for _ in range(args.steps):
+        oracle.dslash(psi, U, BC)
+    dt = time.time() - t0
+    val = FLOP_DSLASH * V * args.steps / dt / 1e9
+    sample = "%d full-lattice D applications at 32^3x64 (fp64 oracle, OpenMP)" % args.steps
+    print(json.dumps({
+        "impl": "reference", "metric": "wilson_clover_dslash_gflops", "value": val, "unit": "GFLOP/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config 3: 32^3x64 eps=0.3, full-lattice Dslash", "precision": "fp64", "recon": 18},
+        "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="b200")
+    ap.add_argument("--full", action="store_true", help="also run config 5 (48^3x96 GCR-DD vs BiCGstab)")
+    ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if args.steps > 20:
+            args.steps = 10
+        run_reference(args, rank)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1109_2935_b200 import inputs, lqcd
+
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    V = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3]
+    Vh = V // 2
+    pk, pk_kind = peaks()
+
+    # ---- setup (not timed): synthetic config-3 lattice -------------------------------------------
+    U = inputs.random_gauge_torch(DIMS, EPS, 1 + rank, device=dev)
+    psi = inputs.gaussian_spinor_torch(DIMS, 2 + rank, device=dev)
+    ctx = lqcd.Context(DIMS, BC, local)
+    ctx.load_gauge(U)
+    ctx.build_clover(CSW)
+    prec, recon = lqcd.PREC_SINGLE, lqcd.RECON_12
+    f = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
+    g = [ctx.new_field(prec) for _ in (0, 1)]
+
+    def step():
+        ctx.dslash(g[0], f[1], 0, False, prec, recon)
+        ctx.dslash(g[1], f[0], 1, False, prec, recon)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = ctx.launch_count()
+    ms = time_region(step, args.steps)
+    launches = ctx.launch_count() - l0
+    if world > 1:
+        dist.barrier()
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- e2e: host buffers through lqcd_apply_host -----------------------------------------------
+    h_in = psi.cpu().pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    e2e_steps = max(3, min(args.steps, 5))
+    ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon)
+    torch.cuda.synchronize()
+    e2e_ms = time_region(lambda: ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon), e2e_steps)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    clocks = sampler.stop() if rank == 0 else None
+    cbytes = V * 12 * 16
+
+    ms_step = ms / args.steps
+    value = FLOP_DSLASH * V * world / (ms_step * 1e-3) / 1e9
+    kern_ms = ms / launches
+    algo_bytes = dslash_bytes(prec, recon) * Vh
+    achieved = algo_bytes / (kern_ms * 1e-3) / 1e9
+
+    out = {
+        "metric": "wilson_clover_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config 3: 32^3x64, eps=0.3, full-lattice Wilson-clover Dslash (both parities)",
+                   "precision": "fp32 storage+arithmetic", "recon": 12, "flop_per_site": FLOP_DSLASH,
+                   "l2": "inputs larger than L2 (gauge 403 MB + spinors 201 MB per step vs 126 MB L2)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                     "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_kind": pk_kind,
+                     "kernel": "dslash_kernel<PrecS,12> (EPI_NONE)", "algorithmic_bytes_per_launch": algo_bytes,
+                     "frac_of_8TBs_nominal": achieved / 8000.0},
+        "e2e": {"value": FLOP_DSLASH * V * world / (e2e_ms / e2e_steps * 1e-3) / 1e9, "unit": "GFLOP/s",
+                "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps},
+        "gpu_launches": launches,
+        "clocks": clocks,
+    }
+
+    if rank == 0 and not args.quick:
+        out["extra"] = extras(ctx, psi, args, torch, lqcd, inputs, pk)
+        n_apps = 10
+        gf, dt, cores, o_out = oracle_dslash_rate(n_apps)
+        out["cpu_baseline"] = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+                               "sample": "%d full-lattice D applications at 32^3x64 in %.1f s (fp64, OpenMP)" % (n_apps, dt)}
+        # parity of the timed configuration against the oracle on the full lattice (same inputs)
+        import numpy as np
+        got = torch.zeros_like(psi)
+        ctx.unpack_spinor(got, g[0], 0, prec)
+        ctx.unpack_spinor(got, g[1], 1, prec)
+        want = torch.from_numpy(o_out).to(dev)      # rank 0's inputs are seeds (1, 2), the oracle's too
+        if want is not None:
+            out["parity_rel_l2_vs_oracle"] = float(torch.linalg.vector_norm(got - want) / torch.linalg.vector_norm(want))
+    elif rank == 0:
+        out["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def extras(ctx, psi, args, torch, lqcd, inputs, pk):
+    """Config-3 sweep (precision x compression, Dslash and Mhat), BLAS-1 rates, config-4 solves."""
+    V = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3]
+    Vh = V // 2
+    ex = {"sweep": [], "blas": [], "solvers": []}
+    names = {0: "fp64", 1: "fp32", 2: "half"}
+    for prec in (0, 1, 2):
+        fin = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
+        fo = [ctx.new_field(prec) for _ in (0, 1)]
+        for recon in (18, 12, 8):
+            def d():
+                ctx.dslash(fo[0], fin[1], 0, False, prec, recon)
+                ctx.dslash(fo[1], fin[0], 1, False, prec, recon)
+
+            def m():
+                ctx.matpc(fo[0], fin[0], 0, False, KAPPA, prec, recon)
+                ctx.matpc(fo[1], fin[1], 1, False, KAPPA, prec, recon)
+            for name, fn, flop, by in (("dslash", d, FLOP_DSLASH, dslash_bytes(prec, recon)),
+                                       ("matpc", m, FLOP_MATPC, matpc_bytes(prec, recon))):
+                for _ in range(3):
+                    fn()
+                ms = time_region(fn, 20) / 40.0          # per parity application
+                gbs = by * Vh / (ms * 1e-3) / 1e9
+                ex["sweep"].append({"op": name, "prec": names[prec], "recon": recon, "us": ms * 1e3,
+                                    "gflops": flop * Vh / (ms * 1e-3) / 1e9, "gbs": gbs,
+                                    "frac_measured_peak": gbs / pk["hbm_gbs"], "frac_8TBs": gbs / 8000.0,
+                                    "bytes_per_site": by})
+        # fused BLAS-1: axpy+norm (3 passes) and cdot (2 passes)
+        for _ in range(3):
+            ctx.axpy_norm(0.5, fin[0], fo[0], prec)
+        t0 = time_region(lambda: ctx.axpy_norm(1e-3, fin[0], fo[0], prec), 20) / 20.0
+        t1 = time_region(lambda: ctx.cdot(fin[0], fo[0], prec), 20) / 20.0
+        ex["blas"].append({"prec": names[prec], "axpy_norm_us": t0 * 1e3, "axpy_norm_gbs": 3 * SPINOR_B[prec] * Vh / (t0 * 1e-3) / 1e9,
+                           "cdot_us": t1 * 1e3, "cdot_gbs": 2 * SPINOR_B[prec] * Vh / (t1 * 1e-3) / 1e9,
+                           "note": "includes one host read-back of the result per call"})
+        del fin, fo
+    # config 4: eps = 0.2, mixed-precision BiCGstab, fp64 outer, to 1e-10
+    dev = psi.device
+    U4 = inputs.random_gauge_torch(DIMS, 0.2, 11, device=dev)
+    ctx.load_gauge(U4)
+    ctx.build_clover(CSW)
+    b = inputs.gaussian_spinor_torch(DIMS, 12, device=dev)
+    x = torch.zeros_like(b)
+    for sloppy, recon in ((1, 12), (2, 12)):
+        p = ctx.make_params(KAPPA, CSW, 1e-10, solver=lqcd.SOLVER_BICGSTAB, prec=(0, sloppy, sloppy), recon=(18, recon, recon))
+        ctx.invert(x, b, p, allow_fail=True)        # warm-up (allocations, clover copies)
+        info = ctx.invert(x, b, p, allow_fail=True)
+        info.update({"config": 4, "solver": "bicgstab", "sloppy": names[sloppy], "recon_sloppy": recon,
+                     "effective_gflops": info["gflop"] / info["seconds"]})
+        ex["solvers"].append(info)
+    p = ctx.make_params(KAPPA, CSW, 1e-10, solver=lqcd.SOLVER_GCR_DD, prec=(0, 1, 2), recon=(18, 12, 12),
+                        gcr_kmax=16, schwarz_block=(8, 8, 8, 16), mr_steps=10)
+    ctx.invert(x, b, p, allow_fail=True)
+    info = ctx.invert(x, b, p, allow_fail=True)
+    info.update({"config": "4 (lattice) with GCR-DD, 8^3x16 blocks", "solver": "gcr_dd", "sloppy": "fp32", "precond": "half",
+                 "effective_gflops": info["gflop"] / info["seconds"]})
+    ex["solvers"].append(info)
+    return ex
+
+
+if __name__ == "__main__":
+    main()
