@@ -103,19 +103,17 @@ def time_region(fn, reps):
     return e0.elapsed_time(e1)
 
 
-def oracle_dslash_rate(n_apps, dims=DIMS, eps=EPS):
-    """The oracle, as it stands, on the host cores: full-lattice D applications."""
+def oracle_dslash_rate(n_apps, U, psi):
+    """The oracle, as it stands, on the host cores: full-lattice D applications on the same
+    arrays the GPU path was given (numpy complex128, canonical layout)."""
     import numpy as np
     import oracle
-    from paper_1109_2935_b200 import inputs
-    U = inputs.random_gauge_torch(dims, eps, 1).numpy()
-    psi = inputs.gaussian_spinor_torch(dims, 2).numpy()
     oracle.num_threads()                      # loads (and if needed builds) the library outside the timed region
     t0 = time.time()
     for _ in range(n_apps):
         out = oracle.dslash(psi, U, BC)
     dt = time.time() - t0
-    V = int(np.prod(dims))
+    V = int(np.prod(psi.shape[:4]))
     return FLOP_DSLASH * V * n_apps / dt / 1e9, dt, oracle.num_threads(), out
 
 
@@ -250,7 +248,7 @@ def main():
     if rank == 0 and not args.quick:
         out["extra"] = extras(ctx, psi, args, torch, lqcd, inputs, pk)
         n_apps = 10
-        gf, dt, cores, o_out = oracle_dslash_rate(n_apps)
+        gf, dt, cores, o_out = oracle_dslash_rate(n_apps, U.cpu().numpy(), psi.cpu().numpy())
         out["cpu_baseline"] = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
                                "sample": "%d full-lattice D applications at 32^3x64 in %.1f s (fp64, OpenMP)" % (n_apps, dt)}
         # parity of the timed configuration against the oracle on the full lattice (same inputs)

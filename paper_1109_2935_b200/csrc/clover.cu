@@ -229,10 +229,9 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(char* out, const char
   typedef typename P::real R;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= g.ns) return;
-  R x[24], y[24], cl[72];
+  R x[24], y[24];
   load_site<P, 24>(x, in, g.ns, i);
-  load_site<P, 72>(cl, clov + (long long)parity * site_bytes<P>(72, true) * g.ns, g.ns, i);
-  clover_mul<R>(y, x, cl);
+  clover_site<P>(y, x, clov + (long long)parity * site_bytes<P>(72, true) * g.ns, g.ns, i);
   store_site<P, 24>(y, out, g.ns, i);
 }
 

@@ -74,19 +74,49 @@ template <class P> __host__ __device__ constexpr int site_bytes(int n, bool with
 
 #define LQ_FIXED_MAX 32767.0f
 #define LQ_FIXED_INV (1.0f / 32767.0f)
+// 16-bit fixed point is stored in offset binary (u = q + 32768, q in [-32767, 32767]) so that
+// decoding is one byte-permute into the mantissa of 2^23 and one FADD, and encoding is one FFMA
+// whose result's low 16 bits are u (round-to-nearest-even done by the FP adder); no I2F / F2I.
+#define LQ_MAGIC_DEC 8421376.0f      /* 2^23 + 32768 */
+#define LQ_MAGIC_ENC 12615680.0f     /* 1.5*2^23 + 32768 */
+
+LQ_DEV float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+LQ_DEV double fma_(double a, double b, double c) { return fma(a, b, c); }
+
+// the two 16-bit fields of w as floats holding the signed integers q
+LQ_DEV float fixed_lo(unsigned w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - LQ_MAGIC_DEC; }
+LQ_DEV float fixed_hi(unsigned w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - LQ_MAGIC_DEC; }
+// pack rint(a*sc), rint(b*sc) (|.| <= 32767) as two offset-binary 16-bit fields
+LQ_DEV unsigned fixed_pack(float a, float b, float sc) {
+  const unsigned ua = __float_as_uint(fmaf(a, sc, LQ_MAGIC_ENC)), ub = __float_as_uint(fmaf(b, sc, LQ_MAGIC_ENC));
+  return __byte_perm(ua, ub, 0x5410);
+}
 
 // ---------------------------------------------------------------- site vectors with a norm (spinor: 24, clover: 72)
-// R9: half = int16 q_i = rint(v_i * 32767 / n), n = max_i |v_i| (fp32) per site; decode v_i = q_i * n/32767.
+// R9: half = 16-bit fixed point q_i = rint(v_i * 32767 / n), n = max_i |v_i| (fp32) per site; decode v_i = q_i * n/32767.
+// load_site_raw returns v and scale with (true value) = scale * v, so that callers can fold
+// the scale into an FMA coefficient instead of spending one FMUL per element.
 template <class P, int N>
-LQ_DEV void load_site(typename P::real* __restrict__ v, const char* __restrict__ f, long long ns, long long i) {
+LQ_DEV void load_site_raw(typename P::real* __restrict__ v, typename P::real& scale, const char* __restrict__ f, long long ns, long long i) {
   if constexpr (!P::HALF) {
     Rec<typename P::store_t, N>::load(v, f, ns, i);
+    scale = 1;
   } else {
-    alignas(16) short q[N];
-    Rec<short, N>::load(q, f, ns, i);
-    const float n = ld_nc(reinterpret_cast<const float*>(f + (long long)(2 * N) * ns) + i) * LQ_FIXED_INV;
+    alignas(16) unsigned w[N / 2];
+    Rec<unsigned, N / 2>::load(w, f, ns, i);
+    scale = ld_nc(reinterpret_cast<const float*>(f + (long long)(2 * N) * ns) + i) * LQ_FIXED_INV;
 #pragma unroll
-    for (int k = 0; k < N; ++k) v[k] = (float)q[k] * n;
+    for (int k = 0; k < N / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
+  }
+}
+
+template <class P, int N>
+LQ_DEV void load_site(typename P::real* __restrict__ v, const char* __restrict__ f, long long ns, long long i) {
+  typename P::real sc;
+  load_site_raw<P, N>(v, sc, f, ns, i);
+  if constexpr (P::HALF) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) v[k] *= sc;
   }
 }
 
@@ -99,10 +129,10 @@ LQ_DEV void store_site(const typename P::real* __restrict__ v, char* __restrict_
 #pragma unroll
     for (int k = 0; k < N; ++k) m = fmaxf(m, fabsf(v[k]));
     const float sc = (m > 0.f) ? (LQ_FIXED_MAX / m) : 0.f;
-    alignas(16) short q[N];
+    alignas(16) unsigned w[N / 2];
 #pragma unroll
-    for (int k = 0; k < N; ++k) q[k] = (short)__float2int_rn(v[k] * sc);
-    Rec<short, N>::store(q, f, ns, i);
+    for (int k = 0; k < N / 2; ++k) w[k] = fixed_pack(v[2 * k], v[2 * k + 1], sc);
+    Rec<unsigned, N / 2>::store(w, f, ns, i);
     reinterpret_cast<float*>(f + (long long)(2 * N) * ns)[i] = m;
   }
 }
@@ -121,22 +151,30 @@ LQ_DEV float sqrt_(float x) { return sqrtf(x); }
 LQ_DEV double sqrt_(double x) { return sqrt(x); }
 
 // ---------------------------------------------------------------- gauge links (PAPER.md:164 (a); R10)
-// u[18] = row-major 3x3 complex.  RECON 18: as stored.  12: rows 0,1 stored, row2 = conj(row0 x row1).
-// 8: a2,a3,b1,arg(a1),arg(c1) stored (the parametrisation of ref. [3] of the paper).
+// u[18] = row-major 3x3 complex with (true link) = uscale * u.  RECON 18: as stored.  12: rows
+// 0,1 stored, row2 = conj(row0 x row1).  8: a2,a3,b1,arg(a1),arg(c1) stored (the
+// parametrisation of ref. [3] of the paper).  In half precision the 16-bit integers are kept
+// unscaled (uscale = 1/32767 is folded into the caller's accumulate coefficient).
 template <class P, int RECON>
-LQ_DEV void load_link(typename P::real* __restrict__ u, const char* __restrict__ g, long long ns, long long i) {
+LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale, const char* __restrict__ g, long long ns, long long i) {
   typedef typename P::real R;
-  typedef typename P::store_t S;
-  alignas(16) S raw[RECON];
-  Rec<S, RECON>::load(raw, g, ns, i);
   R v[RECON];
   if constexpr (P::HALF) {
+    alignas(16) unsigned w[RECON / 2];
+    Rec<unsigned, RECON / 2>::load(w, g, ns, i);
 #pragma unroll
-    for (int k = 0; k < RECON; ++k) v[k] = (float)raw[k] * LQ_FIXED_INV;
-    if constexpr (RECON == 8) { v[6] *= 3.14159265358979323846f; v[7] *= 3.14159265358979323846f; }
+    for (int k = 0; k < RECON / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
+    if constexpr (RECON == 8) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) v[k] *= LQ_FIXED_INV;
+      v[6] *= 3.14159265358979323846f * LQ_FIXED_INV; v[7] *= 3.14159265358979323846f * LQ_FIXED_INV;
+      uscale = 1;
+    } else {
+      uscale = LQ_FIXED_INV;
+    }
   } else {
-#pragma unroll
-    for (int k = 0; k < RECON; ++k) v[k] = raw[k];
+    Rec<typename P::store_t, RECON>::load(v, g, ns, i);
+    uscale = 1;
   }
   if constexpr (RECON == 18) {
 #pragma unroll
@@ -144,6 +182,22 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, const char* __restrict__
   } else if constexpr (RECON == 12) {
 #pragma unroll
     for (int k = 0; k < 12; ++k) u[k] = v[k];
+    // row2 = conj(row0 x row1) (times uscale, so that all three rows carry the same scale)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int j = (c + 1) % 3, k = (c + 2) % 3;
+      R re = u[2 * j] * u[6 + 2 * k];
+      re = fma_(-u[2 * j + 1], u[6 + 2 * k + 1], re);
+      re = fma_(-u[2 * k], u[6 + 2 * j], re);
+      re = fma_(u[2 * k + 1], u[6 + 2 * j + 1], re);
+      R im = u[2 * k] * u[6 + 2 * j + 1];
+      im = fma_(u[2 * k + 1], u[6 + 2 * j], im);
+      im = fma_(-u[2 * j], u[6 + 2 * k + 1], im);
+      im = fma_(-u[2 * j + 1], u[6 + 2 * k], im);
+      if constexpr (P::HALF) { re *= LQ_FIXED_INV; im *= LQ_FIXED_INV; }
+      u[12 + 2 * c] = re;
+      u[12 + 2 * c + 1] = im;
+    }
   } else {
     const cx<R> a2 = {v[0], v[1]}, a3 = {v[2], v[3]}, b1 = {v[4], v[5]};
     const R N = a2.re * a2.re + a2.im * a2.im + a3.re * a3.re + a3.im * a3.im;
@@ -170,17 +224,6 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, const char* __restrict__
     u[12] = cc1.re; u[13] = cc1.im;
     u[14] = (b1a3.re - qa2.re) * iN;  u[15] = (b1a3.im - qa2.im) * iN;
     u[16] = -(qa3.re + b1a2.re) * iN; u[17] = -(qa3.im + b1a2.im) * iN;
-  }
-  if constexpr (RECON == 12) {
-    // row2 = conj(row0 x row1)
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      const int j = (c + 1) % 3, k = (c + 2) % 3;
-      const R re = (u[2 * j] * u[6 + 2 * k] - u[2 * j + 1] * u[6 + 2 * k + 1]) - (u[2 * k] * u[6 + 2 * j] - u[2 * k + 1] * u[6 + 2 * j + 1]);
-      const R im = (u[2 * j] * u[6 + 2 * k + 1] + u[2 * j + 1] * u[6 + 2 * k]) - (u[2 * k] * u[6 + 2 * j + 1] + u[2 * k + 1] * u[6 + 2 * j]);
-      u[12 + 2 * c] = re;
-      u[12 + 2 * c + 1] = -im;
-    }
   }
 }
 
@@ -212,7 +255,7 @@ LQ_DEV void quantize_link(const double* __restrict__ v, typename P::store_t* __r
       double x = v[k];
       if (RECON == 8 && k >= 6) x *= (1.0 / 3.14159265358979323846);
       x = fmin(1.0, fmax(-1.0, x));
-      q[k] = (short)__double2int_rn(x * 32767.0);
+      q[k] = (short)(unsigned short)(__double2int_rn(x * 32767.0) + 32768);   // offset binary
     }
   }
 }

@@ -50,53 +50,58 @@ template <> struct GammaRow<1> { static constexpr int j0 = 3, c0 = 2, j1 = 2, c1
 template <> struct GammaRow<2> { static constexpr int j0 = 2, c0 = 1, j1 = 3, c1 = 3; };   // gamma_z
 template <> struct GammaRow<3> { static constexpr int j0 = 2, c0 = 0, j1 = 3, c1 = 0; };   // gamma_t
 
-// One hop: acc += sgn * (1 + sigma*gamma_MU) W psi,  W = U (FWD) or U^dagger (!FWD).
+// One hop: acc += coef * (1 + sigma*gamma_MU) W psi,  W = U (FWD) or U^dagger (!FWD).
+// coef carries the boundary sign and, in half precision, the spinor norm and the link scale.
+// All multiply-adds are written as explicit FMAs (nvcc does not re-associate a*b - c*d + e).
 template <int MU, bool FWD, typename R>
-LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restrict__ u, R sigma, R sgn) {
+LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restrict__ u, R sigma, R coef) {
   typedef GammaRow<MU> G;
   // project: h0 = psi_0 + sigma*c0*psi_j0, h1 = psi_1 + sigma*c1*psi_j1   (3 colours each)
   cx<R> h[2][3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const cx<R> p0 = {psi[2 * c], psi[2 * c + 1]};
-    const cx<R> p1 = {psi[6 + 2 * c], psi[6 + 2 * c + 1]};
     const cx<R> q0 = unit_mul<G::c0>(cx<R>{psi[6 * G::j0 + 2 * c], psi[6 * G::j0 + 2 * c + 1]});
     const cx<R> q1 = unit_mul<G::c1>(cx<R>{psi[6 * G::j1 + 2 * c], psi[6 * G::j1 + 2 * c + 1]});
-    h[0][c] = {p0.re + sigma * q0.re, p0.im + sigma * q0.im};
-    h[1][c] = {p1.re + sigma * q1.re, p1.im + sigma * q1.im};
+    h[0][c] = {fma_(sigma, q0.re, psi[2 * c]), fma_(sigma, q0.im, psi[2 * c + 1])};
+    h[1][c] = {fma_(sigma, q1.re, psi[6 + 2 * c]), fma_(sigma, q1.im, psi[6 + 2 * c + 1])};
   }
-  // colour multiply
+  // colour multiply: 6 FMA per real output
   cx<R> w[2][3];
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
-      R re = 0, im = 0;
+      R re, im;
+      if (FWD) {                         // sum_k U[r][k] * h[k]
+        re = u[6 * r] * h[s][0].re;             im = u[6 * r] * h[s][0].im;
+        re = fma_(-u[6 * r + 1], h[s][0].im, re); im = fma_(u[6 * r + 1], h[s][0].re, im);
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        if (FWD) {                       // U[r][k] * h[k]
-          const R ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
-          re += ur * h[s][k].re - ui * h[s][k].im;
-          im += ur * h[s][k].im + ui * h[s][k].re;
-        } else {                         // conj(U[k][r]) * h[k]
-          const R ur = u[6 * k + 2 * r], ui = u[6 * k + 2 * r + 1];
-          re += ur * h[s][k].re + ui * h[s][k].im;
-          im += ur * h[s][k].im - ui * h[s][k].re;
+        for (int k = 1; k < 3; ++k) {
+          re = fma_(u[6 * r + 2 * k], h[s][k].re, re);      im = fma_(u[6 * r + 2 * k], h[s][k].im, im);
+          re = fma_(-u[6 * r + 2 * k + 1], h[s][k].im, re); im = fma_(u[6 * r + 2 * k + 1], h[s][k].re, im);
+        }
+      } else {                           // sum_k conj(U[k][r]) * h[k]
+        re = u[2 * r] * h[s][0].re;             im = u[2 * r] * h[s][0].im;
+        re = fma_(u[2 * r + 1], h[s][0].im, re);  im = fma_(-u[2 * r + 1], h[s][0].re, im);
+#pragma unroll
+        for (int k = 1; k < 3; ++k) {
+          re = fma_(u[6 * k + 2 * r], h[s][k].re, re);     im = fma_(u[6 * k + 2 * r], h[s][k].im, im);
+          re = fma_(u[6 * k + 2 * r + 1], h[s][k].im, re); im = fma_(-u[6 * k + 2 * r + 1], h[s][k].re, im);
         }
       }
       w[s][r] = {re, im};
     }
   }
   // reconstruct: r_0 = w0, r_1 = w1, r_j0 = sigma*conj(c0)*w0, r_j1 = sigma*conj(c1)*w1
-  const R ss = sgn * sigma;
+  const R ss = coef * sigma;
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    acc[2 * c] += sgn * w[0][c].re;      acc[2 * c + 1] += sgn * w[0][c].im;
-    acc[6 + 2 * c] += sgn * w[1][c].re;  acc[6 + 2 * c + 1] += sgn * w[1][c].im;
+    acc[2 * c] = fma_(coef, w[0][c].re, acc[2 * c]);          acc[2 * c + 1] = fma_(coef, w[0][c].im, acc[2 * c + 1]);
+    acc[6 + 2 * c] = fma_(coef, w[1][c].re, acc[6 + 2 * c]);  acc[6 + 2 * c + 1] = fma_(coef, w[1][c].im, acc[6 + 2 * c + 1]);
     const cx<R> t0 = unit_mul<(4 - G::c0) % 4>(w[0][c]);
     const cx<R> t1 = unit_mul<(4 - G::c1) % 4>(w[1][c]);
-    acc[6 * G::j0 + 2 * c] += ss * t0.re; acc[6 * G::j0 + 2 * c + 1] += ss * t0.im;
-    acc[6 * G::j1 + 2 * c] += ss * t1.re; acc[6 * G::j1 + 2 * c + 1] += ss * t1.im;
+    acc[6 * G::j0 + 2 * c] = fma_(ss, t0.re, acc[6 * G::j0 + 2 * c]); acc[6 * G::j0 + 2 * c + 1] = fma_(ss, t0.im, acc[6 * G::j0 + 2 * c + 1]);
+    acc[6 * G::j1 + 2 * c] = fma_(ss, t1.re, acc[6 * G::j1 + 2 * c]); acc[6 * G::j1 + 2 * c + 1] = fma_(ss, t1.im, acc[6 * G::j1 + 2 * c + 1]);
   }
 }
 
@@ -116,16 +121,31 @@ LQ_DEV void clover_mul(R* __restrict__ out, const R* __restrict__ in, const R* _
       for (int j = 0; j < 6; ++j) {
         if (j < i) {
           const R lr = c[6 + 2 * (i * (i - 1) / 2 + j)], li = c[6 + 2 * (i * (i - 1) / 2 + j) + 1];
-          re += lr * x[2 * j] - li * x[2 * j + 1];
-          im += lr * x[2 * j + 1] + li * x[2 * j];
+          re = fma_(lr, x[2 * j], re);     re = fma_(-li, x[2 * j + 1], re);
+          im = fma_(lr, x[2 * j + 1], im); im = fma_(li, x[2 * j], im);
         } else if (j > i) {
           const R lr = c[6 + 2 * (j * (j - 1) / 2 + i)], li = c[6 + 2 * (j * (j - 1) / 2 + i) + 1];
-          re += lr * x[2 * j] + li * x[2 * j + 1];
-          im += lr * x[2 * j + 1] - li * x[2 * j];
+          re = fma_(lr, x[2 * j], re);     re = fma_(li, x[2 * j + 1], re);
+          im = fma_(lr, x[2 * j + 1], im); im = fma_(-li, x[2 * j], im);
         }
       }
       o[2 * i] = re; o[2 * i + 1] = im;
     }
+  }
+}
+
+// out = C in with C read from a packed clover field; in half precision the per-site norm is
+// applied to the 24 outputs instead of the 72 stored entries.
+template <class P>
+LQ_DEV void clover_site(typename P::real* __restrict__ out, const typename P::real* __restrict__ in,
+                        const char* __restrict__ clov, long long ns, long long idx) {
+  typedef typename P::real R;
+  R cl[72], sc;
+  load_site_raw<P, 72>(cl, sc, clov, ns, idx);
+  clover_mul<R>(out, in, cl);
+  if constexpr (P::HALF) {
+#pragma unroll
+    for (int k = 0; k < 24; ++k) out[k] *= sc;
   }
 }
 
@@ -154,10 +174,17 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
   }
 }
 
+#ifndef LQ_DSLASH_BLOCK
 #define LQ_DSLASH_BLOCK 128
+#endif
+// minimum resident CTAs per SM: caps registers at 80 for the fp32-arithmetic kernels (6 CTAs =
+// 24 warps/SM; measured best, profiles/r1_occupancy_sweep.md); fp64 needs the registers.
+#ifndef LQ_DSLASH_MINB
+#define LQ_DSLASH_MINB 6
+#endif
 
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
-__global__ void __launch_bounds__(LQ_DSLASH_BLOCK)
+__global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? 1 : LQ_DSLASH_MINB))
 dslash_kernel(const DslashArgs a) {
   typedef typename P::real R;
   const Geom& g = a.g;
@@ -201,17 +228,17 @@ dslash_kernel(const DslashArgs a) {
     {                                                                                           \
       const R sf = (c[MU] + 1 == g.X[MU]) ? (R)g.bc[MU] : R(1);                                 \
       if (sf != R(0)) {                                                                         \
-        R u[18], psi[24];                                                                       \
-        load_link<P, RECON>(u, g_out + MU * link_bytes, g.ns, idx);                             \
-        load_site<P, 24>(psi, a.in, g.ns, base + nf[MU]);                                       \
-        hop<MU, true, R>(acc, psi, u, sig_f, sf);                                               \
+        R u[18], psi[24], us, ps;                                                               \
+        load_link<P, RECON>(u, us, g_out + MU * link_bytes, g.ns, idx);                         \
+        load_site_raw<P, 24>(psi, ps, a.in, g.ns, base + nf[MU]);                               \
+        hop<MU, true, R>(acc, psi, u, sig_f, P::HALF ? sf * us * ps : sf);                      \
       }                                                                                         \
       const R sb = (c[MU] == 0) ? (R)g.bc[MU] : R(1);                                           \
       if (sb != R(0)) {                                                                         \
-        R u[18], psi[24];                                                                       \
-        load_link<P, RECON>(u, g_in + MU * link_bytes, g.ns, base + nbk[MU]);                   \
-        load_site<P, 24>(psi, a.in, g.ns, base + nbk[MU]);                                      \
-        hop<MU, false, R>(acc, psi, u, -sig_f, sb);                                             \
+        R u[18], psi[24], us, ps;                                                               \
+        load_link<P, RECON>(u, us, g_in + MU * link_bytes, g.ns, base + nbk[MU]);               \
+        load_site_raw<P, 24>(psi, ps, a.in, g.ns, base + nbk[MU]);                              \
+        hop<MU, false, R>(acc, psi, u, -sig_f, P::HALF ? sb * us * ps : sb);                    \
       }                                                                                         \
     }
     LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3)
@@ -222,20 +249,18 @@ dslash_kernel(const DslashArgs a) {
       load_site<P, 24>(yv, a.y, g.ns, idx);
       const R coef = (R)a.a;
       if constexpr (CLOVX) {
-        R cl[72], ay[24];
-        load_site<P, 72>(cl, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
-        clover_mul<R>(ay, yv, cl);
+        R ay[24];
+        clover_site<P>(ay, yv, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
 #pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = ay[k] + coef * acc[k];
+        for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], ay[k]);
       } else {
 #pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = yv[k] + coef * acc[k];
+        for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], yv[k]);
       }
     }
     if constexpr (CLOVOUT) {
-      R cl[72], t[24];
-      load_site<P, 72>(cl, a.clov_out + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
-      clover_mul<R>(t, acc, cl);
+      R t[24];
+      clover_site<P>(t, acc, a.clov_out + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
 #pragma unroll
       for (int k = 0; k < 24; ++k) acc[k] = t[k];
     }
