@@ -30,8 +30,27 @@ struct PrecS { typedef float  store_t; typedef float  real; static constexpr boo
 struct PrecH { typedef short  store_t; typedef float  real; static constexpr bool HALF = true;  static constexpr int ID = 2; };
 
 #define LQ_DEV __device__ __forceinline__
+#ifndef LQ_GAUGE_STREAM
+#define LQ_GAUGE_STREAM true
+#endif
 
 template <typename V> LQ_DEV V ld_nc(const V* p) { return __ldg(p); }
+// streaming variants for data with no reuse (gauge links): do not allocate in L1
+LQ_DEV int4 ld_stream(const int4* p) {
+  int4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+LQ_DEV int2 ld_stream(const int2* p) {
+  int2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
+LQ_DEV int ld_stream(const int* p) {
+  int v;
+  asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
 
 // ---------------------------------------------------------------- packed records
 template <typename T, int N>
@@ -43,18 +62,22 @@ struct Rec {
   static constexpr int E16 = 16 / (int)sizeof(T), E8 = 8 / (int)sizeof(T), E4 = 4 / (int)sizeof(T);
   static_assert(BYTES % 4 == 0, "record must be a multiple of 4 bytes");
 
+  template <bool STREAM = false>
   LQ_DEV static void load(T* __restrict__ v, const char* __restrict__ base, long long ns, long long i) {
 #pragma unroll
     for (int k = 0; k < N16; ++k) {
-      int4 t = ld_nc(reinterpret_cast<const int4*>(base + 16ll * k * ns) + i);
+      const int4* p = reinterpret_cast<const int4*>(base + 16ll * k * ns) + i;
+      int4 t = STREAM ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int4*>(v + k * E16) = t;
     }
     if (N8) {
-      int2 t = ld_nc(reinterpret_cast<const int2*>(base + 16ll * N16 * ns) + i);
+      const int2* p = reinterpret_cast<const int2*>(base + 16ll * N16 * ns) + i;
+      int2 t = STREAM ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int2*>(v + N16 * E16) = t;
     }
     if (N4) {
-      int t = ld_nc(reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i);
+      const int* p = reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i;
+      int t = STREAM ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int*>(v + N16 * E16 + N8 * E8) = t;
     }
   }
@@ -161,7 +184,7 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
   R v[RECON];
   if constexpr (P::HALF) {
     alignas(16) unsigned w[RECON / 2];
-    Rec<unsigned, RECON / 2>::load(w, g, ns, i);
+    Rec<unsigned, RECON / 2>::template load<LQ_GAUGE_STREAM>(w, g, ns, i);
 #pragma unroll
     for (int k = 0; k < RECON / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
     if constexpr (RECON == 8) {
@@ -173,7 +196,7 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
       uscale = LQ_FIXED_INV;
     }
   } else {
-    Rec<typename P::store_t, RECON>::load(v, g, ns, i);
+    Rec<typename P::store_t, RECON>::template load<LQ_GAUGE_STREAM>(v, g, ns, i);
     uscale = 1;
   }
   if constexpr (RECON == 18) {
