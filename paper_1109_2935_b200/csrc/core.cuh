@@ -31,7 +31,7 @@ struct PrecH { typedef short  store_t; typedef float  real; static constexpr boo
 
 #define LQ_DEV __device__ __forceinline__
 #ifndef LQ_GAUGE_STREAM
-#define LQ_GAUGE_STREAM true
+#define LQ_GAUGE_STREAM 1
 #endif
 
 template <typename V> LQ_DEV V ld_nc(const V* p) { return __ldg(p); }
@@ -46,6 +46,34 @@ LQ_DEV int2 ld_stream(const int2* p) {
   asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
   return v;
 }
+LQ_DEV unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+LQ_DEV int4 ld_shared(const int4* p) {
+  int4 v;
+  asm volatile("ld.shared.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_addr(p)) : "memory");
+  return v;
+}
+LQ_DEV int2 ld_shared(const int2* p) {
+  int2 v;
+  asm volatile("ld.shared.v2.s32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(smem_addr(p)) : "memory");
+  return v;
+}
+LQ_DEV int ld_shared(const int* p) {
+  int v;
+  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_addr(p)) : "memory");
+  return v;
+}
+// asynchronous global -> shared copies (LDGSTS): the bytes in flight occupy no registers
+template <int BYTES> LQ_DEV void cp_async(void* smem_dst, const void* gsrc) {
+  if constexpr (BYTES == 16)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr(smem_dst)), "l"(gsrc) : "memory");
+  else if constexpr (BYTES == 8)
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(smem_dst)), "l"(gsrc) : "memory");
+  else
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr(smem_dst)), "l"(gsrc) : "memory");
+}
+LQ_DEV void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> LQ_DEV void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 LQ_DEV int ld_stream(const int* p) {
   int v;
   asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
@@ -62,24 +90,34 @@ struct Rec {
   static constexpr int E16 = 16 / (int)sizeof(T), E8 = 8 / (int)sizeof(T), E4 = 4 / (int)sizeof(T);
   static_assert(BYTES % 4 == 0, "record must be a multiple of 4 bytes");
 
-  template <bool STREAM = false>
+  // MODE 0: read-only global (ld.global.nc), 1: streaming global (no L1 allocation),
+  // 2: shared memory staging buffer laid out like a packed field with ns = CTA size, i = thread
+  template <int MODE = 0>
   LQ_DEV static void load(T* __restrict__ v, const char* __restrict__ base, long long ns, long long i) {
 #pragma unroll
     for (int k = 0; k < N16; ++k) {
       const int4* p = reinterpret_cast<const int4*>(base + 16ll * k * ns) + i;
-      int4 t = STREAM ? ld_stream(p) : ld_nc(p);
+      int4 t = MODE == 2 ? ld_shared(p) : MODE == 1 ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int4*>(v + k * E16) = t;
     }
     if (N8) {
       const int2* p = reinterpret_cast<const int2*>(base + 16ll * N16 * ns) + i;
-      int2 t = STREAM ? ld_stream(p) : ld_nc(p);
+      int2 t = MODE == 2 ? ld_shared(p) : MODE == 1 ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int2*>(v + N16 * E16) = t;
     }
     if (N4) {
       const int* p = reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i;
-      int t = STREAM ? ld_stream(p) : ld_nc(p);
+      int t = MODE == 2 ? ld_shared(p) : MODE == 1 ? ld_stream(p) : ld_nc(p);
       *reinterpret_cast<int*>(v + N16 * E16 + N8 * E8) = t;
     }
+  }
+  // record i of the global field -> record `tid` of a staging buffer of `nt` records
+  LQ_DEV static void stage(char* __restrict__ sbase, int nt, int tid, const char* __restrict__ base, long long ns, long long i) {
+#pragma unroll
+    for (int k = 0; k < N16; ++k)
+      cp_async<16>(sbase + 16 * k * nt + 16 * tid, reinterpret_cast<const int4*>(base + 16ll * k * ns) + i);
+    if (N8) cp_async<8>(sbase + 16 * N16 * nt + 8 * tid, reinterpret_cast<const int2*>(base + 16ll * N16 * ns) + i);
+    if (N4) cp_async<4>(sbase + (16 * N16 + 8 * N8) * nt + 4 * tid, reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i);
   }
   LQ_DEV static void store(const T* __restrict__ v, char* __restrict__ base, long long ns, long long i) {
 #pragma unroll
@@ -119,15 +157,16 @@ LQ_DEV unsigned fixed_pack(float a, float b, float sc) {
 // R9: half = 16-bit fixed point q_i = rint(v_i * 32767 / n), n = max_i |v_i| (fp32) per site; decode v_i = q_i * n/32767.
 // load_site_raw returns v and scale with (true value) = scale * v, so that callers can fold
 // the scale into an FMA coefficient instead of spending one FMUL per element.
-template <class P, int N>
+template <class P, int N, int MODE = 0>
 LQ_DEV void load_site_raw(typename P::real* __restrict__ v, typename P::real& scale, const char* __restrict__ f, long long ns, long long i) {
   if constexpr (!P::HALF) {
-    Rec<typename P::store_t, N>::load(v, f, ns, i);
+    Rec<typename P::store_t, N>::template load<MODE>(v, f, ns, i);
     scale = 1;
   } else {
     alignas(16) unsigned w[N / 2];
-    Rec<unsigned, N / 2>::load(w, f, ns, i);
-    scale = ld_nc(reinterpret_cast<const float*>(f + (long long)(2 * N) * ns) + i) * LQ_FIXED_INV;
+    Rec<unsigned, N / 2>::template load<MODE>(w, f, ns, i);
+    const int* np = reinterpret_cast<const int*>(f + (long long)(2 * N) * ns) + i;
+    scale = __int_as_float(MODE == 2 ? ld_shared(np) : ld_nc(np)) * LQ_FIXED_INV;
 #pragma unroll
     for (int k = 0; k < N / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
   }
@@ -178,13 +217,13 @@ LQ_DEV double sqrt_(double x) { return sqrt(x); }
 // 0,1 stored, row2 = conj(row0 x row1).  8: a2,a3,b1,arg(a1),arg(c1) stored (the
 // parametrisation of ref. [3] of the paper).  In half precision the 16-bit integers are kept
 // unscaled (uscale = 1/32767 is folded into the caller's accumulate coefficient).
-template <class P, int RECON>
+template <class P, int RECON, int MODE = LQ_GAUGE_STREAM>
 LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale, const char* __restrict__ g, long long ns, long long i) {
   typedef typename P::real R;
   R v[RECON];
   if constexpr (P::HALF) {
     alignas(16) unsigned w[RECON / 2];
-    Rec<unsigned, RECON / 2>::template load<LQ_GAUGE_STREAM>(w, g, ns, i);
+    Rec<unsigned, RECON / 2>::template load<MODE>(w, g, ns, i);
 #pragma unroll
     for (int k = 0; k < RECON / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
     if constexpr (RECON == 8) {
@@ -196,7 +235,7 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
       uscale = LQ_FIXED_INV;
     }
   } else {
-    Rec<typename P::store_t, RECON>::template load<LQ_GAUGE_STREAM>(v, g, ns, i);
+    Rec<typename P::store_t, RECON>::template load<MODE>(v, g, ns, i);
     uscale = 1;
   }
   if constexpr (RECON == 18) {

@@ -183,7 +183,19 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
 #define LQ_DSLASH_MINB 6
 #endif
 
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+// bytes of one staging buffer (one hop of every thread of the CTA): link + neighbour spinor (+ norm)
+template <class P, int RECON> struct HopStage {
+  static constexpr int LINK_B = RECON * (int)sizeof(typename P::store_t);
+  static constexpr int SPIN_B = site_bytes<P>(24, true);
+  static constexpr int BYTES = LQ_DSLASH_BLOCK * (LINK_B + SPIN_B);
+};
+
+// NST = 0: neighbour data is loaded straight into registers (fp64).
+// NST > 0: software pipeline over the 8 hops through NST per-thread staging buffers in shared
+// memory filled by cp.async: while hop h is computed, the loads of hops h+1 .. h+NST-1 are in
+// flight without holding registers.  The slots are private to a thread, so no CTA barrier is
+// needed: cp.async.wait_group orders a thread's own copies.
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST>
 __global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? 1 : LQ_DSLASH_MINB))
 dslash_kernel(const DslashArgs a) {
   typedef typename P::real R;
@@ -224,6 +236,7 @@ dslash_kernel(const DslashArgs a) {
       nbk[3] = (c[3] == 0) ? cb + (g.X[3] - 1) * st : cb - st;
     }
 
+    if constexpr (NST == 0) {
     // a hop that crosses an open (Dirichlet) boundary gets coefficient 0; its loads stay inside
     // the box (wrapped index), so no branch is needed and the hops can be scheduled freely
 #define LQ_HOP(MU)                                                                              \
@@ -245,6 +258,51 @@ dslash_kernel(const DslashArgs a) {
     }
     LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3)
 #undef LQ_HOP
+    } else {
+      extern __shared__ __align__(16) char lq_stage[];
+      typedef HopStage<P, RECON> HS;
+      const int tid = threadIdx.x;
+      // hop h: mu = h/2, forward for even h.  Issue = start the async copies of its link and spinor.
+#define LQ_ISSUE(H)                                                                                        \
+      {                                                                                                    \
+        constexpr int MU_ = (H) / 2;                                                                       \
+        constexpr bool FW_ = ((H) & 1) == 0;                                                               \
+        char* sb_ = lq_stage + ((H) % NST) * HS::BYTES;                                                    \
+        const long long li_ = FW_ ? idx : base + nbk[MU_];                                                 \
+        const long long si_ = FW_ ? base + nf[MU_] : base + nbk[MU_];                                      \
+        Rec<typename P::store_t, RECON>::stage(sb_, LQ_DSLASH_BLOCK, tid, (FW_ ? g_out : g_in) + MU_ * link_bytes, g.ns, li_); \
+        char* ss_ = sb_ + LQ_DSLASH_BLOCK * HS::LINK_B;                                                    \
+        Rec<typename P::store_t, 24>::stage(ss_, LQ_DSLASH_BLOCK, tid, a.in, g.ns, si_);                   \
+        if (P::HALF) cp_async<4>(ss_ + 48 * LQ_DSLASH_BLOCK + 4 * tid, reinterpret_cast<const float*>(a.in + 48ll * g.ns) + si_); \
+      }
+#define LQ_PHOP(H)                                                                                         \
+      {                                                                                                    \
+        constexpr int MU_ = (H) / 2;                                                                       \
+        constexpr bool FW_ = ((H) & 1) == 0;                                                               \
+        cp_async_wait<NST - 1>();                                                                          \
+        const char* sb_ = lq_stage + ((H) % NST) * HS::BYTES;                                              \
+        R u[18], psi[24], us, ps;                                                                          \
+        load_link<P, RECON, 2>(u, us, sb_, LQ_DSLASH_BLOCK, tid);                                          \
+        load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);        \
+        if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                       \
+        cp_async_commit();                                                                                 \
+        const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
+        hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, P::HALF ? sg_ * us * ps : sg_);                \
+      }
+#pragma unroll
+      for (int h = 0; h < NST; ++h) {
+        switch (h) {                       // NST <= 4
+          case 0: LQ_ISSUE(0) break;
+          case 1: LQ_ISSUE(1) break;
+          case 2: LQ_ISSUE(2) break;
+          default: LQ_ISSUE(3) break;
+        }
+        cp_async_commit();
+      }
+      LQ_PHOP(0) LQ_PHOP(1) LQ_PHOP(2) LQ_PHOP(3) LQ_PHOP(4) LQ_PHOP(5) LQ_PHOP(6) LQ_PHOP(7)
+#undef LQ_PHOP
+#undef LQ_ISSUE
+    }
 
     R yv[24];
     if constexpr (XPAY) {

@@ -5,17 +5,40 @@
 
 namespace lq {
 
+#ifndef LQ_PIPE_FP32
+#define LQ_PIPE_FP32 2
+#endif
+#ifndef LQ_PIPE_HALF
+#define LQ_PIPE_HALF 3
+#endif
+
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
+  constexpr int NST = sizeof(typename P::real) == 8 ? 0 : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
+  constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
+  auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST>;
+  if (NST > 0) {
+    static bool configured = false;       // per instantiation
+    if (!configured) {
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+      cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+      configured = true;
+    }
+  }
+  kern<<<grid, block, SMEM, s>>>(a);
+}
+
 template <class P, int RECON>
 static cudaError_t launch_dslash_r(const DslashArgs& a, int epi, cudaStream_t s) {
   dim3 grid((a.g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);
   dim3 block(LQ_DSLASH_BLOCK);
   switch (epi) {
-    case EPI_NONE:            dslash_kernel<P, RECON, false, false, false, false><<<grid, block, 0, s>>>(a); break;
-    case EPI_CLOVOUT:         dslash_kernel<P, RECON, false, false, true,  false><<<grid, block, 0, s>>>(a); break;
-    case EPI_CLOVX_XPAY:      dslash_kernel<P, RECON, true,  true,  false, false><<<grid, block, 0, s>>>(a); break;
-    case EPI_XPAY:            dslash_kernel<P, RECON, true,  false, false, false><<<grid, block, 0, s>>>(a); break;
-    case EPI_XPAY_CLOVOUT:    dslash_kernel<P, RECON, true,  false, true,  false><<<grid, block, 0, s>>>(a); break;
-    case EPI_CLOVX_XPAY_DOTS: dslash_kernel<P, RECON, true,  true,  false, true ><<<grid, block, 0, s>>>(a); break;
+    case EPI_NONE:            launch_one<P, RECON, false, false, false, false>(a, grid, block, s); break;
+    case EPI_CLOVOUT:         launch_one<P, RECON, false, false, true, false>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY:      launch_one<P, RECON, true, true, false, false>(a, grid, block, s); break;
+    case EPI_XPAY:            launch_one<P, RECON, true, false, false, false>(a, grid, block, s); break;
+    case EPI_XPAY_CLOVOUT:    launch_one<P, RECON, true, false, true, false>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY_DOTS: launch_one<P, RECON, true, true, false, true>(a, grid, block, s); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();
