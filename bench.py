@@ -43,6 +43,13 @@ def matpc_bytes(prec, recon):
     return 5 * SPINOR_B[prec] + 16 * recon * LINK_B[prec] + 2 * CLOVER_B[prec]
 
 
+# ncu --set full captures of one launch at 32^3x64 (profiles/r1_dslash_*.md): DRAM bytes read + written,
+# and executed warp instructions (the half-precision kernels are issue-bound)
+NCU_TRAFFIC = {("fp32", 12): 595.03e6, ("half", 12): 298.28e6}
+NCU_WARP_INST = {("half", 12): 76.15e6}
+N_SCHEDULERS = 148 * 4      # one warp instruction per scheduler per clock (B200: 148 SMs x 4 SMSPs)
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -152,6 +159,8 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--full", action="store_true", help="also run config 5 (48^3x96 GCR-DD vs BiCGstab)")
     ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
+    ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"], help="storage precision of the timed Dslash")
+    ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8], help="link compression of the timed Dslash")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -182,7 +191,11 @@ def main():
     ctx = lqcd.Context(DIMS, BC, local)
     ctx.load_gauge(U)
     ctx.build_clover(CSW)
-    prec, recon = lqcd.PREC_SINGLE, lqcd.RECON_12
+    prec = {"fp64": lqcd.PREC_DOUBLE, "fp32": lqcd.PREC_SINGLE, "half": lqcd.PREC_HALF}[args.prec]
+    recon = args.recon
+    pname = {"fp64": "fp64 storage+arithmetic", "fp32": "fp32 storage+arithmetic",
+             "half": "16-bit fixed point + per-site fp32 norm storage, fp32 arithmetic"}[args.prec]
+    dtype = {"fp64": "f64", "fp32": "f32", "half": "i16+f32"}[args.prec]
     f = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
     g = [ctx.new_field(prec) for _ in (0, 1)]
 
@@ -230,21 +243,31 @@ def main():
     out = {
         "metric": "wilson_clover_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": {"workload": "config 3: 32^3x64, eps=0.3, full-lattice Wilson-clover Dslash (both parities)",
-                   "precision": "fp32 storage+arithmetic", "recon": 12, "flop_per_site": FLOP_DSLASH,
+                   "precision": pname, "recon": recon, "flop_per_site": FLOP_DSLASH,
                    "l2": "inputs larger than L2 (gauge 403 MB + spinors 201 MB per step vs 126 MB L2)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                     "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_kind": pk_kind,
-                     "kernel": "dslash_kernel<PrecS,12> (EPI_NONE)", "algorithmic_bytes_per_launch": algo_bytes,
-                     "frac_of_8TBs_nominal": achieved / 8000.0},
+                     "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC.get((args.prec, recon)), "peak_kind": pk_kind,
+                     "kernel": "dslash_kernel<%s,%d> (EPI_NONE)" % (args.prec, recon), "algorithmic_bytes_per_launch": algo_bytes,
+                     "frac_of_8TBs_nominal": achieved / 8000.0,
+                     "traffic_source": "profiles/r1_dslash_%s_r%d.md" % (args.prec, recon) if (args.prec, recon) in NCU_TRAFFIC else None},
         "e2e": {"value": FLOP_DSLASH * V * world / (e2e_ms / e2e_steps * 1e-3) / 1e9, "unit": "GFLOP/s",
                 "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps},
         "gpu_launches": launches,
         "clocks": clocks,
     }
 
+    if (args.prec, recon) in NCU_WARP_INST:
+        # issue-bound kernel: executed warp instructions per launch (ncu) / time vs 1 per scheduler per clock
+        ips = NCU_WARP_INST[(args.prec, recon)] / (kern_ms * 1e-3) / 1e9
+        ipeak = N_SCHEDULERS * pk["sm_max_mhz"] * 1e-3
+        out["roofline_hbm"] = out["roofline"]
+        out["roofline"] = {"bound": "alu", "achieved": ips, "peak": ipeak, "unit": "G warp-inst/s", "frac": ips / ipeak,
+                           "traffic": NCU_TRAFFIC.get((args.prec, recon)), "kernel": out["roofline_hbm"]["kernel"],
+                           "peak_kind": "148 SMs x 4 schedulers x 1 warp instruction/clk x sm_max_mhz (DESIGN.md 6.1)",
+                           "warp_instructions_per_launch": NCU_WARP_INST[(args.prec, recon)]}
     if rank == 0 and not args.quick:
         out["extra"] = extras(ctx, psi, args, torch, lqcd, inputs, pk)
         n_apps = 10
