@@ -153,9 +153,15 @@ int lqcd_invert(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical,
                 const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
 
 /* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */
-/* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned or pageable).
+/* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned for full PCIe speed;
+ * pageable works), owned by the caller, not overlapping.
  * out = D in on both parities (op == 0) or out_p = Mhat in_p on `parity`, rest zero (op == 1),
- * computed in (prec, recon).  Synchronises `stream`. */
+ * computed in (prec, recon).  The call pipelines host->device copy, pack, operator, unpack and
+ * device->host copy over slabs of time slices on two internal copy streams plus `stream`
+ * (staging buffers are cached in the context); it starts after the work already queued on
+ * `stream` and returns after everything, including the copy back, has completed.
+ * Errors: LQCD_EINVAL (null pointer, bad op/parity/prec/recon), LQCD_ESTATE (no gauge / clover),
+ * LQCD_ENOMEM, LQCD_ECUDA. */
 int lqcd_apply_host(lqcd_ctx* ctx, void* out_host, const void* in_host, int op, int parity, int dagger,
                     double kappa, int prec, int recon, void* stream);
 int lqcd_invert_host(lqcd_ctx* ctx, void* x_host, const void* b_host,

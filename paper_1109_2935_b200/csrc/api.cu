@@ -121,7 +121,7 @@ int set_blocks(lqcd_ctx* c, const int* blk) {
 
 // out = [C] ([A] y + a * D in) : one fused launch (dslash.cuh)
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
-              int epi, double a, double kappa, bool blocked, cudaStream_t s) {
+              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0, int cb1) {
   DslashArgs d;
   memset(&d, 0, sizeof(d));
   d.g = blocked ? c->bm.blk : c->nat;
@@ -134,7 +134,8 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
     if (rc) return rc;
     d.clov_y = A; d.clov_out = Ai;
   }
-  d.dots = c->boxdots;
+  if (epi == EPI_CLOVX_XPAY_DOTS) d.dots = c->boxdots;          // whole boxes (the two share storage, dslash.cuh)
+  else { d.range.cb0 = cb0; d.range.cb1 = cb1 < 0 ? d.g.vh : cb1; }
   cudaError_t e;
   switch (prec) {
     case 0: e = launch_dslash<PrecD>(d, recon, epi, s); break;
@@ -192,6 +193,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   memset(c->tmp, 0, sizeof(c->tmp)); memset(c->btmp, 0, sizeof(c->btmp));
   c->S = nullptr; c->partials = nullptr; c->counters = nullptr; c->boxdots = nullptr; c->hS = nullptr;
   c->boxdots_doubles = 0;
+  memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
+  c->have_hpipe = false;
   cudaDeviceProp prop;
   cudaGetDeviceProperties(&prop, device);
   c->n_sm = prop.multiProcessorCount;
@@ -221,6 +224,11 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->boxdots) cudaFree(c->boxdots);
   if (c->hS) cudaFreeHost(c->hS);
   for (void* p : c->pool) cudaFree(p);
+  for (void* p : c->hws) if (p) cudaFree(p);
+  if (c->have_hpipe) {
+    cudaStreamDestroy(c->hs_in); cudaStreamDestroy(c->hs_out); cudaEventDestroy(c->hev_sync);
+    for (int i = 0; i < LQ_HOST_SLABS; ++i) { cudaEventDestroy(c->hev_in[i]); cudaEventDestroy(c->hev_out[i]); }
+  }
   delete c;
   return LQCD_OK;
 }

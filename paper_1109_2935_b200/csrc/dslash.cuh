@@ -30,10 +30,17 @@ struct DslashArgs {
   const char* clov_y;   // A of the output parity (CLOVX)
   const char* clov_out; // A^-1 of the output parity (CLOVOUT)
   double a;             // xpay coefficient
-  double* dots;         // DOTS: [box][chunk][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
+  // The struct is kept at 128 bytes: one more word and ptxas (12.9, sm_100a) spills ~400 bytes
+  // per thread in the 80-register clover-epilogue variants.  A DOTS launch always covers whole
+  // boxes, so the site range shares storage with the partial-sum pointer.
+  union {
+    double* dots;       // DOTS: [box][chunk][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
+    struct { int cb0, cb1; } range;  // !DOTS: sites [cb0, cb1) of every box are computed by this launch
+  };
   int parity;           // output parity
   int dagger;
 };
+static_assert(sizeof(DslashArgs) == 128, "DslashArgs must stay 128 bytes (see above)");
 
 // multiply by a compile-time unit: C = 0: 1, 1: i, 2: -1, 3: -i
 template <int C, typename R> LQ_DEV cx<R> unit_mul(cx<R> z) {
@@ -200,9 +207,9 @@ __global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 
 dslash_kernel(const DslashArgs a) {
   typedef typename P::real R;
   const Geom& g = a.g;
-  const int cb = blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
+  const int cb = (DOTS ? 0 : a.range.cb0) + blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
   const int box = blockIdx.y;
-  const bool active = cb < g.vh;
+  const bool active = cb < (DOTS ? g.vh : a.range.cb1);
   double red[3] = {0, 0, 0};
   if (active) {
     const long long base = (long long)box * g.vh;
@@ -326,13 +333,16 @@ dslash_kernel(const DslashArgs a) {
     }
     store_site<P, 24>(acc, a.out, g.ns, idx);
     if constexpr (DOTS) {
-      // <r,y> = sum conj(r) y, <r,r>
+      // <r,y> = sum conj(r) y, <r,r>: the 12 terms of one site are summed in the arithmetic
+      // precision (FMA chains), the sums over sites in fp64
+      R d0 = 0, d1 = 0, d2 = 0;
 #pragma unroll
       for (int k = 0; k < 12; ++k) {
-        red[0] += (double)(acc[2 * k] * yv[2 * k] + acc[2 * k + 1] * yv[2 * k + 1]);
-        red[1] += (double)(acc[2 * k] * yv[2 * k + 1] - acc[2 * k + 1] * yv[2 * k]);
-        red[2] += (double)(acc[2 * k] * acc[2 * k] + acc[2 * k + 1] * acc[2 * k + 1]);
+        d0 = fma_(acc[2 * k], yv[2 * k], d0);      d0 = fma_(acc[2 * k + 1], yv[2 * k + 1], d0);
+        d1 = fma_(acc[2 * k], yv[2 * k + 1], d1);  d1 = fma_(-acc[2 * k + 1], yv[2 * k], d1);
+        d2 = fma_(acc[2 * k], acc[2 * k], d2);     d2 = fma_(acc[2 * k + 1], acc[2 * k + 1], d2);
       }
+      red[0] = (double)d0; red[1] = (double)d1; red[2] = (double)d2;
     }
   }
   if constexpr (DOTS) {

@@ -30,7 +30,8 @@ static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
 
 template <class P, int RECON>
 static cudaError_t launch_dslash_r(const DslashArgs& a, int epi, cudaStream_t s) {
-  dim3 grid((a.g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);
+  const int nsite = epi == EPI_CLOVX_XPAY_DOTS ? a.g.vh : a.range.cb1 - a.range.cb0;
+  dim3 grid((nsite + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);
   dim3 block(LQ_DSLASH_BLOCK);
   switch (epi) {
     case EPI_NONE:            launch_one<P, RECON, false, false, false, false>(a, grid, block, s); break;

@@ -7,6 +7,8 @@
 #include "blas.cuh"
 #include "../../include/lqcd.h"
 
+#define LQ_HOST_SLABS 16    /* max t-slabs of the host-buffer pipeline (host_api.cu) */
+
 namespace lq {
 
 // Natural layout <-> block-major layout.  The Schwarz preconditioner sees
@@ -44,7 +46,8 @@ cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStre
 // setup kernels (pack.cu, clover.cu)
 cudaError_t run_pack_gauge(double* g64, const double* U_canonical, const Geom& nat, cudaStream_t s);
 cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s);
-cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s);
+cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
+                            long long i0 = 0, long long i1 = -1);   // sites [i0, i1) of the parity field (default: all)
 cudaError_t run_clover_term(double* T72, const double* g64, const Geom& nat, double c_sw, cudaStream_t s);
 cudaError_t run_clover_make(int prec, char* A, char* Ainv, const double* T72, const BlockMap& bm, int blocked, double kappa, cudaStream_t s);
 cudaError_t run_clover_apply(int prec, char* out, const char* in, const char* clov, const Geom& g, int parity, cudaStream_t s);
@@ -93,4 +96,10 @@ struct lqcd_ctx {
   size_t boxdots_doubles;
   double* hS;             // pinned host mirror of S
   std::vector<void*> pool; // solver workspace allocations released at the end of lqcd_invert
+  // lqcd_apply_host: cached staging buffers, copy streams and events of the slab pipeline
+  void* hws[8];
+  size_t hws_bytes[8];
+  cudaStream_t hs_in, hs_out;
+  cudaEvent_t hev_in[LQ_HOST_SLABS], hev_out[LQ_HOST_SLABS], hev_sync;
+  bool have_hpipe;
 };

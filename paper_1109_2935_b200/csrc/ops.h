@@ -11,7 +11,7 @@ int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A
 int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out);
 int set_blocks(lqcd_ctx* c, const int* blk);
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
-              int epi, double a, double kappa, bool blocked, cudaStream_t s);
+              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0 = 0, int cb1 = -1);
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
              bool blocked, bool dots, cudaStream_t s);
 

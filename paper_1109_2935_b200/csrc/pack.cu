@@ -67,9 +67,9 @@ cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64,
 
 // canonical psi[t][z][y][x][4][3] (complex128) <-> packed parity field of precision P
 template <class P>
-__global__ void pack_spinor_kernel(char* packed, double* canonical, const Geom g, int parity, int unpack) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= g.ns) return;
+__global__ void pack_spinor_kernel(char* packed, double* canonical, const Geom g, int parity, int unpack, long long i0, long long i1) {
+  const long long i = i0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= i1) return;
   int c[4];
   cb_to_coords(g, (int)i, parity, c);
   const long long site = c[0] + (long long)g.X[0] * (c[1] + (long long)g.X[1] * (c[2] + (long long)g.X[2] * c[3]));
@@ -86,13 +86,15 @@ __global__ void pack_spinor_kernel(char* packed, double* canonical, const Geom g
   }
 }
 
-cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s) {
-  dim3 grid((unsigned)((nat.ns + 127) / 128)), block(128);
+cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
+                            long long i0, long long i1) {
+  if (i1 < 0) i1 = nat.ns;
+  dim3 grid((unsigned)((i1 - i0 + 127) / 128)), block(128);
   double* c = const_cast<double*>(canonical);
   switch (prec) {
-    case 0: pack_spinor_kernel<PrecD><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack); break;
-    case 1: pack_spinor_kernel<PrecS><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack); break;
-    case 2: pack_spinor_kernel<PrecH><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack); break;
+    case 0: pack_spinor_kernel<PrecD><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
+    case 1: pack_spinor_kernel<PrecS><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
+    case 2: pack_spinor_kernel<PrecH><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

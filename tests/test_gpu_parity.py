@@ -200,3 +200,46 @@ def test_error_codes(cfg1):
         cfg1.ctx.dslash(f, f, 0, False, 0, 18)                  # aliasing
     assert e.value.code == lqcd.EINVAL
     ctx.close()
+
+
+def test_cfg3_full_size_all_precisions():
+    """BASELINE.json config 3 at full size, 32^3x64 (eps = 0.3, kappa = 0.124, c_sw = 1): the launch
+    configuration bench.py times (8192 CTAs x 128 threads per parity).  Dslash in every precision x
+    compression and Mhat in every precision, element by element against the oracle on the same
+    arrays (the oracle applies D to the full lattice in well under a second)."""
+    from paper_1109_2935_b200 import lqcd
+    dims, kappa = (32, 32, 32, 64), 0.124
+    Ut = inputs.random_gauge_torch(dims, 0.3, 1, device="cuda")
+    pt = inputs.gaussian_spinor_torch(dims, 2, device="cuda")
+    ctx = lqcd.Context(dims, BC, 0)
+    ctx.load_gauge(Ut)
+    ctx.build_clover(1.0)
+    U, psi = Ut.cpu().numpy(), pt.cpu().numpy()
+    del Ut
+    want_d = oracle.dslash(psi, U, BC)                      # both parities at once
+    want_ddag = oracle.dslash(psi, U, BC, dagger=True)
+    T = oracle.clover_term(U, 1.0)
+    want_m = oracle.matpc(psi, U, T, BC, kappa, 0)
+    del T
+    par = torch.from_numpy(inputs.parity_mask(dims)).cuda()
+    wd, wdd, wm = (torch.from_numpy(w).cuda() for w in (want_d, want_ddag, want_m))
+    even = (par == 0)[..., None, None]
+    for prec in (0, 1, 2):
+        fin = [ctx.pack_spinor(pt, p, prec) for p in (0, 1)]
+        fo = [ctx.new_field(prec) for _ in (0, 1)]
+        for recon in (18, 12, 8):
+            tol = TOL[prec] if not (prec == 0 and recon == 8) else 1e-9   # 1/N amplification, min N ~ 2e-5 (R10)
+            for dagger, want in ((False, wd), (True, wdd)):
+                got = torch.zeros_like(pt)
+                for p in (0, 1):
+                    ctx.dslash(fo[p], fin[1 - p], p, dagger, prec, recon)
+                    ctx.unpack_spinor(got, fo[p], p, prec)
+                err = float(torch.linalg.vector_norm(got - want) / torch.linalg.vector_norm(want))
+                assert err <= tol, ("dslash", prec, recon, dagger, err)
+            got = torch.zeros_like(pt)
+            ctx.matpc(fo[0], fin[0], 0, False, kappa, prec, recon)
+            ctx.unpack_spinor(got, fo[0], 0, prec)
+            assert float(torch.count_nonzero(got * ~even)) == 0
+            err = float(torch.linalg.vector_norm(got - wm) / torch.linalg.vector_norm(wm))
+            assert err <= tol, ("matpc", prec, recon, err)
+    ctx.close()
