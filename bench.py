@@ -142,6 +142,24 @@ def time_region_clk(fn, reps, index):
     return e0.elapsed_time(e1), clk
 
 
+def max_over_ranks(ms, device):
+    """Max of a per-rank time over all ranks (replicas only: no data-path collective; this all-reduce of
+    one float is the only communication).  Works on any initialised backend (nccl on GPUs, gloo in the
+    CPU test); identity when torch.distributed is not initialised."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(ms)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gflops(flop_per_rank_step, world, ms_per_step):
+    """Aggregate over N independent replicas: every rank did flop_per_rank_step in (max) ms_per_step."""
+    return flop_per_rank_step * world / (ms_per_step * 1e-3) / 1e9
+
+
 def oracle_dslash_rate(n_apps, U, psi):
     """The oracle, as it stands, on the host cores: full-lattice D applications on the same
     arrays the GPU path was given (numpy complex128, canonical layout)."""
@@ -249,9 +267,7 @@ def main():
     launches = ctx.launch_count() - l0
     if world > 1:
         dist.barrier()
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev)
 
     # ---- e2e: host buffers through lqcd_apply_host -----------------------------------------------
     h_in = psi.cpu().pin_memory()
@@ -260,15 +276,12 @@ def main():
     ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon)
     torch.cuda.synchronize()
     e2e_ms = time_region(lambda: ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon), e2e_steps)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dev)
     clocks = sampler.stop() if rank == 0 else None
     cbytes = V * 12 * 16
 
     ms_step = ms / args.steps
-    value = FLOP_DSLASH * V * world / (ms_step * 1e-3) / 1e9
+    value = whole_job_gflops(FLOP_DSLASH * V, world, ms_step)
     kern_ms = ms / launches
     algo_bytes = dslash_bytes(prec, recon) * Vh
     achieved = algo_bytes / (kern_ms * 1e-3) / 1e9
@@ -286,7 +299,7 @@ def main():
                      "kernel": "dslash_kernel<%s,%d> (EPI_NONE)" % (args.prec, recon), "algorithmic_bytes_per_launch": algo_bytes,
                      "frac_of_8TBs_nominal": achieved / 8000.0,
                      "traffic_source": "profiles/r1_dslash_%s_r%d.md" % (args.prec, recon) if (args.prec, recon) in NCU_TRAFFIC else None},
-        "e2e": {"value": FLOP_DSLASH * V * world / (e2e_ms / e2e_steps * 1e-3) / 1e9, "unit": "GFLOP/s",
+        "e2e": {"value": whole_job_gflops(FLOP_DSLASH * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
                 "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps},
         "gpu_launches": launches,
         "clocks": clocks,
