@@ -144,7 +144,16 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
     double maxr = rn;
     int it = 0;
     while (true) {
-      if (it >= p.max_iter) { status = LQCD_ENOCONV; break; }
+      if (it >= p.max_iter) {
+        // iteration cap: fold what the low-precision iteration has accumulated since the last
+        // reliable update into x, so that the caller gets the best iterate and its true residual
+        MultiArgs m; memset(&m, 0, sizeof(m));
+        m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
+        cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+        status = LQCD_ENOCONV;
+        break;
+      }
       { BlasArgs a = mk(c, false, pv, rl, v); if ((rc = blas<OpBicgP>(c, ps, a, s))) return rc; }
       if ((rc = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
       { BlasArgs a = mk(c, false, rt, v); if ((rc = blas<OpBicgAlpha>(c, ps, a, s))) return rc; }
