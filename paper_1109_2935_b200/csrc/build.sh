@@ -3,7 +3,8 @@
 set -e
 cd "$(dirname "$0")"
 OUT=../liblqcd_b200.so
-FLAGS="-gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -std=c++17 -Xcompiler -fPIC --expt-relaxed-constexpr"
+# LQ_EXTRA_FLAGS: e.g. -DLQ_BOUNDS_CHECK for the index-checked debug build (remove build/ first)
+FLAGS="-gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -std=c++17 -Xcompiler -fPIC --expt-relaxed-constexpr $LQ_EXTRA_FLAGS"
 mkdir -p build
 pids=""
 for f in dslash_fp64 dslash_fp32 dslash_half blas clover pack api solver host_api; do

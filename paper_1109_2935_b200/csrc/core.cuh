@@ -34,6 +34,15 @@ struct PrecH { typedef short  store_t; typedef float  real; static constexpr boo
 #define LQ_GAUGE_STREAM 1
 #endif
 
+// Debug build (LQ_EXTRA_FLAGS=-DLQ_BOUNDS_CHECK sh build.sh): every record index of every packed
+// field access is checked against the field's record count and the kernel traps on a violation
+// (compute-sanitizer is not available on the GPU pool this was developed on).
+#ifdef LQ_BOUNDS_CHECK
+#define LQ_CHECK_INDEX(i, ns) do { if ((unsigned long long)(i) >= (unsigned long long)(ns)) __trap(); } while (0)
+#else
+#define LQ_CHECK_INDEX(i, ns) do { } while (0)
+#endif
+
 template <typename V> LQ_DEV V ld_nc(const V* p) { return __ldg(p); }
 // streaming variants for data with no reuse (gauge links): do not allocate in L1
 LQ_DEV int4 ld_stream(const int4* p) {
@@ -94,6 +103,7 @@ struct Rec {
   // 2: shared memory staging buffer laid out like a packed field with ns = CTA size, i = thread
   template <int MODE = 0>
   LQ_DEV static void load(T* __restrict__ v, const char* __restrict__ base, long long ns, long long i) {
+    LQ_CHECK_INDEX(i, ns);
 #pragma unroll
     for (int k = 0; k < N16; ++k) {
       const int4* p = reinterpret_cast<const int4*>(base + 16ll * k * ns) + i;
@@ -113,6 +123,8 @@ struct Rec {
   }
   // record i of the global field -> record `tid` of a staging buffer of `nt` records
   LQ_DEV static void stage(char* __restrict__ sbase, int nt, int tid, const char* __restrict__ base, long long ns, long long i) {
+    LQ_CHECK_INDEX(i, ns);
+    LQ_CHECK_INDEX(tid, nt);
 #pragma unroll
     for (int k = 0; k < N16; ++k)
       cp_async<16>(sbase + 16 * k * nt + 16 * tid, reinterpret_cast<const int4*>(base + 16ll * k * ns) + i);
@@ -120,6 +132,7 @@ struct Rec {
     if (N4) cp_async<4>(sbase + (16 * N16 + 8 * N8) * nt + 4 * tid, reinterpret_cast<const int*>(base + (16ll * N16 + 8ll * N8) * ns) + i);
   }
   LQ_DEV static void store(const T* __restrict__ v, char* __restrict__ base, long long ns, long long i) {
+    LQ_CHECK_INDEX(i, ns);
 #pragma unroll
     for (int k = 0; k < N16; ++k)
       reinterpret_cast<int4*>(base + 16ll * k * ns)[i] = *reinterpret_cast<const int4*>(v + k * E16);
