@@ -115,30 +115,29 @@ LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restr
 // out = C in for one site: two Hermitian 6x6 blocks, 36 reals each: 6 diagonal then the 15
 // lower-triangle entries (i>j) at 6 + 2*(i(i-1)/2 + j).  504 flop (PAPER.md:138 fn.1: 72 reals).
 template <typename R>
+LQ_DEV void clover_block(R* __restrict__ o, const R* __restrict__ x, const R* __restrict__ c) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    R re = c[i] * x[2 * i], im = c[i] * x[2 * i + 1];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      if (j < i) {
+        const R lr = c[6 + 2 * (i * (i - 1) / 2 + j)], li = c[6 + 2 * (i * (i - 1) / 2 + j) + 1];
+        re = fma_(lr, x[2 * j], re);     re = fma_(-li, x[2 * j + 1], re);
+        im = fma_(lr, x[2 * j + 1], im); im = fma_(li, x[2 * j], im);
+      } else if (j > i) {
+        const R lr = c[6 + 2 * (j * (j - 1) / 2 + i)], li = c[6 + 2 * (j * (j - 1) / 2 + i) + 1];
+        re = fma_(lr, x[2 * j], re);     re = fma_(li, x[2 * j + 1], re);
+        im = fma_(lr, x[2 * j + 1], im); im = fma_(-li, x[2 * j], im);
+      }
+    }
+    o[2 * i] = re; o[2 * i + 1] = im;
+  }
+}
+template <typename R>
 LQ_DEV void clover_mul(R* __restrict__ out, const R* __restrict__ in, const R* __restrict__ cl) {
 #pragma unroll
-  for (int ch = 0; ch < 2; ++ch) {
-    const R* c = cl + 36 * ch;
-    const R* x = in + 12 * ch;
-    R* o = out + 12 * ch;
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-      R re = c[i] * x[2 * i], im = c[i] * x[2 * i + 1];
-#pragma unroll
-      for (int j = 0; j < 6; ++j) {
-        if (j < i) {
-          const R lr = c[6 + 2 * (i * (i - 1) / 2 + j)], li = c[6 + 2 * (i * (i - 1) / 2 + j) + 1];
-          re = fma_(lr, x[2 * j], re);     re = fma_(-li, x[2 * j + 1], re);
-          im = fma_(lr, x[2 * j + 1], im); im = fma_(li, x[2 * j], im);
-        } else if (j > i) {
-          const R lr = c[6 + 2 * (j * (j - 1) / 2 + i)], li = c[6 + 2 * (j * (j - 1) / 2 + i) + 1];
-          re = fma_(lr, x[2 * j], re);     re = fma_(li, x[2 * j + 1], re);
-          im = fma_(lr, x[2 * j + 1], im); im = fma_(-li, x[2 * j], im);
-        }
-      }
-      o[2 * i] = re; o[2 * i + 1] = im;
-    }
-  }
+  for (int ch = 0; ch < 2; ++ch) clover_block<R>(out + 12 * ch, in + 12 * ch, cl + 36 * ch);
 }
 
 // out = C in with C read from a packed clover field; in half precision the per-site norm is
@@ -184,10 +183,14 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
 #ifndef LQ_DSLASH_BLOCK
 #define LQ_DSLASH_BLOCK 128
 #endif
-// minimum resident CTAs per SM: caps registers at 80 for the fp32-arithmetic kernels (6 CTAs =
-// 24 warps/SM; measured best, profiles/r1_occupancy_sweep.md); fp64 needs the registers.
+// minimum resident CTAs per SM for the fp32-arithmetic kernels: 5 (96 registers, 20 warps/SM).
+// Measured at 32^3x64 in bursts at full clock, 6 / 5 / 4 CTAs: Mhat fp32 r12 302.7 / 296.2 / 300.1 us,
+// Mhat half r12 234.4 / 228.3 / 233.0 us, Dslash fp32 r12 97.7 / 97.5 / 100.2 us.  At 6 (80 registers)
+// the clover-epilogue variants spill 60-230 bytes per thread, and with the L1 carved out for the
+// staging ring those spills miss L1 (ncu: 3 % hit rate) and travel to L2: the MR-step kernel lost
+// 30 us of 150 to them.  fp64 takes the registers it needs (1 CTA minimum).
 #ifndef LQ_DSLASH_MINB
-#define LQ_DSLASH_MINB 6
+#define LQ_DSLASH_MINB 5
 #endif
 
 // bytes of one staging buffer (one hop of every thread of the CTA): link + neighbour spinor (+ norm)
@@ -210,7 +213,7 @@ dslash_kernel(const DslashArgs a) {
   const int cb = (DOTS ? 0 : a.range.cb0) + blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
   const int box = blockIdx.y;
   const bool active = cb < (DOTS ? g.vh : a.range.cb1);
-  double red[3] = {0, 0, 0};
+  R d0 = 0, d1 = 0, d2 = 0;                 // DOTS: this site's <r,y> (re, im) and <r,r>
   if (active) {
     const long long base = (long long)box * g.vh;
     const long long idx = base + cb;
@@ -311,15 +314,35 @@ dslash_kernel(const DslashArgs a) {
 #undef LQ_ISSUE
     }
 
-    R yv[24];
     if constexpr (XPAY) {
+      R yv[24];
       load_site<P, 24>(yv, a.y, g.ns, idx);
       const R coef = (R)a.a;
       if constexpr (CLOVX) {
-        R ay[24];
-        clover_site<P>(ay, yv, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
+        // r = A y + coef * acc, one chiral block at a time so that y, A y and the clover block
+        // die early (the DOTS variant needs y for the partial sums as well)
+        R cl[72], sc;
+        load_site_raw<P, 72>(cl, sc, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
 #pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], ay[k]);
+        for (int ch = 0; ch < 2; ++ch) {
+          R ay[12];
+          clover_block<R>(ay, yv + 12 * ch, cl + 36 * ch);
+#pragma unroll
+          for (int k = 0; k < 12; ++k) {
+            if constexpr (P::HALF) ay[k] *= sc;
+            acc[12 * ch + k] = fma_(coef, acc[12 * ch + k], ay[k]);
+          }
+          if constexpr (DOTS) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+              const R rr = acc[12 * ch + 2 * k], ri = acc[12 * ch + 2 * k + 1];
+              const R yr = yv[12 * ch + 2 * k], yi = yv[12 * ch + 2 * k + 1];
+              d0 = fma_(rr, yr, d0); d0 = fma_(ri, yi, d0);
+              d1 = fma_(rr, yi, d1); d1 = fma_(-ri, yr, d1);
+              d2 = fma_(rr, rr, d2); d2 = fma_(ri, ri, d2);
+            }
+          }
+        }
       } else {
 #pragma unroll
         for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], yv[k]);
@@ -332,20 +355,9 @@ dslash_kernel(const DslashArgs a) {
       for (int k = 0; k < 24; ++k) acc[k] = t[k];
     }
     store_site<P, 24>(acc, a.out, g.ns, idx);
-    if constexpr (DOTS) {
-      // <r,y> = sum conj(r) y, <r,r>: the 12 terms of one site are summed in the arithmetic
-      // precision (FMA chains), the sums over sites in fp64
-      R d0 = 0, d1 = 0, d2 = 0;
-#pragma unroll
-      for (int k = 0; k < 12; ++k) {
-        d0 = fma_(acc[2 * k], yv[2 * k], d0);      d0 = fma_(acc[2 * k + 1], yv[2 * k + 1], d0);
-        d1 = fma_(acc[2 * k], yv[2 * k + 1], d1);  d1 = fma_(-acc[2 * k + 1], yv[2 * k], d1);
-        d2 = fma_(acc[2 * k], acc[2 * k], d2);     d2 = fma_(acc[2 * k + 1], acc[2 * k + 1], d2);
-      }
-      red[0] = (double)d0; red[1] = (double)d1; red[2] = (double)d2;
-    }
   }
   if constexpr (DOTS) {
+    double red[3] = {(double)d0, (double)d1, (double)d2};   // sums over sites in fp64
     __shared__ double sm[3 * (LQ_DSLASH_BLOCK / 32)];
     cta_reduce<3, LQ_DSLASH_BLOCK>(red, sm);
     if (threadIdx.x == 0) {

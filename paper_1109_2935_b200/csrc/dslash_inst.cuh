@@ -9,7 +9,7 @@ namespace lq {
 #define LQ_PIPE_FP32 2
 #endif
 #ifndef LQ_PIPE_HALF
-#define LQ_PIPE_HALF 3
+#define LQ_PIPE_HALF 4
 #endif
 
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>

@@ -12,7 +12,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liblqcd_b200.so")
+# LQCD_B200_LIB selects another build of the same library (e.g. the index-checked debug build)
+LIB_PATH = os.environ.get("LQCD_B200_LIB") or os.path.join(_HERE, "liblqcd_b200.so")
 
 PREC_DOUBLE, PREC_SINGLE, PREC_HALF = 0, 1, 2
 RECON_18, RECON_12, RECON_8 = 18, 12, 8
