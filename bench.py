@@ -212,6 +212,7 @@ def main():
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
     ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"], help="storage precision of the timed Dslash")
     ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8], help="link compression of the timed Dslash")
+    ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per launch (>1: lqcd_dslash_mrhs; the BASELINE metric is 1)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -247,12 +248,24 @@ def main():
     pname = {"fp64": "fp64 storage+arithmetic", "fp32": "fp32 storage+arithmetic",
              "half": "16-bit fixed point + per-site fp32 norm storage, fp32 arithmetic"}[args.prec]
     dtype = {"fp64": "f64", "fp32": "f32", "half": "i16+f32"}[args.prec]
-    f = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
-    g = [ctx.new_field(prec) for _ in (0, 1)]
+    nrhs = args.nrhs
+    if nrhs == 1:
+        f = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
+        g = [ctx.new_field(prec) for _ in (0, 1)]
 
-    def step():
-        ctx.dslash(g[0], f[1], 0, False, prec, recon)
-        ctx.dslash(g[1], f[0], 1, False, prec, recon)
+        def step():
+            ctx.dslash(g[0], f[1], 0, False, prec, recon)
+            ctx.dslash(g[1], f[0], 1, False, prec, recon)
+    else:
+        f = [ctx.new_fields(prec, nrhs) for _ in (0, 1)]
+        g = [ctx.new_fields(prec, nrhs) for _ in (0, 1)]
+        for p in (0, 1):
+            for r in range(nrhs):                      # distinct sources: psi scaled and cyclically shifted in t
+                ctx.pack_spinor((psi.roll(r, 0) * (1.0 + 0.25 * r)).contiguous(), p, prec, out=f[p][r])
+
+        def step():
+            ctx.dslash_mrhs(g[0], f[1], nrhs, 0, False, prec, recon)
+            ctx.dslash_mrhs(g[1], f[0], nrhs, 1, False, prec, recon)
 
     for _ in range(args.warmup):
         step()
@@ -281,9 +294,9 @@ def main():
     cbytes = V * 12 * 16
 
     ms_step = ms / args.steps
-    value = whole_job_gflops(FLOP_DSLASH * V, world, ms_step)
+    value = whole_job_gflops(FLOP_DSLASH * V * nrhs, world, ms_step)
     kern_ms = ms / launches
-    algo_bytes = dslash_bytes(prec, recon) * Vh
+    algo_bytes = (2 * SPINOR_B[prec] * nrhs + 8 * recon * LINK_B[prec]) * Vh     # links once per launch
     achieved = algo_bytes / (kern_ms * 1e-3) / 1e9
 
     out = {
@@ -291,12 +304,12 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": {"workload": "config 3: 32^3x64, eps=0.3, full-lattice Wilson-clover Dslash (both parities)",
-                   "precision": pname, "recon": recon, "flop_per_site": FLOP_DSLASH,
+                   "precision": pname, "recon": recon, "flop_per_site": FLOP_DSLASH, "nrhs": nrhs,
                    "l2": "inputs larger than L2 (gauge 403 MB + spinors 201 MB per step vs 126 MB L2)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                     "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC.get((args.prec, recon)), "peak_kind": pk_kind,
-                     "kernel": "dslash_kernel<%s,%d> (EPI_NONE)" % (args.prec, recon), "algorithmic_bytes_per_launch": algo_bytes,
+                     "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC.get((args.prec, recon)) if nrhs == 1 else None, "peak_kind": pk_kind,
+                     "kernel": ("dslash_kernel<%s,%d> (EPI_NONE)" if nrhs == 1 else "dslash_mrhs_kernel<%s,%d> (EPI_NONE)") % (args.prec, recon), "algorithmic_bytes_per_launch": algo_bytes,
                      "frac_of_8TBs_nominal": achieved / 8000.0,
                      "traffic_source": "profiles/r1_dslash_%s_r%d.md" % (args.prec, recon) if (args.prec, recon) in NCU_TRAFFIC else None},
         "e2e": {"value": whole_job_gflops(FLOP_DSLASH * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
@@ -305,7 +318,7 @@ def main():
         "clocks": clocks,
     }
 
-    if (args.prec, recon) in NCU_WARP_INST:
+    if (args.prec, recon) in NCU_WARP_INST and nrhs == 1:
         # issue-bound kernel: executed warp instructions per launch (ncu) / time vs 1 per scheduler per clock
         ips = NCU_WARP_INST[(args.prec, recon)] / (kern_ms * 1e-3) / 1e9
         ipeak = N_SCHEDULERS * pk["sm_max_mhz"] * 1e-3
@@ -326,8 +339,8 @@ def main():
         # parity of the timed configuration against the oracle on the full lattice (same inputs)
         import numpy as np
         got = torch.zeros_like(psi)
-        ctx.unpack_spinor(got, g[0], 0, prec)
-        ctx.unpack_spinor(got, g[1], 1, prec)
+        ctx.unpack_spinor(got, g[0] if nrhs == 1 else g[0][0], 0, prec)     # right-hand side 0 is psi itself
+        ctx.unpack_spinor(got, g[1] if nrhs == 1 else g[1][0], 1, prec)
         want = torch.from_numpy(o_out).to(dev)      # rank 0's inputs are seeds (1, 2), the oracle's too
         if want is not None:
             out["parity_rel_l2_vs_oracle"] = float(torch.linalg.vector_norm(got - want) / torch.linalg.vector_norm(want))
@@ -382,6 +395,27 @@ def extras(ctx, psi, args, torch, lqcd, inputs, pk):
         ex["blas"].append({"prec": names[prec], "axpy_norm_us": t0 * 1e3, "axpy_norm_gbs": 3 * SPINOR_B[prec] * Vh / (t0 * 1e-3) / 1e9,
                            "cdot_us": t1 * 1e3, "cdot_gbs": 2 * SPINOR_B[prec] * Vh / (t1 * 1e-3) / 1e9,
                            "note": "includes one host read-back of the result per call"})
+        del fin, fo
+    # multi-right-hand-side operators: 12 sources per launch, per-source time
+    ex["mrhs"] = []
+    for prec in (() if args.solvers_only else (0, 1, 2)):
+        nrhs = 12
+        fin, fo = ctx.new_fields(prec, nrhs), ctx.new_fields(prec, nrhs)
+        for r in range(nrhs):
+            ctx.pack_spinor(psi, 1, prec, out=fin[r])
+        for name, fn, flop, by in (
+                ("dslash_mrhs", lambda: ctx.dslash_mrhs(fo, fin, nrhs, 0, False, prec, 12), FLOP_DSLASH,
+                 2 * SPINOR_B[prec] + 8 * 12 * LINK_B[prec] / 4.0),
+                ("matpc_mrhs", lambda: ctx.matpc_mrhs(fo, fin, nrhs, 1, False, KAPPA, prec, 12), FLOP_MATPC,
+                 5 * SPINOR_B[prec] + 16 * 12 * LINK_B[prec] / 4.0 + 2 * CLOVER_B[prec])):
+            for _ in range(2):
+                fn()
+            bursts = sorted(time_region_clk(fn, 5, psi.device.index or 0) for _ in range(5))
+            us = bursts[2][0] / 5.0 / nrhs * 1e3
+            ex["mrhs"].append({"op": name, "prec": names[prec], "recon": 12, "nrhs": nrhs, "us_per_rhs": us,
+                               "best_us_per_rhs": bursts[0][0] / 5.0 / nrhs * 1e3, "gflops": flop * Vh / (us * 1e-6) / 1e9,
+                               "bytes_per_site_per_rhs": by, "gbs": by * Vh / (us * 1e-6) / 1e9, "sm_mhz_during": bursts[2][1],
+                               "note": "links are read once per 4 right-hand sides (one CTA); clover once per right-hand side"})
         del fin, fo
     # config 4: eps = 0.2, mixed-precision BiCGstab, fp64 outer, to 1e-10
     dev = psi.device

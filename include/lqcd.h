@@ -109,6 +109,19 @@ int lqcd_clover(lqcd_ctx* ctx, void* out, const void* in, int parity, int invers
 int lqcd_matpc(lqcd_ctx* ctx, void* out, const void* in, int parity, int dagger,
                double kappa, int prec, int recon, void* stream);
 
+/* Multi-right-hand-side forms (not in the paper): the same operators applied
+ * to nrhs (1..LQCD_MAX_RHS) packed fields that share the gauge field, in one launch per Dslash.
+ * `in` and `out` hold the nrhs packed fields of precision `prec` back to back (field r starts at
+ * r * lqcd_field_bytes).  A link is loaded, decoded and reconstructed once per CTA for 4
+ * right-hand sides: 2/3 of the compulsory bytes of a single-source fp32/recon-12 Dslash are links.
+ * Same results as nrhs single calls (same arithmetic per site).  Errors as lqcd_dslash, plus
+ * LQCD_EINVAL for nrhs out of range. */
+#define LQCD_MAX_RHS 64
+int lqcd_dslash_mrhs(lqcd_ctx* ctx, void* out, const void* in, int nrhs, int parity_out, int dagger,
+                     int prec, int recon, void* stream);
+int lqcd_matpc_mrhs(lqcd_ctx* ctx, void* out, const void* in, int nrhs, int parity, int dagger,
+                    double kappa, int prec, int recon, void* stream);
+
 /* Schwarz preconditioner K (R7): out = K in on `parity`, n_mr
  * minimum-residual steps on the Dirichlet-cut Mhat_D with one alpha per block.  in/out are
  * packed fields (natural layout) of precision `prec_io`; the MR iteration itself runs in

@@ -160,6 +160,51 @@ int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, dou
                    -kappa * kappa, kappa, blocked, s);
 }
 
+// multi-right-hand-side Dslash: the same fused launch for nrhs fields sharing the links
+int op_dslash_mrhs(lqcd_ctx* c, char* out, const char* in, const char* y, int nrhs, int parity_out, int dagger, int prec,
+                   int recon, int epi, double a, double kappa, cudaStream_t s) {
+  if (nrhs < 1 || nrhs > LQCD_MAX_RHS) return fail(c, LQCD_EINVAL, "nrhs");
+  DslashArgs d;
+  memset(&d, 0, sizeof(d));
+  d.g = c->nat;
+  d.out = out; d.in = in; d.y = y; d.a = a; d.parity = parity_out;
+  d.dagger = (dagger ? 1 : 0) | (nrhs << 8);
+  d.range.cb0 = 0; d.range.cb1 = d.g.vh;
+  int rc = get_gauge(c, prec, recon, false, &d.gauge, s);
+  if (rc) return rc;
+  if (epi != EPI_NONE && epi != EPI_XPAY) {
+    const char *A, *Ai;
+    rc = get_clover(c, prec, kappa, false, &A, &Ai, s);
+    if (rc) return rc;
+    d.clov_y = A; d.clov_out = Ai;
+  }
+  cudaError_t e;
+  switch (prec) {
+    case 0: e = launch_dslash_mrhs<PrecD>(d, nrhs, recon, epi, s); break;
+    case 1: e = launch_dslash_mrhs<PrecS>(d, nrhs, recon, epi, s); break;
+    case 2: e = launch_dslash_mrhs<PrecH>(d, nrhs, recon, epi, s); break;
+    default: return fail(c, LQCD_EINVAL, "bad precision");
+  }
+  c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dslash_mrhs launch", e);
+  return LQCD_OK;
+}
+
+int op_matpc_mrhs(lqcd_ctx* c, char* out, const char* in, int nrhs, int parity, int dagger, double kappa, int prec, int recon,
+                  cudaStream_t s) {
+  const size_t need = spinor_bytes(prec, c->nat.ns) * (size_t)nrhs;
+  if (c->mtmp_bytes < need) {
+    if (c->mtmp) cudaFree(c->mtmp);                   // synchronises: no launch still uses the old buffer
+    c->mtmp = nullptr; c->mtmp_bytes = 0;
+    int rc = dev_alloc(c, (void**)&c->mtmp, need);
+    if (rc) return rc;
+    c->mtmp_bytes = need;
+  }
+  int rc = op_dslash_mrhs(c, c->mtmp, in, nullptr, nrhs, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, s);
+  if (rc) return rc;
+  return op_dslash_mrhs(c, out, c->mtmp, in, nrhs, parity, dagger, prec, recon, EPI_CLOVX_XPAY, -kappa * kappa, kappa, s);
+}
+
 }  // namespace lq
 
 // ================================================================================================
@@ -195,6 +240,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   c->boxdots_doubles = 0;
   memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
   c->have_hpipe = false;
+  c->mtmp = nullptr; c->mtmp_bytes = 0;
   cudaDeviceProp prop;
   cudaGetDeviceProperties(&prop, device);
   c->n_sm = prop.multiProcessorCount;
@@ -225,6 +271,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->hS) cudaFreeHost(c->hS);
   for (void* p : c->pool) cudaFree(p);
   for (void* p : c->hws) if (p) cudaFree(p);
+  if (c->mtmp) cudaFree(c->mtmp);
   if (c->have_hpipe) {
     cudaStreamDestroy(c->hs_in); cudaStreamDestroy(c->hs_out); cudaEventDestroy(c->hev_sync);
     for (int i = 0; i < LQ_HOST_SLABS; ++i) { cudaEventDestroy(c->hev_in[i]); cudaEventDestroy(c->hev_out[i]); }
@@ -309,6 +356,23 @@ int lqcd_clover(lqcd_ctx* c, void* out, const void* in, int parity, int inverse,
   cudaError_t e = run_clover_apply(prec, (char*)out, (const char*)in, inverse ? Ai : A, c->nat, parity, s);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "clover_apply", e);
+}
+
+int lqcd_dslash_mrhs(lqcd_ctx* c, void* out, const void* in, int nrhs, int parity_out, int dagger, int prec, int recon, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity_out | 1) != 1) return fail(c, LQCD_EINVAL, "dslash_mrhs arguments");
+  cudaSetDevice(c->device);
+  return op_dslash_mrhs(c, (char*)out, (const char*)in, nullptr, nrhs, parity_out, dagger, prec, recon, EPI_NONE, 0.0, 0.0,
+                        (cudaStream_t)stream);
+}
+
+int lqcd_matpc_mrhs(lqcd_ctx* c, void* out, const void* in, int nrhs, int parity, int dagger, double kappa, int prec, int recon,
+                    void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity | 1) != 1 || nrhs < 1 || nrhs > LQCD_MAX_RHS || prec < 0 || prec > 2)
+    return fail(c, LQCD_EINVAL, "matpc_mrhs arguments");
+  cudaSetDevice(c->device);
+  return op_matpc_mrhs(c, (char*)out, (const char*)in, nrhs, parity, dagger, kappa, prec, recon, (cudaStream_t)stream);
 }
 
 int lqcd_matpc(lqcd_ctx* c, void* out, const void* in, int parity, int dagger, double kappa, int prec, int recon, void* stream) {

@@ -180,6 +180,56 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
   }
 }
 
+// Fused epilogue of one site (shared by the single- and multi-right-hand-side kernels):
+//   XPAY: acc = [A] y + coef * acc (CLOVX: A = clover block of the site);  CLOVOUT: acc = C acc;
+//   DOTS: d0 + i d1 += <acc, y>, d2 += <acc, acc> for this site (before CLOVOUT; only used with CLOVX).
+template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __restrict__ y, const char* __restrict__ clov_y,
+                            const char* __restrict__ clov_out, double coef_d, int p, long long ns, long long idx,
+                            typename P::real& d0, typename P::real& d1, typename P::real& d2) {
+  typedef typename P::real R;
+  if constexpr (XPAY) {
+    R yv[24];
+    load_site<P, 24>(yv, y, ns, idx);
+    const R coef = (R)coef_d;
+    if constexpr (CLOVX) {
+      // r = A y + coef * acc, one chiral block at a time so that y, A y and the clover block
+      // die early (the DOTS variant needs y for the partial sums as well)
+      R cl[72], sc;
+      load_site_raw<P, 72>(cl, sc, clov_y + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+#pragma unroll
+      for (int ch = 0; ch < 2; ++ch) {
+        R ay[12];
+        clover_block<R>(ay, yv + 12 * ch, cl + 36 * ch);
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+          if constexpr (P::HALF) ay[k] *= sc;
+          acc[12 * ch + k] = fma_(coef, acc[12 * ch + k], ay[k]);
+        }
+        if constexpr (DOTS) {
+#pragma unroll
+          for (int k = 0; k < 6; ++k) {
+            const R rr = acc[12 * ch + 2 * k], ri = acc[12 * ch + 2 * k + 1];
+            const R yr = yv[12 * ch + 2 * k], yi = yv[12 * ch + 2 * k + 1];
+            d0 = fma_(rr, yr, d0); d0 = fma_(ri, yi, d0);
+            d1 = fma_(rr, yi, d1); d1 = fma_(-ri, yr, d1);
+            d2 = fma_(rr, rr, d2); d2 = fma_(ri, ri, d2);
+          }
+        }
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], yv[k]);
+    }
+  }
+  if constexpr (CLOVOUT) {
+    R t[24];
+    clover_site<P>(t, acc, clov_out + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+#pragma unroll
+    for (int k = 0; k < 24; ++k) acc[k] = t[k];
+  }
+}
+
 #ifndef LQ_DSLASH_BLOCK
 #define LQ_DSLASH_BLOCK 128
 #endif
@@ -314,46 +364,7 @@ dslash_kernel(const DslashArgs a) {
 #undef LQ_ISSUE
     }
 
-    if constexpr (XPAY) {
-      R yv[24];
-      load_site<P, 24>(yv, a.y, g.ns, idx);
-      const R coef = (R)a.a;
-      if constexpr (CLOVX) {
-        // r = A y + coef * acc, one chiral block at a time so that y, A y and the clover block
-        // die early (the DOTS variant needs y for the partial sums as well)
-        R cl[72], sc;
-        load_site_raw<P, 72>(cl, sc, a.clov_y + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
-#pragma unroll
-        for (int ch = 0; ch < 2; ++ch) {
-          R ay[12];
-          clover_block<R>(ay, yv + 12 * ch, cl + 36 * ch);
-#pragma unroll
-          for (int k = 0; k < 12; ++k) {
-            if constexpr (P::HALF) ay[k] *= sc;
-            acc[12 * ch + k] = fma_(coef, acc[12 * ch + k], ay[k]);
-          }
-          if constexpr (DOTS) {
-#pragma unroll
-            for (int k = 0; k < 6; ++k) {
-              const R rr = acc[12 * ch + 2 * k], ri = acc[12 * ch + 2 * k + 1];
-              const R yr = yv[12 * ch + 2 * k], yi = yv[12 * ch + 2 * k + 1];
-              d0 = fma_(rr, yr, d0); d0 = fma_(ri, yi, d0);
-              d1 = fma_(rr, yi, d1); d1 = fma_(-ri, yr, d1);
-              d2 = fma_(rr, rr, d2); d2 = fma_(ri, ri, d2);
-            }
-          }
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, acc[k], yv[k]);
-      }
-    }
-    if constexpr (CLOVOUT) {
-      R t[24];
-      clover_site<P>(t, acc, a.clov_out + (long long)p * site_bytes<P>(72, true) * g.ns, g.ns, idx);
-#pragma unroll
-      for (int k = 0; k < 24; ++k) acc[k] = t[k];
-    }
+    dslash_epilogue<P, XPAY, CLOVX, CLOVOUT, DOTS>(acc, a.y, a.clov_y, a.clov_out, a.a, p, g.ns, idx, d0, d1, d2);
     store_site<P, 24>(acc, a.out, g.ns, idx);
   }
   if constexpr (DOTS) {

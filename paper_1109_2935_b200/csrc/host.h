@@ -102,4 +102,6 @@ struct lqcd_ctx {
   cudaStream_t hs_in, hs_out;
   cudaEvent_t hev_in[LQ_HOST_SLABS], hev_out[LQ_HOST_SLABS], hev_sync;
   bool have_hpipe;
+  char* mtmp;             // multi-right-hand-side Mhat temporary (grow-only)
+  size_t mtmp_bytes;
 };

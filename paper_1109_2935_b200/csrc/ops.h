@@ -15,6 +15,13 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
              bool blocked, bool dots, cudaStream_t s);
 
+// multi-right-hand-side forms (dslash_mrhs.cuh): in / out / y hold nrhs packed fields back to back
+int op_dslash_mrhs(lqcd_ctx* c, char* out, const char* in, const char* y, int nrhs, int parity_out, int dagger, int prec,
+                   int recon, int epi, double a, double kappa, cudaStream_t s);
+int op_matpc_mrhs(lqcd_ctx* c, char* out, const char* in, int nrhs, int parity, int dagger, double kappa, int prec, int recon,
+                  cudaStream_t s);
+
 template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);
+template <class P> cudaError_t launch_dslash_mrhs(const DslashArgs& a, int nrhs, int recon, int epi, cudaStream_t s);
 
 }  // namespace lq

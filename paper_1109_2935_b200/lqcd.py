@@ -24,7 +24,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_schwarz", "lqcd_invert", "lqcd_apply_host", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
 ]
 
@@ -82,6 +82,8 @@ def load_library():
             "lqcd_dslash": (i, [vp, vp, vp, i, i, i, i, vp]),
             "lqcd_clover": (i, [vp, vp, vp, i, i, d, i, vp]),
             "lqcd_matpc": (i, [vp, vp, vp, i, i, d, i, i, vp]),
+            "lqcd_dslash_mrhs": (i, [vp, vp, vp, i, i, i, i, i, vp]),
+            "lqcd_matpc_mrhs": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_schwarz": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, vp]),
             "lqcd_invert": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_apply_host": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
@@ -174,6 +176,18 @@ class Context:
 
     def matpc(self, out, inp, parity, dagger, kappa, prec, recon):
         self._check(self.lib.lqcd_matpc(self.h, _ptr(out), _ptr(inp), parity, int(dagger), kappa, prec, recon, _stream()))
+        return out
+
+    def new_fields(self, prec, nrhs):
+        """nrhs packed fields back to back (the layout of the *_mrhs calls); row r is field r."""
+        return torch.empty((nrhs, self.field_bytes(prec)), dtype=torch.uint8, device=self.device)
+
+    def dslash_mrhs(self, out, inp, nrhs, parity_out, dagger, prec, recon):
+        self._check(self.lib.lqcd_dslash_mrhs(self.h, _ptr(out), _ptr(inp), nrhs, parity_out, int(dagger), prec, recon, _stream()))
+        return out
+
+    def matpc_mrhs(self, out, inp, nrhs, parity, dagger, kappa, prec, recon):
+        self._check(self.lib.lqcd_matpc_mrhs(self.h, _ptr(out), _ptr(inp), nrhs, parity, int(dagger), kappa, prec, recon, _stream()))
         return out
 
     def schwarz(self, out, inp, parity, kappa, block, n_mr, omega_mr, prec, recon, prec_io):

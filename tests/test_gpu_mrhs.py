@@ -1,0 +1,71 @@
+"""Multi-right-hand-side Dslash / Mhat (-m gpu): every right-hand side of lqcd_dslash_mrhs and
+lqcd_matpc_mrhs against the oracle applied to that source alone, and against the single-source
+calls (same arithmetic per site: bit-identical), on a ragged lattice (Vh = 960 = 30 CTAs of 32
+sites) and for right-hand-side counts that are not multiples of the 4 a CTA handles."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1109_2935_b200 import inputs
+from test_gpu_parity import Case, _rel, TOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ragged():
+    return Case((6, 4, 10, 8), 0.3, bc=(-1, 1, 1, -1))
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+@pytest.mark.parametrize("nrhs", [1, 3, 4, 6])
+def test_mrhs_matches_oracle_and_single(ragged, prec, nrhs):
+    c = ragged
+    ctx, kappa = c.ctx, 0.124
+    srcs = [inputs.gaussian_spinor(c.dims, 100 + r) * (1.0 + r) for r in range(nrhs)]    # different norms per source
+    dev = [torch.from_numpy(s).cuda() for s in srcs]
+    for recon in (18, 12, 8):
+        tol = TOL[prec] if not (prec == 0 and recon == 8) else 1e-11
+        for parity in (0, 1):
+            for dagger in (False, True):
+                fin = ctx.new_fields(prec, nrhs)
+                fout = ctx.new_fields(prec, nrhs)
+                for r in range(nrhs):
+                    ctx.pack_spinor(dev[r], 1 - parity, prec, out=fin[r])
+                ctx.dslash_mrhs(fout, fin, nrhs, parity, dagger, prec, recon)
+                for r in range(nrhs):
+                    got = torch.zeros_like(dev[r])
+                    ctx.unpack_spinor(got, fout[r], parity, prec)
+                    want = oracle.dslash(srcs[r] * c.mask(1 - parity), c.U, c.bc, dagger=dagger) * c.mask(parity)
+                    assert _rel(got.cpu().numpy(), want) <= tol, ("dslash", recon, parity, dagger, r)
+                    single = ctx.new_field(prec)
+                    ctx.dslash(single, fin[r], parity, dagger, prec, recon)
+                    assert torch.equal(single, fout[r]), ("dslash vs single", recon, parity, dagger, r)
+            fin = ctx.new_fields(prec, nrhs)
+            fout = ctx.new_fields(prec, nrhs)
+            for r in range(nrhs):
+                ctx.pack_spinor(dev[r], parity, prec, out=fin[r])
+            ctx.matpc_mrhs(fout, fin, nrhs, parity, False, kappa, prec, recon)
+            for r in range(nrhs):
+                got = torch.zeros_like(dev[r])
+                ctx.unpack_spinor(got, fout[r], parity, prec)
+                want = oracle.matpc(srcs[r], c.U, c.T, c.bc, kappa, parity)
+                assert _rel(got.cpu().numpy(), want) <= tol, ("matpc", recon, parity, r)
+                single = ctx.new_field(prec)
+                ctx.matpc(single, fin[r], parity, False, kappa, prec, recon)
+                assert torch.equal(single, fout[r]), ("matpc vs single", recon, parity, r)
+
+
+def test_mrhs_argument_errors(ragged):
+    c = ragged
+    lq = c.lqcd
+    f = c.ctx.new_fields(1, 2)
+    g = c.ctx.new_fields(1, 2)
+    for bad in (0, -1, 65):
+        with pytest.raises(lq.LqcdError) as e:
+            c.ctx.dslash_mrhs(f, g, bad, 0, False, 1, 12)
+        assert e.value.code == lq.EINVAL
+    with pytest.raises(lq.LqcdError) as e:
+        c.ctx.matpc_mrhs(f, f, 2, 0, False, 0.12, 1, 12)            # aliasing
+    assert e.value.code == lq.EINVAL
