@@ -239,6 +239,9 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
 // the clover-epilogue variants spill 60-230 bytes per thread, and with the L1 carved out for the
 // staging ring those spills miss L1 (ncu: 3 % hit rate) and travel to L2: the MR-step kernel lost
 // 30 us of 150 to them.  fp64 takes the registers it needs (1 CTA minimum).
+#ifndef LQ_DSLASH_MINB64
+#define LQ_DSLASH_MINB64 2
+#endif
 #ifndef LQ_DSLASH_MINB
 #define LQ_DSLASH_MINB 5
 #endif
@@ -256,7 +259,7 @@ template <class P, int RECON> struct HopStage {
 // flight without holding registers.  The slots are private to a thread, so no CTA barrier is
 // needed: cp.async.wait_group orders a thread's own copies.
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST>
-__global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? 1 : LQ_DSLASH_MINB))
+__global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? LQ_DSLASH_MINB64 : LQ_DSLASH_MINB))
 dslash_kernel(const DslashArgs a) {
   typedef typename P::real R;
   const Geom& g = a.g;

@@ -5,6 +5,11 @@
 
 namespace lq {
 
+// fp64: the ring pays for the plain hopping term (32^3x64 r18 272 -> 246 us, r12 222 -> 212, r8 323 -> 282) but
+// not with a clover epilogue (Mhat r18 696 -> 730 us), which keeps loading straight into registers
+#ifndef LQ_PIPE_FP64
+#define LQ_PIPE_FP64 2
+#endif
 #ifndef LQ_PIPE_FP32
 #define LQ_PIPE_FP32 2
 #endif
@@ -14,16 +19,20 @@ namespace lq {
 
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
 static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
-  constexpr int NST = sizeof(typename P::real) == 8 ? 0 : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
+  constexpr int NST = sizeof(typename P::real) == 8 ? ((CLOVX || CLOVOUT) ? 0 : LQ_PIPE_FP64) : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
   constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
   auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST>;
-  if (NST > 0) {
-    static bool configured = false;       // per instantiation
-    if (!configured) {
+  static bool configured = false;         // per instantiation
+  if (!configured) {
+    if (NST > 0) {
       cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
       cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-      configured = true;
+    } else {
+      // no staging ring: ask for the largest L1.  Without a preference the SM keeps the carve-out of
+      // the previous kernel, and after a ring kernel the fp64 clover variants lost 5 % (696 -> 730 us)
+      cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
     }
+    configured = true;
   }
   kern<<<grid, block, SMEM, s>>>(a);
 }
