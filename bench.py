@@ -194,7 +194,9 @@ def run_reference(args, rank):
         "impl": "reference", "metric": "wilson_clover_dslash_gflops", "value": val, "unit": "GFLOP/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config 3: 32^3x64 eps=0.3, full-lattice Dslash", "precision": "fp64", "recon": 18},
+        "config": {"workload": "config 3: 32^3x64, eps=0.3, full-lattice Wilson-clover Dslash (both parities)",
+                   "precision": "fp64 (the oracle as it stands: no compression, no checkerboard storage)", "recon": 18,
+                   "flop_per_site": FLOP_DSLASH, "parallelism": "host cores, OpenMP"},
         "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
