@@ -432,15 +432,15 @@ def extras(ctx, psi, args, torch, lqcd, inputs, pk):
     for sloppy, recon in ((1, 12), (2, 12)):
         p = ctx.make_params(KAPPA, CSW, 1e-10, solver=lqcd.SOLVER_BICGSTAB, prec=(0, sloppy, sloppy), recon=(18, recon, recon))
         ctx.invert(x, b, p, allow_fail=True)        # warm-up (allocations, clover copies)
-        info = ctx.invert(x, b, p, allow_fail=True)
-        info.update({"config": 4, "solver": "bicgstab", "sloppy": names[sloppy], "recon_sloppy": recon,
+        info = min((ctx.invert(x, b, p, allow_fail=True) for _ in range(3)), key=lambda r: r["seconds"])
+        info.update({"config": 4, "best_of": 3, "solver": "bicgstab", "sloppy": names[sloppy], "recon_sloppy": recon,
                      "effective_gflops": info["gflop"] / info["seconds"]})
         ex["solvers"].append(info)
     p = ctx.make_params(KAPPA, CSW, 1e-10, solver=lqcd.SOLVER_GCR_DD, prec=(0, 1, 2), recon=(18, 12, 12),
                         gcr_kmax=16, schwarz_block=(8, 8, 8, 16), mr_steps=10)
     ctx.invert(x, b, p, allow_fail=True)
-    info = ctx.invert(x, b, p, allow_fail=True)
-    info.update({"config": "4 (lattice) with GCR-DD, 8^3x16 blocks", "solver": "gcr_dd", "sloppy": "fp32", "precond": "half",
+    info = min((ctx.invert(x, b, p, allow_fail=True) for _ in range(3)), key=lambda r: r["seconds"])
+    info.update({"config": "4 (lattice) with GCR-DD, 8^3x16 blocks", "best_of": 3, "solver": "gcr_dd", "sloppy": "fp32", "precond": "half",
                  "effective_gflops": info["gflop"] / info["seconds"]})
     ex["solvers"].append(info)
     if args.full:

@@ -108,7 +108,7 @@ int set_blocks(lqcd_ctx* c, const int* blk) {
   c->bm.nat = c->nat;
   c->bm.blk = make_geom(blk, bcb, nb);
   c->have_blocks = true;
-  const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * 4;
+  const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * (LQ_DSLASH_BLOCK / 32) * 4;
   if (need > c->boxdots_doubles) {
     if (c->boxdots) cudaFree(c->boxdots);
     c->boxdots = nullptr; c->boxdots_doubles = 0;

@@ -34,7 +34,7 @@ struct BlasArgs {
   double* S;              // device scalars
   double* partials;       // [nb][gridDim.x][NV]
   unsigned* counters;     // [nb], zero on entry, reset by the last CTA
-  const double* boxdots;  // MR: per-box partial dots written by the Dslash epilogue [nb][nchunk][4]
+  const double* boxdots;  // MR: per-box partial dots written by the Dslash epilogue [nb][nchunk][4], nchunk = CTAs per box x warps per CTA
   int nchunk;
   double c[4];            // host coefficients
   int i0, i1;

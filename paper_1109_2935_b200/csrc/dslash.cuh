@@ -34,7 +34,7 @@ struct DslashArgs {
   // per thread in the 80-register clover-epilogue variants.  A DOTS launch always covers whole
   // boxes, so the site range shares storage with the partial-sum pointer.
   union {
-    double* dots;       // DOTS: [box][chunk][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
+    double* dots;       // DOTS: [box][chunk][warp][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
     struct { int cb0, cb1; } range;  // !DOTS: sites [cb0, cb1) of every box are computed by this launch
   };
   int parity;           // output parity
@@ -371,11 +371,16 @@ dslash_kernel(const DslashArgs a) {
     store_site<P, 24>(acc, a.out, g.ns, idx);
   }
   if constexpr (DOTS) {
-    double red[3] = {(double)d0, (double)d1, (double)d2};   // sums over sites in fp64
-    __shared__ double sm[3 * (LQ_DSLASH_BLOCK / 32)];
-    cta_reduce<3, LQ_DSLASH_BLOCK>(red, sm);
-    if (threadIdx.x == 0) {
-      double* d = a.dots + ((long long)box * gridDim.x + blockIdx.x) * 4;
+    // per-warp partial sums (sites in fp64, fixed shuffle order: deterministic); no CTA barrier.
+    // The MR update kernel adds the gridDim.x * (LQ_DSLASH_BLOCK/32) partials of its box.
+    double red[3] = {(double)d0, (double)d1, (double)d2};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) red[k] += __shfl_down_sync(0xffffffffu, red[k], o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      double* d = a.dots + (((long long)box * gridDim.x + blockIdx.x) * (LQ_DSLASH_BLOCK / 32) + (threadIdx.x >> 5)) * 4;
       d[0] = red[0]; d[1] = red[1]; d[2] = red[2]; d[3] = 0;
     }
   }

@@ -43,7 +43,7 @@ BlasArgs mk(lqcd_ctx* c, bool blocked, char* v0 = nullptr, char* v1 = nullptr, c
   a.ns = g.ns; a.vh = g.vh; a.nb = g.nb;
   a.S = c->S; a.partials = c->partials; a.counters = c->counters;
   a.boxdots = c->boxdots;
-  a.nchunk = (g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK;
+  a.nchunk = (g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK * (LQ_DSLASH_BLOCK / 32);   // per-warp partials per box
   return a;
 }
 
