@@ -243,3 +243,51 @@ def test_cfg3_full_size_all_precisions():
             err = float(torch.linalg.vector_norm(got - wm) / torch.linalg.vector_norm(wm))
             assert err <= tol, ("matpc", prec, recon, err)
     ctx.close()
+
+
+def test_cfg5_full_size_operator_and_schwarz():
+    """BASELINE.json config 5 at full size, 48^3x96 (10.6 M sites, eps = 0.2, kappa = 0.124, c_sw = 1):
+    Dslash (fp32 and half, recon-12), Mhat (half) and the Schwarz preconditioner K with 256 blocks
+    of 12^3x24 and 10 MR steps in half precision, element by element against the oracle on the same
+    arrays.  K's tolerance is the one of DESIGN.md R7 / SURVEY 8(c).8 (error compounds over steps)."""
+    from paper_1109_2935_b200 import lqcd
+    dims, kappa, blk = (48, 48, 48, 96), 0.124, (12, 12, 12, 24)
+    Ut = inputs.random_gauge_torch(dims, 0.2, 21, device="cuda")
+    pt = inputs.gaussian_spinor_torch(dims, 22, device="cuda")
+    ctx = lqcd.Context(dims, BC, 0)
+    ctx.load_gauge(Ut)
+    ctx.build_clover(1.0)
+    U, psi = Ut.cpu().numpy(), pt.cpu().numpy()
+    del Ut
+    par = torch.from_numpy(inputs.parity_mask(dims)).cuda()
+    even = (par == 0)[..., None, None]
+    want_d = torch.from_numpy(oracle.dslash(psi, U, BC)).cuda()
+    for prec in (1, 2):
+        fin = [ctx.pack_spinor(pt, p, prec) for p in (0, 1)]
+        got = torch.zeros_like(pt)
+        for p in (0, 1):
+            fo = ctx.new_field(prec)
+            ctx.dslash(fo, fin[1 - p], p, False, prec, 12)
+            ctx.unpack_spinor(got, fo, p, prec)
+        err = float(torch.linalg.vector_norm(got - want_d) / torch.linalg.vector_norm(want_d))
+        assert err <= TOL[prec], ("dslash", prec, err)
+    del want_d
+    T = oracle.clover_term(U, 1.0)
+    want_m = torch.from_numpy(oracle.matpc(psi, U, T, BC, kappa, 0)).cuda()
+    fo = ctx.new_field(2)
+    ctx.matpc(fo, fin[0], 0, False, kappa, 2, 12)
+    got = torch.zeros_like(pt)
+    ctx.unpack_spinor(got, fo, 0, 2)
+    err = float(torch.linalg.vector_norm(got - want_m) / torch.linalg.vector_norm(want_m))
+    assert err <= TOL[2], ("matpc", err)
+    del want_m
+    for n_mr, tol in ((1, 5e-3), (10, 2e-2)):
+        want_k = torch.from_numpy(oracle.schwarz(psi, U, T, BC, kappa, 0, blk, n_mr=n_mr)).cuda()
+        fk = ctx.new_field(1)
+        ctx.schwarz(fk, ctx.pack_spinor(pt, 0, 1), 0, kappa, blk, n_mr, 1.0, 2, 12, 1)
+        got = torch.zeros_like(pt)
+        ctx.unpack_spinor(got, fk, 0, 1)
+        assert float(torch.count_nonzero(got * ~even)) == 0
+        err = float(torch.linalg.vector_norm(got - want_k) / torch.linalg.vector_norm(want_k))
+        assert err <= tol, ("schwarz", n_mr, err)
+    ctx.close()

@@ -164,3 +164,32 @@ def test_apply_host_slab_pipeline_equals_device_path():
                 c.ctx.unpack_spinor(ref, fo, parity, prec)
                 assert torch.equal(hout, ref.cpu())
                 assert _rel(hout.numpy(), oracle.matpc(psi, c.U, c.T, c.bc, kappa, parity, dagger=dagger)) <= tol
+
+
+def test_cfg4_full_size_solves_true_residual_by_oracle():
+    """BASELINE.json config 4 at full size (32^3x64, eps = 0.2, kappa = 0.124, c_sw = 1, Gaussian source):
+    mixed-precision BiCGstab (inner fp32 and half) and GCR-DD to 1e-10; the true residual
+    ||b - M x|| / ||b|| is recomputed with the ORACLE's full-lattice operator.  (The oracle's own
+    solve at this size takes minutes; x = M^-1 b is unique, so the residual pins it.)"""
+    from paper_1109_2935_b200 import lqcd
+    dims, kappa = (32, 32, 32, 64), 0.124
+    Ut = inputs.random_gauge_torch(dims, 0.2, 11, device="cuda")
+    bt = inputs.gaussian_spinor_torch(dims, 12, device="cuda")
+    ctx = lqcd.Context(dims, BC, 0)
+    ctx.load_gauge(Ut)
+    ctx.build_clover(1.0)
+    U, b = Ut.cpu().numpy(), bt.cpu().numpy()
+    del Ut
+    T = oracle.clover_term(U, 1.0)
+    bn = np.linalg.norm(b)
+    runs = [(lqcd.SOLVER_BICGSTAB, (0, 1, 1), {}), (lqcd.SOLVER_BICGSTAB, (0, 2, 2), {}),
+            (lqcd.SOLVER_GCR_DD, (0, 1, 2), dict(gcr_kmax=16, schwarz_block=(8, 8, 8, 16), mr_steps=10))]
+    for solver, prec, kw in runs:
+        p = ctx.make_params(kappa, 1.0, 1e-10, solver=solver, prec=prec, recon=(18, 12, 12), **kw)
+        x = torch.zeros_like(bt)
+        info = ctx.invert(x, bt, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-10
+        res = np.linalg.norm(b - oracle.M(x.cpu().numpy(), U, T, BC, kappa)) / bn
+        assert res <= 1.05e-10, (solver, prec, res)
+        assert abs(res - info["true_residual"]) <= 0.05 * res      # the library's fp64 residual is the oracle's
+    ctx.close()
