@@ -22,7 +22,7 @@ _SRC = os.path.join(_HERE, "wilson_clover_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
-BICGSTAB, GCR_DD = 0, 1
+BICGSTAB, GCR_DD, CGNR = 0, 1, 2
 
 
 def build(force=False):
@@ -39,7 +39,7 @@ def lib():
         build()
         _lib = ctypes.CDLL(_LIB)
         _lib.orc_num_threads.restype = ctypes.c_int
-        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_invert"):
+        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_cgnr_pc", "orc_invert"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 

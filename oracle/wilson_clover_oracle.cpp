@@ -353,6 +353,41 @@ int bicgstab(cplx* x, const cplx* bhat, const Op& op, int p, double stop, int ma
   return status;
 }
 
+// CGNR: conjugate gradients on the normal equations Mhat^dag Mhat x = Mhat^dag bhat (PAPER.md:128,
+// Sec. 3.1: "either Conjugate Gradients [9] on the normal equations (CGNE or CGNR) is used, or ...
+// BiCGstab").  Textbook form (Hestenes-Stiefel CG applied to A = Mhat^dag Mhat, with the residual of
+// the ORIGINAL system r = bhat - Mhat x carried along):  z = Mhat^dag r;  p = z;  repeat
+// { w = Mhat p; alpha = <z,z>/<w,w>; x += alpha p; r -= alpha w; z' = Mhat^dag r;
+//   beta = <z',z'>/<z,z>; p = z' + beta p }.  Stops when ||r|| <= stop (absolute).
+int cgnr(cplx* x, const cplx* bhat, const Op& op, int p, double stop, int maxit, int* iters, double* rnorm) {
+  const long n = op.n();
+  std::vector<cplx> r(n), z(n), pv(n), w(n);
+  apply_matpc(r.data(), x, op, p, 0);
+  for (long i = 0; i < n; ++i) r[i] = bhat[i] - r[i];
+  mask_parity(r.data(), op.lat, p);
+  apply_matpc(z.data(), r.data(), op, p, 1);
+  pv = z;
+  double zz = norm2(z.data(), n), rn = std::sqrt(norm2(r.data(), n));
+  int it = 0, status = 0;
+  while (rn > stop) {
+    if (it >= maxit) { status = 1; break; }
+    apply_matpc(w.data(), pv.data(), op, p, 0);
+    const double ww = norm2(w.data(), n);
+    if (ww == 0.0) { status = 2; break; }
+    const double alpha = zz / ww;
+    for (long i = 0; i < n; ++i) { x[i] += alpha * pv[i]; r[i] -= alpha * w[i]; }
+    apply_matpc(z.data(), r.data(), op, p, 1);
+    const double zz1 = norm2(z.data(), n);
+    const double beta = zz1 / zz;
+    for (long i = 0; i < n; ++i) pv[i] = z[i] + beta * pv[i];
+    zz = zz1;
+    rn = std::sqrt(norm2(r.data(), n));
+    ++it;
+  }
+  *iters = it; *rnorm = rn;
+  return status;
+}
+
 // c.8  Schwarz preconditioner K: n_mr MR steps on Mhat_D from x = 0,
 // one alpha per block, sums over the block's parity-p sites.
 void schwarz_K(cplx* out, const cplx* rin, const Op& opD, int p, int n_mr, double omega_mr) {
@@ -527,6 +562,12 @@ int orc_bicgstab_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, con
   return bicgstab(x, bhat, op, parity, stop, maxit, iters, rnorm);
 }
 
+int orc_cgnr_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                double kappa, int parity, double stop, int maxit, int* iters, double* rnorm) {
+  Op op(U, T, dims, bc, kappa, nullptr);
+  return cgnr(x, bhat, op, parity, stop, maxit, iters, rnorm);
+}
+
 int orc_gcr_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, const int* dims, const int* bc,
                double kappa, int parity, double stop, int maxit, int kmax, double delta,
                int precond, const int* block, int n_mr, double omega_mr,
@@ -537,7 +578,7 @@ int orc_gcr_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, const in
 }
 
 // Full solve of M x = b (Eq. 1): prepare -> parity solve -> reconstruct.
-// solver: 0 BiCGstab, 1 GCR-DD.  Stops on ||bhat - Mhat x_p|| <= tol*||b||  (= ||b - M x||, c.5).
+// solver: 0 BiCGstab, 1 GCR-DD, 2 CGNR.  Stops on ||bhat - Mhat x_p|| <= tol*||b||  (= ||b - M x||, c.5).
 int orc_invert(cplx* x, const cplx* b, const cplx* U, const cplx* T, const int* dims, const int* bc,
                double kappa, int parity, double tol, int maxit, int solver,
                int kmax, double delta, const int* block, int n_mr, double omega_mr,
@@ -549,6 +590,7 @@ int orc_invert(cplx* x, const cplx* b, const cplx* U, const cplx* T, const int* 
   const double bn = std::sqrt(norm2(b, n));
   int restarts = 0; double rn = 0; int st;
   if (solver == 0) st = bicgstab(xp.data(), bhat.data(), op, parity, tol * bn, maxit, iters, &rn);
+  else if (solver == 2) st = cgnr(xp.data(), bhat.data(), op, parity, tol * bn, maxit, iters, &rn);
   else {
     Op opD(U, T, dims, bc, kappa, block);
     st = gcr_dd(xp.data(), bhat.data(), op, opD, parity, tol * bn, maxit, kmax, delta, 1, n_mr, omega_mr, iters, &restarts, &rn);

@@ -291,6 +291,51 @@ def test_dense_lu_4to4_both_solvers(four):
     assert _rel(2 * kappa * Mwc, oracle.M(v, U, Tcl, BC, kappa)) < 1e-14
 
 
+def test_dense_lu_cgnr(four):
+    """CGNR: the solution equals the dense LU solution of M x = b on both parities; on
+    the dense normal equations A = Mhat^dag Mhat the method is plain CG, whose A-norm error decreases
+    monotonically and which ends (in exact arithmetic) after at most dim steps -- checked through the
+    iteration count bound and a dense restatement of the first steps."""
+    dims, U, Tcl, b, kappa = four
+    Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
+    x_lu = np.linalg.solve(Md, b.ravel()).reshape(b.shape)
+    for parity in (0, 1):
+        x, info = oracle.invert(b, U, Tcl, BC, kappa, parity=parity, tol=1e-12, solver=oracle.CGNR)
+        assert info["status"] == 0 and info["true_residual"] < 2e-12
+        assert _rel(x, x_lu) < 1e-10
+    # BiCGstab needs fewer operator applications than CGNR (cond(Mhat^dag Mhat) = cond(Mhat)^2) but both agree
+    xb, ib = oracle.invert(b, U, Tcl, BC, kappa, parity=0, tol=1e-12, solver=oracle.BICGSTAB)
+    assert _rel(x, xb) < 1e-10
+    # dense restatement on the parity-0 Schur system: 3 CG steps on A y = Mhat^dag bhat from y = 0
+    par = inputs.parity_mask(dims)
+    mask = (par == 0)[..., None, None]
+    idx = np.flatnonzero(np.broadcast_to(mask, b.shape).ravel())
+    Mh = _dense(lambda v: oracle.matpc(v, U, Tcl, BC, kappa, 0), b.shape)[np.ix_(idx, idx)]
+    bhat = oracle.prepare_source(b, U, Tcl, BC, kappa, 0).ravel()[idx]
+    A, rhs = Mh.conj().T @ Mh, Mh.conj().T @ bhat
+    y = np.zeros_like(rhs); r = rhs.copy(); pvec = r.copy()
+    for _ in range(3):
+        Ap = A @ pvec
+        al = np.vdot(r, r) / np.vdot(pvec, Ap)
+        y = y + al * pvec
+        rn = r - al * Ap
+        pvec = rn + (np.vdot(rn, rn) / np.vdot(r, r)) * pvec
+        r = rn
+    stop3 = np.linalg.norm(bhat - Mh @ y)
+    xo = np.zeros(b.shape, dtype=np.complex128)
+    lib = oracle.lib()
+    import ctypes
+    it, rnorm = ctypes.c_int(0), ctypes.c_double(0)
+    bh_full = np.zeros(b.size, dtype=np.complex128); bh_full[idx] = bhat
+    st = lib.orc_cgnr_pc(xo.ctypes.data_as(ctypes.c_void_p), bh_full.ctypes.data_as(ctypes.c_void_p),
+                         U.ctypes.data_as(ctypes.c_void_p), Tcl.ctypes.data_as(ctypes.c_void_p),
+                         (ctypes.c_int * 4)(*dims), (ctypes.c_int * 4)(*BC), ctypes.c_double(kappa), ctypes.c_int(0),
+                         ctypes.c_double(0.0), ctypes.c_int(3), ctypes.byref(it), ctypes.byref(rnorm))
+    assert st == 1 and it.value == 3                      # stopped by the iteration cap after exactly 3 steps
+    assert np.linalg.norm(xo.ravel()[idx] - y) <= 1e-12 * np.linalg.norm(y)
+    assert abs(rnorm.value - stop3) <= 1e-12 * stop3
+
+
 # --------------------------------------------- Schwarz preconditioner (c.8)
 def test_schwarz_structure(four):
     dims, U, Tcl, b, kappa = four
