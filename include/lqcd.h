@@ -8,7 +8,7 @@
  *   problem           M x = b                                    PAPER.md:88-92  Sec. 2.1 Eq. 1
  *   operator          M = A(kappa) - kappa D,  A = 1 + kappa T   PAPER.md:98-108 Sec. 2.2 Eq. 2 (R1-R4)
  *   even-odd          Mhat = A_pp - kappa^2 D A^-1 D             PAPER.md:128    Sec. 3.1     (R6)
- *   solvers           mixed-precision BiCGstab
+ *   solvers           mixed-precision BiCGstab, CGNR
  *                     GCR-DD (Algorithm 1) + additive Schwarz/MR PAPER.md:146, :248-292 Sec. 8.1
  *
  * Conventions
@@ -65,6 +65,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 
 #define LQCD_SOLVER_BICGSTAB 0
 #define LQCD_SOLVER_GCR_DD   1
+#define LQCD_SOLVER_CGNR     2   /* CG on Mhat^dag Mhat x = Mhat^dag bhat, mixed precision, reliable updates */
 
 #define LQCD_FIELD_SPINOR_PARITY 0
 
@@ -150,7 +151,7 @@ typedef struct {
 
 typedef struct {
   int    status;          /* LQCD_OK, LQCD_ENOCONV, LQCD_EBREAKDOWN */
-  int    iterations;      /* BiCGstab iterations / GCR outer iterations */
+  int    iterations;      /* BiCGstab / CGNR iterations, GCR outer iterations */
   int    restarts;        /* reliable updates (BiCGstab) or restarts (GCR) */
   int    matpc_sloppy, matpc_outer, matpc_precond;   /* operator applications by precision */
   double true_residual;   /* ||bhat - Mhat x_p|| / ||b|| in fp64 = ||b - M x|| / ||b|| */

@@ -25,6 +25,7 @@ cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s) 
 LQ_INST(OpZero) LQ_INST(OpNorm2) LQ_INST(OpCdot) LQ_INST(OpAxpyNorm) LQ_INST(OpXmyNorm)
 LQ_INST(OpBicgInit) LQ_INST(OpBicgP) LQ_INST(OpBicgAlpha) LQ_INST(OpBicgS) LQ_INST(OpBicgOmega) LQ_INST(OpBicgXR)
 LQ_INST(OpGcrScale)
+LQ_INST(OpCgInit) LQ_INST(OpCgP) LQ_INST(OpCgAlpha) LQ_INST(OpCgXR)
 typedef OpMrUpdate<true, false> OpMrFirst;
 typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;

@@ -181,6 +181,59 @@ struct OpBicgXR {          // v0 = x, v1 = p, v2 = s->r, v3 = t, v4 = rtilde
   }
 };
 
+// ---- CGNR (CG on the normal equations Mhat^dag Mhat x = Mhat^dag bhat) -------------
+// Device scalars: zz = <z,z> in S_RHO, alpha in S_ALPHA, beta in S_BETA (all real), rr in S_RR.
+struct OpCgInit {          // v0 = z, v1 = p : p = z ; zz = ||z||^2          (start, i0 = 0)
+  //                          i0 = 1 (after a reliable update): beta = ||z||^2 / zz_old ; p = z + beta p is done by OpCgP
+  static constexpr int NV = 1, READ = 1, WRITE = 0;
+  typedef NoCoef Coef;
+  LQ_DEV static void prepare(Coef&, const BlasArgs&, int) {}
+  template <typename R> LQ_DEV static void site(const Coef&, R* z, R*, R*, R*, R*, double* red) { site_norm2(z, red[0]); }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+    double* S = a.S;
+    if (a.i0 == 0) { S[S_BETA] = 0; S[S_FLAG] = 0; }
+    else S[S_BETA] = (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;
+    S[S_RHO] = s[0];
+  }
+};
+
+struct OpCgP {             // v0 = p, v1 = z : p = z + beta p
+  static constexpr int NV = 0, READ = 3, WRITE = 1;
+  struct Coef { double b; };
+  LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int) { c.b = a.S[S_BETA]; }
+  template <typename R> LQ_DEV static void site(const Coef& c, R* p, R* z, R*, R*, R*, double*) {
+    const R b = (R)c.b;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) p[k] = fma_(b, p[k], z[k]);
+  }
+  LQ_DEV static void finalize(const double*, const BlasArgs&, int) {}
+};
+
+struct OpCgAlpha {         // v0 = w = Mhat p : alpha = zz / ||w||^2
+  static constexpr int NV = 1, READ = 1, WRITE = 0;
+  typedef NoCoef Coef;
+  LQ_DEV static void prepare(Coef&, const BlasArgs&, int) {}
+  template <typename R> LQ_DEV static void site(const Coef&, R* w, R*, R*, R*, R*, double* red) { site_norm2(w, red[0]); }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+    double* S = a.S;
+    if (!(s[0] > 0.0)) { S[S_FLAG] = 1; S[S_ALPHA] = 0; return; }
+    S[S_ALPHA] = S[S_RHO] / s[0];
+  }
+};
+
+struct OpCgXR {            // v0 = x, v1 = p, v2 = r, v3 = w : x += alpha p ; r -= alpha w ; rr = ||r||^2
+  static constexpr int NV = 1, READ = 15, WRITE = 5;
+  struct Coef { double a; };
+  LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int) { c.a = a.S[S_ALPHA]; }
+  template <typename R> LQ_DEV static void site(const Coef& c, R* x, R* p, R* r, R* w, R*, double* red) {
+    const R al = (R)c.a;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) { x[k] = fma_(al, p[k], x[k]); r[k] = fma_(-al, w[k], r[k]); }
+    site_norm2(r, red[0]);
+  }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) { a.S[S_RR] = s[0]; }
+};
+
 // ---- GCR (Algorithm 1) --------------------------------------------------------------------------
 struct OpGcrScale {        // v0 = z_k, v1 = rhat : z_k /= gamma ; rhat -= alpha z_k ; rr = ||rhat||^2
   static constexpr int NV = 1, READ = 3, WRITE = 3;

@@ -2,6 +2,8 @@
 //   * mixed-precision BiCGstab with reliable updates  (reading R11)
 //   * additive-Schwarz preconditioner K = n_MR minimum-residual steps on the Dirichlet-cut
 //     Mhat_D, one alpha per block                      (reading R7)
+//   * CGNR with reliable updates                        ("CG on the normal equations")
+//   * CGNR with reliable updates                        (CG on the normal equations)
 //   * GCR-DD, Algorithm 1                               (reading R8)
 // The host loop only launches kernels; all Krylov scalars live on the device (blas_ops.cuh).
 // One scalar (||r||^2) is read back per iteration for the convergence / restart decision.
@@ -198,6 +200,78 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
   return status;
 }
 
+// ---------------------------------------------------------------- CGNR with reliable updates
+// CG on Mhat^dag Mhat x = Mhat^dag bhat.  The residual of the ORIGINAL system
+// r = bhat - Mhat x is carried in low precision and replaced by the true fp64 residual at reliable
+// updates (same trigger as BiCGstab, R11); the search direction is kept across updates with
+// beta = ||z_new||^2 / ||z_old||^2.  Per iteration: Mhat p, Mhat^dag r and four fused BLAS-1 passes.
+int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
+               lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
+  const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
+  const long long ns = c->nat.ns;
+  Work wk(c);
+  char *r_hi, *xl, *rl, *z, *pv, *w;
+  int rc;
+  if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
+  char** lo[] = {&xl, &rl, &z, &pv, &w};
+  for (char** q : lo) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
+  double rn;
+  if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
+  cnt.mat_outer++;
+  res->iterations = 0; res->restarts = 0;
+  const double delta = p.delta > 0 ? p.delta : 0.1;
+  int status = LQCD_OK;
+  auto fold = [&]() -> int {            // x += x_l (outer precision), x_l = 0
+    MultiArgs m; memset(&m, 0, sizeof(m));
+    m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
+    cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+    BlasArgs a = mk(c, false, xl);
+    return blas<OpZero>(c, ps, a, s);
+  };
+  if (rn > stop) {
+    if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+    for (char* q : {xl, pv}) { BlasArgs a = mk(c, false, q); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+    if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+    cnt.mat_sloppy++;
+    { BlasArgs a = mk(c, false, z); a.i0 = 0; if ((rc = blas<OpCgInit>(c, ps, a, s))) return rc; }
+    { BlasArgs a = mk(c, false, pv, z); if ((rc = blas<OpCgP>(c, ps, a, s))) return rc; }      // beta = 0: p = z
+    double maxr = rn;
+    int it = 0;
+    while (true) {
+      if (it >= p.max_iter) { if ((rc = fold())) return rc; status = LQCD_ENOCONV; break; }
+      if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      { BlasArgs a = mk(c, false, w); if ((rc = blas<OpCgAlpha>(c, ps, a, s))) return rc; }
+      { BlasArgs a = mk(c, false, xl, pv, rl, w); if ((rc = blas<OpCgXR>(c, ps, a, s))) return rc; }
+      cnt.mat_sloppy++; cnt.blas_flop_sites += 24.0 * (2 + 4 + 2); ++it;
+      if ((rc = read_S(c, S_RR, 2, s))) return rc;
+      const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
+      if (!(rr == rr) || flag != 0.0) status = LQCD_EBREAKDOWN;
+      const double rln = sqrt(rr);
+      if (rln > maxr) maxr = rln;
+      if (status == LQCD_EBREAKDOWN || rln <= stop || rln < delta * maxr) {
+        if ((rc = fold())) return rc;
+        if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
+        cnt.mat_outer++; res->restarts++;
+        if (rn <= stop) { status = LQCD_OK; break; }
+        if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
+        if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+        maxr = rn;
+      }
+      // z = Mhat^dag r ; beta = <z,z>/<z,z>_old ; p = z + beta p   (after a breakdown: restart, beta = 0)
+      if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      cnt.mat_sloppy++;
+      { BlasArgs a = mk(c, false, z); a.i0 = (status == LQCD_EBREAKDOWN) ? 0 : 1; if ((rc = blas<OpCgInit>(c, ps, a, s))) return rc; }
+      status = LQCD_OK;
+      { BlasArgs a = mk(c, false, pv, z); if ((rc = blas<OpCgP>(c, ps, a, s))) return rc; }
+      cnt.blas_flop_sites += 24.0 * (2 + 2);
+    }
+    res->iterations = it;
+  }
+  res->iterated_residual = rn;
+  return status;
+}
+
 // ---------------------------------------------------------------- GCR-DD (Algorithm 1)
 int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
               lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
@@ -288,7 +362,7 @@ int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
   if ((p->parity | 1) != 1) return fail(c, LQCD_EINVAL, "parity");
   for (int pr : {p->prec_outer, p->prec_sloppy, p->prec_precond}) if (pr < 0 || pr > 2) return fail(c, LQCD_EINVAL, "precision");
   for (int r : {p->recon_outer, p->recon_sloppy, p->recon_precond}) if (recon_index(r) < 0) return fail(c, LQCD_EINVAL, "recon");
-  if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "solver");
+  if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD && p->solver != LQCD_SOLVER_CGNR) return fail(c, LQCD_EINVAL, "solver");
   if (!(p->tol > 0) || p->max_iter < 1) return fail(c, LQCD_EINVAL, "tol / max_iter");
   if (p->solver == LQCD_SOLVER_GCR_DD && p->precondition && p->mr_steps < 1) return fail(c, LQCD_EINVAL, "mr_steps");
   return LQCD_OK;
@@ -366,6 +440,7 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   const double stop = p->tol * bnorm;
   int status;
   if (p->solver == LQCD_SOLVER_BICGSTAB) status = solve_bicgstab(c, xp, bhat, *p, stop, res, cnt, s);
+  else if (p->solver == LQCD_SOLVER_CGNR) status = solve_cgnr(c, xp, bhat, *p, stop, res, cnt, s);
   else status = solve_gcr(c, xp, bhat, *p, stop, res, cnt, s);
   if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) { cudaEventDestroy(e0); cudaEventDestroy(e1); return status; }
   // true residual of the Schur system in the outer precision = ||b - M x|| (R6)

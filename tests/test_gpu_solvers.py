@@ -193,3 +193,28 @@ def test_cfg4_full_size_solves_true_residual_by_oracle():
         assert res <= 1.05e-10, (solver, prec, res)
         assert abs(res - info["true_residual"]) <= 0.05 * res      # the library's fp64 residual is the oracle's
     ctx.close()
+
+
+@pytest.mark.parametrize("prec", [(0, 0, 0), (0, 1, 1), (0, 2, 2)])
+def test_cgnr(mid, prec):
+    """CGNR in fp64 and mixed precision: same unique solution as the oracle's solve, true
+    residual by the oracle's operator; in fp64 the iteration count equals the oracle's CGNR (+-1: same
+    recurrence, different summation order); CGNR needs more operator applications than BiCGstab."""
+    c = mid
+    lq = c.lqcd
+    kappa = 0.124
+    b = inputs.gaussian_spinor(c.dims, 2)
+    for parity in (0, 1):
+        p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_CGNR, prec=prec, recon=(18, 12, 12), parity=parity)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-10
+        res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+        assert res <= 1.05e-10
+        xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=parity, tol=1e-10, solver=oracle.CGNR)
+        assert _rel(x, xo) <= 1e-8
+        if prec == (0, 0, 0):
+            assert abs(info["iterations"] - io["iterations"]) <= 1
+            assert info["matpc_sloppy"] == 2 * info["iterations"]      # Mhat^dag r0, then (Mhat p, Mhat^dag r) per step, none after the last
+    pb = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB, prec=prec, recon=(18, 12, 12))
+    xb, ib = _solve(c, b, pb)
+    assert ib["matpc_sloppy"] < info["matpc_sloppy"]
