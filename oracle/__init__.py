@@ -39,7 +39,7 @@ def lib():
         build()
         _lib = ctypes.CDLL(_LIB)
         _lib.orc_num_threads.restype = ctypes.c_int
-        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_cgnr_pc", "orc_invert"):
+        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_cgnr_pc", "orc_invert", "orc_invert_sym"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -115,6 +115,26 @@ def matpc(psi, U, Tcl, bc, kappa, parity, dagger=False, block=None):
     lib().orc_matpc(_p(out), _p(psi), _p(U), _p(Tcl), _i4(dims_of(psi)), _i4(bc), ctypes.c_double(kappa),
                     ctypes.c_int(parity), ctypes.c_int(int(dagger)), _blk(block))
     return out
+
+
+def matpc_sym(psi, U, Tcl, bc, kappa, parity, dagger=False):
+    """Symmetric even-odd form: Mhat_s = 1 - kappa^2 A_pp^-1 D A_pbar^-1 D  (= A_pp^-1 Mhat)."""
+    psi, U, Tcl = _c(psi), _c(U), _c(Tcl)
+    out = np.empty_like(psi)
+    lib().orc_matpc_sym(_p(out), _p(psi), _p(U), _p(Tcl), _i4(dims_of(psi)), _i4(bc), ctypes.c_double(kappa),
+                        ctypes.c_int(parity), ctypes.c_int(int(dagger)))
+    return out
+
+
+def invert_sym(b, U, Tcl, bc, kappa, parity=0, tol=1e-12, maxit=10000, solver=BICGSTAB):
+    """Full-lattice solve of M x = b through the symmetric Schur system.  Returns (x, info)."""
+    b, U, Tcl = _c(b), _c(U), _c(Tcl)
+    x = np.zeros_like(b)
+    it, tr = ctypes.c_int(0), ctypes.c_double(0)
+    st = lib().orc_invert_sym(_p(x), _p(b), _p(U), _p(Tcl), _i4(dims_of(b)), _i4(bc), ctypes.c_double(kappa),
+                              ctypes.c_int(parity), ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.c_int(solver),
+                              ctypes.byref(it), ctypes.byref(tr))
+    return x, dict(status=st, iterations=it.value, true_residual=tr.value)
 
 
 def prepare_source(b, U, Tcl, bc, kappa, parity):

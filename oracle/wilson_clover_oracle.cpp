@@ -275,8 +275,9 @@ void mask_parity(cplx* v, const Lat& lat, int keep) {
 struct Op {                         // everything an operator application needs
   const cplx* U; const cplx* T; Lat lat; double kappa;
   const int* blk;                   // Schwarz block extents or nullptr
-  Op(const cplx* U_, const cplx* T_, const int* dims, const int* bc, double k, const int* blk_)
-    : U(U_), T(T_), lat(dims, bc), kappa(k), blk(blk_) {}
+  int sym;                          // 0: asymmetric Schur complement (default), 1: symmetric form (c.5 "Optional")
+  Op(const cplx* U_, const cplx* T_, const int* dims, const int* bc, double k, const int* blk_, int sym_ = 0)
+    : U(U_), T(T_), lat(dims, bc), kappa(k), blk(blk_), sym(sym_) {}
   long n() const { return lat.V * 12; }
 };
 
@@ -292,7 +293,34 @@ void apply_M(cplx* out, const cplx* in, const Op& op, int dagger) {
 
 // c.5  Mhat = A_pp - kappa^2 D_{p pbar} A_{pbar pbar}^{-1} D_{pbar p}   (reading R6), by masking.
 // in/out are full-lattice arrays; only parity-p sites of `in` are read, the rest of out is 0.
+// Symmetric form (same reference [11]):  Mhat_s = 1 - kappa^2 A_pp^-1 D A_pbar^-1 D = A_pp^-1 Mhat,
+// Mhat_s^dag = 1 - kappa^2 D^dag A_pbar^-1 D^dag A_pp^-1 (A is Hermitian).
+void apply_matpc_sym(cplx* out, const cplx* in, const Op& op, int p, int dagger) {
+  const long n = op.n();
+  std::vector<cplx> xin(in, in + n), t1(n), t2(n);
+  mask_parity(xin.data(), op.lat, p);
+  if (!dagger) {
+    dslash(t1.data(), xin.data(), op.U, op.lat, 0, op.blk);
+    mask_parity(t1.data(), op.lat, 1 - p);
+    clover_apply(t2.data(), t1.data(), op.T, op.lat, op.kappa, 1, 1 - p);
+    dslash(t1.data(), t2.data(), op.U, op.lat, 0, op.blk);
+    mask_parity(t1.data(), op.lat, p);
+    clover_apply(t2.data(), t1.data(), op.T, op.lat, op.kappa, 1, p);
+  } else {
+    clover_apply(t1.data(), xin.data(), op.T, op.lat, op.kappa, 1, p);
+    dslash(t2.data(), t1.data(), op.U, op.lat, 1, op.blk);
+    mask_parity(t2.data(), op.lat, 1 - p);
+    clover_apply(t1.data(), t2.data(), op.T, op.lat, op.kappa, 1, 1 - p);
+    dslash(t2.data(), t1.data(), op.U, op.lat, 1, op.blk);
+    mask_parity(t2.data(), op.lat, p);
+  }
+  const double k2 = op.kappa * op.kappa;
+#pragma omp parallel for schedule(static)
+  for (long i = 0; i < n; ++i) out[i] = xin[i] - k2 * t2[i];
+}
+
 void apply_matpc(cplx* out, const cplx* in, const Op& op, int p, int dagger) {
+  if (op.sym) { apply_matpc_sym(out, in, op, p, dagger); return; }
   const long n = op.n();
   std::vector<cplx> xin(in, in + n), t1(n), t2(n);
   mask_parity(xin.data(), op.lat, p);
@@ -575,6 +603,38 @@ int orc_gcr_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, const in
   Op op(U, T, dims, bc, kappa, nullptr);
   Op opD(U, T, dims, bc, kappa, block);
   return gcr_dd(x, bhat, op, opD, parity, stop, maxit, kmax, delta, precond, n_mr, omega_mr, iters, restarts, rnorm);
+}
+
+// Symmetric even-odd form: out = Mhat_s in  (or Mhat_s^dag in)
+void orc_matpc_sym(cplx* out, const cplx* in, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                   double kappa, int parity, int dagger) {
+  Op op(U, T, dims, bc, kappa, nullptr, 1);
+  apply_matpc(out, in, op, parity, dagger);
+}
+
+// Full solve of M x = b through the SYMMETRIC Schur system Mhat_s x_p = A_pp^-1 bhat (solver 0 BiCGstab,
+// 2 CGNR).  ||b - M x|| = ||A_pp r_s|| <= ||A|| ||r_s|| < 2 ||r_s|| (clover eigenvalues within
+// 1 +- 6 kappa c_sw, kappa c_sw < 1/6), so iterating to ||r_s|| <= tol ||b|| / 2 meets the full-system criterion.
+int orc_invert_sym(cplx* x, const cplx* b, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                   double kappa, int parity, double tol, int maxit, int solver, int* iters, double* true_res) {
+  Op op(U, T, dims, bc, kappa, nullptr, 1);
+  Op opa(U, T, dims, bc, kappa, nullptr, 0);
+  const long n = op.n();
+  std::vector<cplx> bhat(n), bs(n), xp(n, 0);
+  orc_prepare_source(bhat.data(), b, U, T, dims, bc, kappa, parity);
+  clover_apply(bs.data(), bhat.data(), T, op.lat, kappa, 1, parity);
+  const double bn = std::sqrt(norm2(b, n));
+  double rn = 0; int st;
+  if (solver == 2) st = cgnr(xp.data(), bs.data(), op, parity, 0.5 * tol * bn, maxit, iters, &rn);
+  else st = bicgstab(xp.data(), bs.data(), op, parity, 0.5 * tol * bn, maxit, iters, &rn);
+  for (long i = 0; i < n; ++i) x[i] = xp[i];
+  orc_reconstruct(x, b, U, T, dims, bc, kappa, parity);
+  std::vector<cplx> mx(n);
+  apply_M(mx.data(), x, opa, 0);
+  double d = 0;
+  for (long i = 0; i < n; ++i) d += std::norm(b[i] - mx[i]);
+  *true_res = std::sqrt(d) / bn;
+  return st;
 }
 
 // Full solve of M x = b (Eq. 1): prepare -> parity solve -> reconstruct.

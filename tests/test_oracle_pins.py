@@ -336,6 +336,28 @@ def test_dense_lu_cgnr(four):
     assert abs(rnorm.value - stop3) <= 1e-12 * stop3
 
 
+def test_symmetric_even_odd_form(four):
+    """Mhat_s = A_pp^-1 Mhat as dense matrices; the dagger flag is the true adjoint; solving through the
+    symmetric system gives the dense-LU solution of M x = b with the full-system criterion met."""
+    dims, U, Tcl, b, kappa = four
+    par = inputs.parity_mask(dims)
+    for p in (0, 1):
+        mask = (par == p)[..., None, None]
+        idx = np.flatnonzero(np.broadcast_to(mask, b.shape).ravel())
+        Mh = _dense(lambda v: oracle.matpc(v, U, Tcl, BC, kappa, p), b.shape)[np.ix_(idx, idx)]
+        Ms = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p), b.shape)[np.ix_(idx, idx)]
+        Msd = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p, dagger=True), b.shape)[np.ix_(idx, idx)]
+        A = _dense(lambda v: oracle.clover_apply(v, Tcl, kappa, parity=p), b.shape)[np.ix_(idx, idx)]
+        assert np.linalg.norm(A @ Ms - Mh) <= 1e-13 * np.linalg.norm(Mh)
+        assert np.linalg.norm(Msd - Ms.conj().T) <= 1e-13 * np.linalg.norm(Ms)
+    Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
+    x_lu = np.linalg.solve(Md, b.ravel()).reshape(b.shape)
+    for solver in (oracle.BICGSTAB, oracle.CGNR):
+        x, info = oracle.invert_sym(b, U, Tcl, BC, kappa, parity=0, tol=1e-12, solver=solver)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-12
+        assert _rel(x, x_lu) < 1e-10
+
+
 # --------------------------------------------- Schwarz preconditioner (c.8)
 def test_schwarz_structure(four):
     dims, U, Tcl, b, kappa = four
