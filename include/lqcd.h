@@ -67,6 +67,9 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_SOLVER_GCR_DD   1
 #define LQCD_SOLVER_CGNR     2   /* CG on Mhat^dag Mhat x = Mhat^dag bhat, mixed precision, reliable updates */
 
+#define LQCD_MATPC_ASYMMETRIC 0
+#define LQCD_MATPC_SYMMETRIC  1
+
 #define LQCD_FIELD_SPINOR_PARITY 0
 
 /* Create a context for a lattice dims = (X,Y,Z,T), all even and >= 2, with per-direction
@@ -110,6 +113,12 @@ int lqcd_clover(lqcd_ctx* ctx, void* out, const void* in, int parity, int invers
 int lqcd_matpc(lqcd_ctx* ctx, void* out, const void* in, int parity, int dagger,
                double kappa, int prec, int recon, void* stream);
 
+/* Symmetric even-odd form (SURVEY.md 8(c).5 "Optional"; same Schur complement, reference [11] of the
+ * paper, left-multiplied by A_pp^-1):  out = Mhat_s in,  Mhat_s = 1 - kappa^2 A_pp^-1 D A_pbar^-1 D = A_pp^-1 Mhat;
+ * dagger != 0 applies Mhat_s^dag = 1 - kappa^2 D^dag A^-1 D^dag A^-1.  Same bytes and flops as lqcd_matpc. */
+int lqcd_matpc_sym(lqcd_ctx* ctx, void* out, const void* in, int parity, int dagger,
+                   double kappa, int prec, int recon, void* stream);
+
 /* Multi-right-hand-side forms (not in the paper): the same operators applied
  * to nrhs (1..LQCD_MAX_RHS) packed fields that share the gauge field, in one launch per Dslash.
  * `in` and `out` hold the nrhs packed fields of precision `prec` back to back (field r starts at
@@ -147,6 +156,9 @@ typedef struct {
   double mr_omega;        /* 1.0 */
   int    use_initial_guess;
   int    precondition;    /* GCR: 1 = Schwarz/MR preconditioner, 0 = plain GCR */
+  int    matpc_type;      /* LQCD_MATPC_ASYMMETRIC (default, R6) or LQCD_MATPC_SYMMETRIC: the Krylov iteration runs on
+                             Mhat_s x_p = A_pp^-1 bhat; the stopping test stays ||b - M x|| <= tol ||b|| (fp64, at
+                             reliable updates).  BiCGstab and CGNR only. */
 } lqcd_invert_params;
 
 typedef struct {

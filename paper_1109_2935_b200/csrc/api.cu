@@ -148,12 +148,32 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
   return LQCD_OK;
 }
 
-// out = Mhat in  (R6):  tmp = A^-1 D in ;  out = A in - kappa^2 D tmp
+// out = Mhat in  (R6):  tmp = A^-1 D in ;  out = A in - kappa^2 D tmp.
+// sym != 0: the symmetric form Mhat_s = 1 - kappa^2 A^-1 D A^-1 D:  tmp = A^-1 D in ; out = in - kappa^2 A^-1 D tmp,
+// and Mhat_s^dag = 1 - kappa^2 D^dag A^-1 D^dag A^-1:  t0 = A^-1 in ; tmp = A^-1 D^dag t0 ; out = in - kappa^2 D^dag tmp.
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
-             bool blocked, bool dots, cudaStream_t s) {
+             bool blocked, bool dots, cudaStream_t s, int sym) {
   char* tmp;
   int rc = get_tmp(c, prec, blocked, &tmp);
   if (rc) return rc;
+  if (sym) {
+    if (blocked || dots) return fail(c, LQCD_EINVAL, "symmetric form is not available for the Schwarz operator");
+    if (!dagger) {
+      rc = op_dslash(c, tmp, in, nullptr, 1 - parity, 0, prec, recon, EPI_CLOVOUT, 0.0, kappa, false, s);
+      if (rc) return rc;
+      return op_dslash(c, out, tmp, in, parity, 0, prec, recon, EPI_XPAY_CLOVD, -kappa * kappa, kappa, false, s);
+    }
+    char*& t2 = c->tmp2[prec];
+    if (!t2) { rc = dev_alloc(c, (void**)&t2, spinor_bytes(prec, c->nat.ns)); if (rc) return rc; }
+    const char *A, *Ai;
+    rc = get_clover(c, prec, kappa, false, &A, &Ai, s);
+    if (rc) return rc;
+    cudaError_t e = run_clover_apply(prec, t2, in, Ai, c->nat, parity, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_apply", e);
+    rc = op_dslash(c, tmp, t2, nullptr, 1 - parity, 1, prec, recon, EPI_CLOVOUT, 0.0, kappa, false, s);
+    if (rc) return rc;
+    return op_dslash(c, out, tmp, in, parity, 1, prec, recon, EPI_XPAY, -kappa * kappa, kappa, false, s);
+  }
   rc = op_dslash(c, tmp, in, nullptr, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, blocked, s);
   if (rc) return rc;
   return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, dots ? EPI_CLOVX_XPAY_DOTS : EPI_CLOVX_XPAY,
@@ -235,7 +255,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   memset(c->gauge, 0, sizeof(c->gauge)); memset(c->bgauge, 0, sizeof(c->bgauge));
   memset(c->clov, 0, sizeof(c->clov)); memset(c->clovinv, 0, sizeof(c->clovinv));
   memset(c->bclov, 0, sizeof(c->bclov)); memset(c->bclovinv, 0, sizeof(c->bclovinv));
-  memset(c->tmp, 0, sizeof(c->tmp)); memset(c->btmp, 0, sizeof(c->btmp));
+  memset(c->tmp, 0, sizeof(c->tmp)); memset(c->btmp, 0, sizeof(c->btmp)); memset(c->tmp2, 0, sizeof(c->tmp2));
   c->S = nullptr; c->partials = nullptr; c->counters = nullptr; c->boxdots = nullptr; c->hS = nullptr;
   c->boxdots_doubles = 0;
   memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
@@ -261,7 +281,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   cudaSetDevice(c->device);
   cudaDeviceSynchronize();
   drop_gauge_copies(c); drop_clover_copies(c); drop_block_copies(c);
-  for (int i = 0; i < 3; ++i) free_p(c->tmp[i]);
+  for (int i = 0; i < 3; ++i) { free_p(c->tmp[i]); free_p(c->tmp2[i]); }
   if (c->g64) cudaFree(c->g64);
   if (c->T72) cudaFree(c->T72);
   if (c->S) cudaFree(c->S);
@@ -356,6 +376,13 @@ int lqcd_clover(lqcd_ctx* c, void* out, const void* in, int parity, int inverse,
   cudaError_t e = run_clover_apply(prec, (char*)out, (const char*)in, inverse ? Ai : A, c->nat, parity, s);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "clover_apply", e);
+}
+
+int lqcd_matpc_sym(lqcd_ctx* c, void* out, const void* in, int parity, int dagger, double kappa, int prec, int recon, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity | 1) != 1 || prec < 0 || prec > 2) return fail(c, LQCD_EINVAL, "matpc_sym arguments");
+  cudaSetDevice(c->device);
+  return op_matpc(c, (char*)out, (const char*)in, parity, dagger ? 1 : 0, kappa, prec, recon, false, false, (cudaStream_t)stream, 1);
 }
 
 int lqcd_dslash_mrhs(lqcd_ctx* c, void* out, const void* in, int nrhs, int parity_out, int dagger, int prec, int recon, void* stream) {

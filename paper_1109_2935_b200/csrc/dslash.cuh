@@ -182,12 +182,23 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
 
 // Fused epilogue of one site (shared by the single- and multi-right-hand-side kernels):
 //   XPAY: acc = [A] y + coef * acc (CLOVX: A = clover block of the site);  CLOVOUT: acc = C acc;
+//   XPAY && CLOVX && CLOVOUT: acc = y + coef * C acc (symmetric even-odd form);
 //   DOTS: d0 + i d1 += <acc, y>, d2 += <acc, acc> for this site (before CLOVOUT; only used with CLOVX).
 template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
 LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __restrict__ y, const char* __restrict__ clov_y,
                             const char* __restrict__ clov_out, double coef_d, int p, long long ns, long long idx,
                             typename P::real& d0, typename P::real& d1, typename P::real& d2) {
   typedef typename P::real R;
+  if constexpr (XPAY && CLOVX && CLOVOUT) {
+    // symmetric even-odd form, second half: acc = y + coef * C acc
+    R t[24], yv[24];
+    clover_site<P>(t, acc, clov_out + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+    load_site<P, 24>(yv, y, ns, idx);
+    const R coef = (R)coef_d;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) acc[k] = fma_(coef, t[k], yv[k]);
+    return;
+  }
   if constexpr (XPAY) {
     R yv[24];
     load_site<P, 24>(yv, y, ns, idx);
@@ -393,7 +404,8 @@ enum DslashEpi {
   EPI_CLOVX_XPAY = 2, // out = A y + a D in
   EPI_XPAY = 3,       // out = y + a D in
   EPI_XPAY_CLOVOUT = 4, // out = C (y + a D in)
-  EPI_CLOVX_XPAY_DOTS = 5  // EPI_CLOVX_XPAY + per-box <out,y>, <out,out>
+  EPI_CLOVX_XPAY_DOTS = 5, // EPI_CLOVX_XPAY + per-box <out,y>, <out,out>
+  EPI_XPAY_CLOVD = 6       // out = y + a C (D in)   (symmetric even-odd form)
 };
 
 template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);

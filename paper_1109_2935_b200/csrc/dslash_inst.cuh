@@ -49,6 +49,7 @@ static cudaError_t launch_dslash_r(const DslashArgs& a, int epi, cudaStream_t s)
     case EPI_XPAY:            launch_one<P, RECON, true, false, false, false>(a, grid, block, s); break;
     case EPI_XPAY_CLOVOUT:    launch_one<P, RECON, true, false, true, false>(a, grid, block, s); break;
     case EPI_CLOVX_XPAY_DOTS: launch_one<P, RECON, true, true, false, true>(a, grid, block, s); break;
+    case EPI_XPAY_CLOVD:      launch_one<P, RECON, true, true, true, false>(a, grid, block, s); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

@@ -87,6 +87,7 @@ struct lqcd_ctx {
   char* bclovinv[3];
   // workspace
   char* tmp[3];           // matpc temporary, natural layout, per precision
+  char* tmp2[3];          // second temporary (symmetric form, dagger)
   char* btmp[3];          // block-major temporary
   double* S;              // device scalars (lq::S_TOTAL doubles)
   double* partials;       // reduction partials

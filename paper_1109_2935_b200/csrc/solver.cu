@@ -92,6 +92,21 @@ int residual(lqcd_ctx* c, char* r, const char* b, const char* x, int parity, dou
 
 struct Counts { long long mat_sloppy = 0, mat_outer = 0, mat_precond = 0; double blas_flop_sites = 0; };
 
+// Symmetric even-odd form (lqcd.h LQCD_MATPC_SYMMETRIC): the Krylov iteration runs on
+// Mhat_s x = A^-1 bhat, whose residual is r_s = A^-1 (bhat - Mhat x).  Called right after residual():
+// r <- A_pp^-1 r in place (outer precision) and *rsn = ||r_s||.  The convergence test stays on ||bhat - Mhat x||.
+int to_symmetric_residual(lqcd_ctx* c, char* r, int parity, double kappa, int prec, double* rsn, cudaStream_t s) {
+  const char *A, *Ai;
+  int rc = get_clover(c, prec, kappa, false, &A, &Ai, s);
+  if (rc) return rc;
+  cudaError_t e = run_clover_apply(prec, r, r, Ai, c->nat, parity, s); c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_apply", e);
+  double n2;
+  if ((rc = norm2(c, prec, r, &n2, s))) return rc;
+  *rsn = sqrt(n2);
+  return LQCD_OK;
+}
+
 }  // namespace
 
 namespace lq {
@@ -132,9 +147,21 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
   if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
   char** lo[] = {&xl, &rl, &rt, &pv, &v, &t};
   for (char** q : lo) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
-  double rn;
-  if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
-  cnt.mat_outer++;
+  const int sym = p.matpc_type == LQCD_MATPC_SYMMETRIC;
+  double rn, rin, istop = stop;       // rin, istop: norm and stopping threshold of the residual the inner iteration sees
+  // true residual in the outer precision; symmetric form: hand A^-1 r to the inner iteration and scale its threshold
+  auto true_residual = [&]() -> int {
+    int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
+    if (rc2) return rc2;
+    cnt.mat_outer++;
+    rin = rn;
+    if (sym && rn > stop) {
+      if ((rc2 = to_symmetric_residual(c, r_hi, par, p.kappa, po, &rin, s))) return rc2;
+      istop = stop * (rin / rn);
+    }
+    return LQCD_OK;
+  };
+  if ((rc = true_residual())) return rc;
   res->iterations = 0; res->restarts = 0;
   const double delta = p.delta > 0 ? p.delta : 0.1;
   int status = LQCD_OK;
@@ -143,7 +170,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
     if ((rc = convert(c, ps, ps, rt, rl, 0, par, s))) return rc;
     for (char* z : {xl, pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
     { BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc; }
-    double maxr = rn;
+    double maxr = rin;
     int it = 0;
     while (true) {
       if (it >= p.max_iter) {
@@ -157,10 +184,10 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
         break;
       }
       { BlasArgs a = mk(c, false, pv, rl, v); if ((rc = blas<OpBicgP>(c, ps, a, s))) return rc; }
-      if ((rc = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      if ((rc = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
       { BlasArgs a = mk(c, false, rt, v); if ((rc = blas<OpBicgAlpha>(c, ps, a, s))) return rc; }
       { BlasArgs a = mk(c, false, rl, v); if ((rc = blas<OpBicgS>(c, ps, a, s))) return rc; }
-      if ((rc = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      if ((rc = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
       { BlasArgs a = mk(c, false, t, rl); if ((rc = blas<OpBicgOmega>(c, ps, a, s))) return rc; }
       { BlasArgs a = mk(c, false, xl, pv, rl, t, rt); if ((rc = blas<OpBicgXR>(c, ps, a, s))) return rc; }
       cnt.mat_sloppy += 2; cnt.blas_flop_sites += 1056; ++it;
@@ -169,15 +196,15 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
       if (!(rr == rr) || flag != 0.0) { status = LQCD_EBREAKDOWN; }
       const double rln = sqrt(rr);
       if (rln > maxr) maxr = rln;
-      if (status == LQCD_EBREAKDOWN || rln <= stop || rln < delta * maxr) {
+      if (status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr) {
         // reliable update: fold x_l into x, recompute the true residual in the outer precision
         MultiArgs m; memset(&m, 0, sizeof(m));
         m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
         cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
         if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
         { BlasArgs a = mk(c, false, xl); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
-        if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
-        cnt.mat_outer++; res->restarts++;
+        if ((rc = true_residual())) return rc;
+        res->restarts++;
         if (rn <= stop) { status = LQCD_OK; break; }
         if (status == LQCD_EBREAKDOWN) {
           // restart the recurrence from the true residual
@@ -191,7 +218,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
           if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
           BlasArgs a = mk(c, false, rt, rl); a.i0 = 1; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
         }
-        maxr = rn;
+        maxr = rin;
       }
     }
     res->iterations = it;
@@ -215,9 +242,20 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
   if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
   char** lo[] = {&xl, &rl, &z, &pv, &w};
   for (char** q : lo) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
-  double rn;
-  if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
-  cnt.mat_outer++;
+  const int sym = p.matpc_type == LQCD_MATPC_SYMMETRIC;
+  double rn, rin, istop = stop;
+  auto true_residual = [&]() -> int {      // as in solve_bicgstab
+    int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
+    if (rc2) return rc2;
+    cnt.mat_outer++;
+    rin = rn;
+    if (sym && rn > stop) {
+      if ((rc2 = to_symmetric_residual(c, r_hi, par, p.kappa, po, &rin, s))) return rc2;
+      istop = stop * (rin / rn);
+    }
+    return LQCD_OK;
+  };
+  if ((rc = true_residual())) return rc;
   res->iterations = 0; res->restarts = 0;
   const double delta = p.delta > 0 ? p.delta : 0.1;
   int status = LQCD_OK;
@@ -232,15 +270,15 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
   if (rn > stop) {
     if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
     for (char* q : {xl, pv}) { BlasArgs a = mk(c, false, q); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
-    if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+    if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
     cnt.mat_sloppy++;
     { BlasArgs a = mk(c, false, z); a.i0 = 0; if ((rc = blas<OpCgInit>(c, ps, a, s))) return rc; }
     { BlasArgs a = mk(c, false, pv, z); if ((rc = blas<OpCgP>(c, ps, a, s))) return rc; }      // beta = 0: p = z
-    double maxr = rn;
+    double maxr = rin;
     int it = 0;
     while (true) {
       if (it >= p.max_iter) { if ((rc = fold())) return rc; status = LQCD_ENOCONV; break; }
-      if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
       { BlasArgs a = mk(c, false, w); if ((rc = blas<OpCgAlpha>(c, ps, a, s))) return rc; }
       { BlasArgs a = mk(c, false, xl, pv, rl, w); if ((rc = blas<OpCgXR>(c, ps, a, s))) return rc; }
       cnt.mat_sloppy++; cnt.blas_flop_sites += 24.0 * (2 + 4 + 2); ++it;
@@ -249,17 +287,17 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
       if (!(rr == rr) || flag != 0.0) status = LQCD_EBREAKDOWN;
       const double rln = sqrt(rr);
       if (rln > maxr) maxr = rln;
-      if (status == LQCD_EBREAKDOWN || rln <= stop || rln < delta * maxr) {
+      if (status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr) {
         if ((rc = fold())) return rc;
-        if ((rc = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s))) return rc;
-        cnt.mat_outer++; res->restarts++;
+        if ((rc = true_residual())) return rc;
+        res->restarts++;
         if (rn <= stop) { status = LQCD_OK; break; }
         if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
         if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
-        maxr = rn;
+        maxr = rin;
       }
       // z = Mhat^dag r ; beta = <z,z>/<z,z>_old ; p = z + beta p   (after a breakdown: restart, beta = 0)
-      if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s))) return rc;
+      if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
       cnt.mat_sloppy++;
       { BlasArgs a = mk(c, false, z); a.i0 = (status == LQCD_EBREAKDOWN) ? 0 : 1; if ((rc = blas<OpCgInit>(c, ps, a, s))) return rc; }
       status = LQCD_OK;
@@ -365,6 +403,8 @@ int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
   if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD && p->solver != LQCD_SOLVER_CGNR) return fail(c, LQCD_EINVAL, "solver");
   if (!(p->tol > 0) || p->max_iter < 1) return fail(c, LQCD_EINVAL, "tol / max_iter");
   if (p->solver == LQCD_SOLVER_GCR_DD && p->precondition && p->mr_steps < 1) return fail(c, LQCD_EINVAL, "mr_steps");
+  if (p->matpc_type != LQCD_MATPC_ASYMMETRIC && p->matpc_type != LQCD_MATPC_SYMMETRIC) return fail(c, LQCD_EINVAL, "matpc_type");
+  if (p->matpc_type == LQCD_MATPC_SYMMETRIC && p->solver == LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "symmetric form: BiCGstab and CGNR only");
   return LQCD_OK;
 }
 

@@ -18,13 +18,14 @@ LIB_PATH = os.environ.get("LQCD_B200_LIB") or os.path.join(_HERE, "liblqcd_b200.
 PREC_DOUBLE, PREC_SINGLE, PREC_HALF = 0, 1, 2
 RECON_18, RECON_12, RECON_8 = 18, 12, 8
 SOLVER_BICGSTAB, SOLVER_GCR_DD, SOLVER_CGNR = 0, 1, 2
+MATPC_ASYMMETRIC, MATPC_SYMMETRIC = 0, 1
 FIELD_SPINOR_PARITY = 0
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_apply_host", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
 ]
 
@@ -37,7 +38,7 @@ class InvertParams(ctypes.Structure):
         ("recon_outer", ctypes.c_int), ("recon_sloppy", ctypes.c_int), ("recon_precond", ctypes.c_int),
         ("parity", ctypes.c_int), ("gcr_kmax", ctypes.c_int), ("schwarz_block", ctypes.c_int * 4),
         ("mr_steps", ctypes.c_int), ("mr_omega", ctypes.c_double),
-        ("use_initial_guess", ctypes.c_int), ("precondition", ctypes.c_int),
+        ("use_initial_guess", ctypes.c_int), ("precondition", ctypes.c_int), ("matpc_type", ctypes.c_int),
     ]
 
 
@@ -82,6 +83,7 @@ def load_library():
             "lqcd_dslash": (i, [vp, vp, vp, i, i, i, i, vp]),
             "lqcd_clover": (i, [vp, vp, vp, i, i, d, i, vp]),
             "lqcd_matpc": (i, [vp, vp, vp, i, i, d, i, i, vp]),
+            "lqcd_matpc_sym": (i, [vp, vp, vp, i, i, d, i, i, vp]),
             "lqcd_dslash_mrhs": (i, [vp, vp, vp, i, i, i, i, i, vp]),
             "lqcd_matpc_mrhs": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_schwarz": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, vp]),
@@ -178,6 +180,10 @@ class Context:
         self._check(self.lib.lqcd_matpc(self.h, _ptr(out), _ptr(inp), parity, int(dagger), kappa, prec, recon, _stream()))
         return out
 
+    def matpc_sym(self, out, inp, parity, dagger, kappa, prec, recon):
+        self._check(self.lib.lqcd_matpc_sym(self.h, _ptr(out), _ptr(inp), parity, int(dagger), kappa, prec, recon, _stream()))
+        return out
+
     def new_fields(self, prec, nrhs):
         """nrhs packed fields back to back (the layout of the *_mrhs calls); row r is field r."""
         return torch.empty((nrhs, self.field_bytes(prec)), dtype=torch.uint8, device=self.device)
@@ -210,7 +216,8 @@ class Context:
     @staticmethod
     def make_params(kappa, c_sw, tol, solver=SOLVER_BICGSTAB, prec=(PREC_DOUBLE, PREC_SINGLE, PREC_HALF),
                     recon=(RECON_18, RECON_12, RECON_12), delta=0.1, max_iter=5000, parity=0, gcr_kmax=16,
-                    schwarz_block=(0, 0, 0, 0), mr_steps=10, mr_omega=1.0, use_initial_guess=False, precondition=True):
+                    schwarz_block=(0, 0, 0, 0), mr_steps=10, mr_omega=1.0, use_initial_guess=False, precondition=True,
+                    matpc_type=MATPC_ASYMMETRIC):
         p = InvertParams()
         p.kappa, p.c_sw, p.tol, p.delta = kappa, c_sw, tol, delta
         p.max_iter, p.solver = max_iter, solver
@@ -221,6 +228,7 @@ class Context:
             p.schwarz_block[k] = int(schwarz_block[k])
         p.mr_steps, p.mr_omega = mr_steps, mr_omega
         p.use_initial_guess, p.precondition = int(use_initial_guess), int(precondition)
+        p.matpc_type = int(matpc_type)
         return p
 
     def invert(self, x, b, params, allow_fail=False):

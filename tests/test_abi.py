@@ -38,12 +38,30 @@ def test_binding_lists_the_same_symbols():
     assert sorted(lqcd.EXPORTS) == _declared()
 
 
-def test_struct_layouts_match_header():
+def test_struct_layouts_match_header(tmp_path):
+    """sizeof / offsetof of the two ABI structs as a C compiler sees include/lqcd.h (gcc, no CUDA needed)
+    against the ctypes mirrors in the binding."""
+    import subprocess
     from paper_1109_2935_b200 import lqcd
-    # lqcd_invert_params: 4 doubles, 10 ints, int[4], int, double, 2 ints  (natural alignment)
-    assert ctypes.sizeof(lqcd.InvertParams) == 4 * 8 + 10 * 4 + 16 + 4 + 4 + 8 + 8
-    assert ctypes.sizeof(lqcd.InvertResult) == 6 * 4 + 4 * 8
-    assert lqcd.InvertParams.mr_omega.offset % 8 == 0
+    src = tmp_path / "layout.c"
+    src.write_text('''#include <stdio.h>
+#include <stddef.h>
+#include "lqcd.h"
+int main(void) {
+  printf("%zu %zu %zu %zu %zu %zu %zu\\n", sizeof(lqcd_invert_params), sizeof(lqcd_invert_result),
+         offsetof(lqcd_invert_params, schwarz_block), offsetof(lqcd_invert_params, mr_omega),
+         offsetof(lqcd_invert_params, matpc_type), offsetof(lqcd_invert_result, true_residual),
+         offsetof(lqcd_invert_result, gflop));
+  return 0;
+}
+''')
+    exe = tmp_path / "layout"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)])
+    got = [int(t) for t in subprocess.check_output([str(exe)], text=True).split()]
+    want = [ctypes.sizeof(lqcd.InvertParams), ctypes.sizeof(lqcd.InvertResult), lqcd.InvertParams.schwarz_block.offset,
+            lqcd.InvertParams.mr_omega.offset, lqcd.InvertParams.matpc_type.offset, lqcd.InvertResult.true_residual.offset,
+            lqcd.InvertResult.gflop.offset]
+    assert got == want
 
 
 def test_create_without_gpu_fails_loudly(lib):

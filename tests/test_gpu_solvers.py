@@ -218,3 +218,35 @@ def test_cgnr(mid, prec):
     pb = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB, prec=prec, recon=(18, 12, 12))
     xb, ib = _solve(c, b, pb)
     assert ib["matpc_sloppy"] < info["matpc_sloppy"]
+
+
+def test_symmetric_even_odd_form(mid):
+    """LQCD_MATPC_SYMMETRIC: lqcd_matpc_sym against the oracle's Mhat_s (and its adjoint) in every precision;
+    BiCGstab and CGNR through the symmetric system reach the same unique solution with the FULL-system
+    criterion ||b - M x|| <= tol ||b|| (oracle's operator); GCR-DD refuses it."""
+    c = mid
+    lq = c.lqcd
+    kappa = 0.124
+    psi = inputs.gaussian_spinor(c.dims, 3)
+    for prec, tol in ((0, 1e-13), (1, 1e-5), (2, 5e-3)):
+        for parity in (0, 1):
+            for dagger in (False, True):
+                want = oracle.matpc_sym(psi, c.U, c.T, c.bc, kappa, parity, dagger=dagger)
+                got = c.gpu_parity_op(lambda o, i: c.ctx.matpc_sym(o, i, parity, dagger, kappa, prec, 12), psi, parity, parity, prec)
+                assert _rel(got, want) <= tol, (prec, parity, dagger)
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    for solver in (lq.SOLVER_BICGSTAB, lq.SOLVER_CGNR):
+        for prec in ((0, 0, 0), (0, 1, 1), (0, 2, 2)):
+            p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=solver, prec=prec, recon=(18, 12, 12), matpc_type=lq.MATPC_SYMMETRIC)
+            x, info = _solve(c, b, p)
+            assert info["status"] == 0 and info["true_residual"] <= 1e-10
+            res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+            assert res <= 1.05e-10, (solver, prec, res)
+            assert _rel(x, xo) <= 1e-8
+    xs, isym = oracle.invert_sym(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-10)
+    assert _rel(xs, xo) <= 1e-8
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, schwarz_block=(4, 4, 4, 8), matpc_type=lq.MATPC_SYMMETRIC)
+    with pytest.raises(lq.LqcdError) as e:
+        _solve(c, b, p)
+    assert e.value.code == lq.EINVAL
