@@ -178,6 +178,16 @@ typedef struct {
 int lqcd_invert(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical,
                 const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
 
+/* Batched solve of M x_r = b_r for nrhs (1..LQCD_MAX_RHS) sources sharing the gauge field: nrhs mixed-
+ * precision BiCGstab recurrences in lockstep on the multi-right-hand-side operators (SURVEY.md 8(f)
+ * NEXT-4; not in the paper).  x_canonical / b_canonical: nrhs canonical full-lattice DEVICE arrays back
+ * to back; result[r] describes source r (seconds and gflop are those of the whole batch).  Every
+ * source is iterated to its own ||b_r - M x_r|| <= tol ||b_r||.  params: solver must be
+ * LQCD_SOLVER_BICGSTAB, matpc_type LQCD_MATPC_ASYMMETRIC.  Returns LQCD_OK, or LQCD_ENOCONV /
+ * LQCD_EBREAKDOWN if at least one source ended that way (see result[r].status).  Synchronises `stream`. */
+int lqcd_invert_mrhs(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical, int nrhs,
+                     const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
+
 /* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */
 /* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned for full PCIe speed;
  * pageable works), owned by the caller, not overlapping.

@@ -265,11 +265,12 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   cudaGetDeviceProperties(&prop, device);
   c->n_sm = prop.multiProcessorCount;
   c->partials_doubles = (size_t)c->n_sm * 8 * 16 + 4096;
-  bool ok = cudaMalloc((void**)&c->S, S_TOTAL * sizeof(double)) == cudaSuccess &&
-            cudaMalloc((void**)&c->partials, c->partials_doubles * sizeof(double)) == cudaSuccess &&
+  // scalars / partials for LQCD_MAX_RHS right-hand sides (batched solves; a single solve uses set 0)
+  bool ok = cudaMalloc((void**)&c->S, (size_t)LQCD_MAX_RHS * S_TOTAL * sizeof(double)) == cudaSuccess &&
+            cudaMalloc((void**)&c->partials, (size_t)LQCD_MAX_RHS * c->partials_doubles * sizeof(double)) == cudaSuccess &&
             cudaMalloc((void**)&c->counters, 4096 * sizeof(unsigned)) == cudaSuccess &&
-            cudaMallocHost((void**)&c->hS, S_TOTAL * sizeof(double)) == cudaSuccess;
-  if (ok) ok = cudaMemset(c->S, 0, S_TOTAL * sizeof(double)) == cudaSuccess &&
+            cudaMallocHost((void**)&c->hS, (size_t)(S_TOTAL + 4 * LQCD_MAX_RHS) * sizeof(double)) == cudaSuccess;
+  if (ok) ok = cudaMemset(c->S, 0, (size_t)LQCD_MAX_RHS * S_TOTAL * sizeof(double)) == cudaSuccess &&
                cudaMemset(c->counters, 0, 4096 * sizeof(unsigned)) == cudaSuccess;
   if (!ok) { lqcd_destroy(c); return LQCD_ENOMEM; }
   *out = c;

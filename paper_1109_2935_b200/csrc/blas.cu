@@ -7,11 +7,12 @@
 namespace lq {
 
 template <class Op>
-cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s) {
+cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s, int nrhs) {
   int gx = (a.vh + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK;
   if (gx > max_ctas) gx = max_ctas;
   if (gx < 1) gx = 1;
-  dim3 grid(gx, a.nb), block(LQ_BLAS_BLOCK);
+  if (nrhs > 1 && (a.nb != 1 || !a.rhs_bytes)) return cudaErrorInvalidValue;
+  dim3 grid(gx, a.nb, nrhs), block(LQ_BLAS_BLOCK);
   switch (prec) {
     case 0: blas_kernel<PrecD, Op><<<grid, block, 0, s>>>(a); break;
     case 1: blas_kernel<PrecS, Op><<<grid, block, 0, s>>>(a); break;
@@ -21,7 +22,7 @@ cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s) 
   return cudaGetLastError();
 }
 
-#define LQ_INST(OP) template cudaError_t run_blas<OP>(int, const BlasArgs&, int, cudaStream_t);
+#define LQ_INST(OP) template cudaError_t run_blas<OP>(int, const BlasArgs&, int, cudaStream_t, int);
 LQ_INST(OpZero) LQ_INST(OpNorm2) LQ_INST(OpCdot) LQ_INST(OpAxpyNorm) LQ_INST(OpXmyNorm)
 LQ_INST(OpBicgInit) LQ_INST(OpBicgP) LQ_INST(OpBicgAlpha) LQ_INST(OpBicgS) LQ_INST(OpBicgOmega) LQ_INST(OpBicgXR)
 LQ_INST(OpGcrScale)

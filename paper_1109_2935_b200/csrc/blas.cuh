@@ -20,6 +20,7 @@ namespace lq {
 enum {
   S_RHO = 0, S_RHO_OLD = 2, S_ALPHA = 4, S_OMEGA = 6, S_BETA = 8, S_RR = 10, S_FLAG = 11,
   S_RTV = 12, S_TS = 14, S_TT = 16, S_OUT = 20 /* generic results: 20..27 */,
+  S_DONE = 28,    // batched solves: nonzero = this right-hand side has converged, its passes are skipped
   S_GCR_GAMMA = 32, S_GCR_ALPHA = 34, S_GCR_ZZ = 36,
   S_GCR_BETA = 64,                         // beta[i][k] complex: S_GCR_BETA + 2*(i*LQ_GCR_KMAX + k)
   S_GCR_GAMMAS = S_GCR_BETA + 2 * LQ_GCR_KMAX * LQ_GCR_KMAX,   // gamma[k]
@@ -38,6 +39,10 @@ struct BlasArgs {
   int nchunk;
   double c[4];            // host coefficients
   int i0, i1;
+  // batched launch over right-hand sides (gridDim.z = nrhs, nb must be 1): right-hand side r uses
+  // v[j] + r * rhs_bytes, S + r * S_TOTAL, partials + r * rhs_partials, counters + r
+  long long rhs_bytes;
+  long long rhs_partials;
 };
 
 struct cd { double re, im; };
@@ -111,9 +116,19 @@ LQ_DEV void reduce_and_finalize(double* red, const BlasArgs& a, int box, F fin) 
 //   struct Coef; prepare(Coef&, const BlasArgs&, int box);
 //   site<R>(const Coef&, R* v0..v4, double* red);  finalize(const double* sum, const BlasArgs&, int box)
 template <class P, class Op>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK) blas_kernel(const BlasArgs a) {
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) blas_kernel(const BlasArgs a0) {
   typedef typename P::real R;
   const int box = blockIdx.y;
+  BlasArgs a = a0;
+  if (a0.rhs_bytes) {                       // one right-hand side per blockIdx.z, each with its own scalars
+    const int r = blockIdx.z;
+    a.S = a0.S + (long long)r * S_TOTAL;
+    if (a.S[S_DONE] != 0.0) return;         // converged: leave its vectors alone
+#pragma unroll
+    for (int j = 0; j < LQ_MAX_VEC; ++j) a.v[j] = a0.v[j] ? a0.v[j] + (long long)r * a0.rhs_bytes : nullptr;
+    a.partials = a0.partials + (long long)r * a0.rhs_partials;
+    a.counters = a0.counters + r;
+  }
   typename Op::Coef coef;
   Op::prepare(coef, a, box);
   constexpr int NV = Op::NV > 0 ? Op::NV : 1;
@@ -136,6 +151,6 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) blas_kernel(const BlasArgs a) {
   }
 }
 
-template <class Op> cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s);
+template <class Op> cudaError_t run_blas(int prec, const BlasArgs& a, int max_ctas, cudaStream_t s, int nrhs = 1);
 
 }  // namespace lq

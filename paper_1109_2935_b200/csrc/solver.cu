@@ -393,6 +393,166 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
   return status;
 }
 
+// ---------------------------------------------------------------- batched BiCGstab (several right-hand sides)
+// nrhs independent BiCGstab recurrences advanced in lockstep: the operator is applied to all of them
+// with the multi-right-hand-side kernels (one link load per 4 sources, dslash_mrhs.cuh), the five
+// fused BLAS-1 passes of an iteration run as one launch each over gridDim.z = nrhs with one set of
+// device scalars per source.  A reliable update (R11) is taken for all sources as soon as one asks for
+// it; a converged source is frozen (S_DONE) and its passes return at once.  x, b: nrhs packed fields.
+BlasArgs mkb(lqcd_ctx* c, int prec, char* v0 = nullptr, char* v1 = nullptr, char* v2 = nullptr, char* v3 = nullptr, char* v4 = nullptr) {
+  BlasArgs a = mk(c, false, v0, v1, v2, v3, v4);
+  a.rhs_bytes = (long long)spinor_bytes(prec, c->nat.ns);
+  a.rhs_partials = (long long)c->partials_doubles;
+  return a;
+}
+BlasArgs mkr(lqcd_ctx* c, int r, char* v0 = nullptr, char* v1 = nullptr, char* v2 = nullptr, char* v3 = nullptr, char* v4 = nullptr) {
+  BlasArgs a = mk(c, false, v0, v1, v2, v3, v4);           // single launch on the scalar set of source r
+  a.S = c->S + (long long)r * S_TOTAL;
+  a.partials = c->partials + (long long)r * c->partials_doubles;
+  a.counters = c->counters + r;
+  return a;
+}
+template <class Op>
+int blasb(lqcd_ctx* c, int prec, const BlasArgs& a, int nrhs, cudaStream_t s) {
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s, nrhs);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "batched blas launch", e);
+}
+// hS[S_TOTAL + 2r .. +1] = S_r[off], S_r[off+1] for all sources (one strided copy), synchronises
+int read_S_all(lqcd_ctx* c, int off, int nrhs, cudaStream_t s) {
+  cudaError_t e = cudaMemcpy2DAsync(c->hS + S_TOTAL, 2 * sizeof(double), c->S + off, S_TOTAL * sizeof(double),
+                                    2 * sizeof(double), nrhs, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "scalar read-back", e);
+}
+int set_done(lqcd_ctx* c, int r, double v, cudaStream_t s) {
+  double* h = c->hS + S_TOTAL + 2 * LQCD_MAX_RHS + r;       // pinned staging word of source r
+  *h = v;
+  cudaError_t e = cudaMemcpyAsync(c->S + (long long)r * S_TOTAL + S_DONE, h, sizeof(double), cudaMemcpyHostToDevice, s);
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "flag write", e);
+}
+
+// r_hi = b - Mhat x for all sources (outer precision); rn[r] = ||r_hi[r]||
+int residual_mrhs(lqcd_ctx* c, char* r_hi, const char* b, const char* x, int nrhs, int par, double kappa, int prec, int recon,
+                  double* rn, cudaStream_t s) {
+  int rc = op_matpc_mrhs(c, r_hi, x, nrhs, par, 0, kappa, prec, recon, s);
+  if (rc) return rc;
+  const size_t fb = spinor_bytes(prec, c->nat.ns);
+  for (int r = 0; r < nrhs; ++r) {
+    BlasArgs a = mkr(c, r, const_cast<char*>(b) + r * fb, r_hi + r * fb);
+    if ((rc = blas<OpXmyNorm>(c, prec, a, s))) return rc;
+  }
+  if ((rc = read_S_all(c, S_OUT, nrhs, s))) return rc;
+  for (int r = 0; r < nrhs; ++r) rn[r] = sqrt(c->hS[S_TOTAL + 2 * r]);
+  return LQCD_OK;
+}
+
+int solve_bicgstab_mrhs(lqcd_ctx* c, char* x, const char* b, int nrhs, const lqcd_invert_params& p, const double* stop,
+                        lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
+  const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
+  const long long ns = c->nat.ns;
+  const size_t fo = spinor_bytes(po, ns), fs = spinor_bytes(ps, ns);
+  Work wk(c);
+  char *r_hi, *xl, *rl, *rt, *pv, *v, *t;
+  int rc;
+  if ((rc = wk.get(&r_hi, fo * nrhs))) return rc;
+  char** lo[] = {&xl, &rl, &rt, &pv, &v, &t};
+  for (char** q : lo) if ((rc = wk.get(q, fs * nrhs))) return rc;
+  std::vector<double> rn(nrhs), maxr(nrhs);
+  std::vector<int> done(nrhs, 0), status(nrhs, LQCD_OK), waiting(nrhs, 0);
+  for (int r = 0; r < nrhs; ++r) if ((rc = set_done(c, r, 0.0, s))) return rc;
+  if ((rc = residual_mrhs(c, r_hi, b, x, nrhs, par, p.kappa, po, p.recon_outer, rn.data(), s))) return rc;
+  cnt.mat_outer += nrhs;
+  const double delta = p.delta > 0 ? p.delta : 0.1;
+  auto restart = [&](int r, int keep) -> int {    // r_l = lo(r_hi); keep = 0: fresh recurrence, 1: after a reliable update
+    int rc2 = convert(c, po, ps, rl + r * fs, r_hi + r * fo, 0, par, s);
+    if (rc2) return rc2;
+    if (!keep) {
+      if ((rc2 = convert(c, ps, ps, rt + r * fs, rl + r * fs, 0, par, s))) return rc2;
+      for (char* z : {pv + r * fs, v + r * fs}) { BlasArgs a = mkr(c, r, z); if ((rc2 = blas<OpZero>(c, ps, a, s))) return rc2; }
+    }
+    BlasArgs a = mkr(c, r, rt + r * fs, rl + r * fs); a.i0 = keep;
+    return blas<OpBicgInit>(c, ps, a, s);
+  };
+  int ndone = 0;
+  for (int r = 0; r < nrhs; ++r) {
+    res[r].iterations = 0; res[r].restarts = 0;
+    maxr[r] = rn[r];
+    { BlasArgs a = mkr(c, r, xl + r * fs); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+    if (rn[r] <= stop[r] || !(rn[r] == rn[r])) {
+      done[r] = 1; ++ndone; status[r] = (rn[r] == rn[r]) ? LQCD_OK : LQCD_EBREAKDOWN;
+      if ((rc = set_done(c, r, 1.0, s))) return rc;
+      for (char* z : {rl + r * fs, rt + r * fs, pv + r * fs, v + r * fs, t + r * fs}) { BlasArgs a = mkr(c, r, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+    } else if ((rc = restart(r, 0))) return rc;
+  }
+  int it = 0;
+  while (ndone < nrhs) {
+    const bool capped = it >= p.max_iter;
+    bool update = capped;
+    int nwant = 0;
+    if (!capped) {
+      { BlasArgs a = mkb(c, ps, pv, rl, v); if ((rc = blasb<OpBicgP>(c, ps, a, nrhs, s))) return rc; }
+      if ((rc = op_matpc_mrhs(c, v, pv, nrhs, par, 0, p.kappa, ps, p.recon_sloppy, s))) return rc;
+      { BlasArgs a = mkb(c, ps, rt, v); if ((rc = blasb<OpBicgAlpha>(c, ps, a, nrhs, s))) return rc; }
+      { BlasArgs a = mkb(c, ps, rl, v); if ((rc = blasb<OpBicgS>(c, ps, a, nrhs, s))) return rc; }
+      if ((rc = op_matpc_mrhs(c, t, rl, nrhs, par, 0, p.kappa, ps, p.recon_sloppy, s))) return rc;
+      { BlasArgs a = mkb(c, ps, t, rl); if ((rc = blasb<OpBicgOmega>(c, ps, a, nrhs, s))) return rc; }
+      { BlasArgs a = mkb(c, ps, xl, pv, rl, t, rt); if ((rc = blasb<OpBicgXR>(c, ps, a, nrhs, s))) return rc; }
+      ++it;
+      cnt.mat_sloppy += 2 * (nrhs - ndone); cnt.blas_flop_sites += 1056.0 * (nrhs - ndone);
+      if ((rc = read_S_all(c, S_RR, nrhs, s))) return rc;
+      for (int r = 0; r < nrhs; ++r) {
+        if (done[r]) continue;
+        res[r].iterations = it;
+        const double rr = c->hS[S_TOTAL + 2 * r], flag = c->hS[S_TOTAL + 2 * r + 1];
+        if (!(rr == rr) || flag != 0.0) status[r] = LQCD_EBREAKDOWN;
+        const double rln = sqrt(rr);
+        if (rln > maxr[r]) maxr[r] = rln;
+        const bool want = rln <= stop[r] || rln < delta * maxr[r];
+        waiting[r] = want ? waiting[r] + 1 : 0;
+        if (want) ++nwant;
+        if (status[r] == LQCD_EBREAKDOWN || waiting[r] > 4) update = true;
+      }
+      // the update costs one outer-precision Mhat for every source, so it is shared: taken when all
+      // unfinished sources ask for it, or one has been asking for more than 4 iterations, or broke down
+      if (nwant == nrhs - ndone) update = true;
+    }
+    if (!update) continue;
+    // reliable update of every unfinished source: x += x_l, true residual in the outer precision
+    for (int r = 0; r < nrhs; ++r) {
+      if (done[r]) continue;
+      MultiArgs m; memset(&m, 0, sizeof(m));
+      m.b = mk(c, false); m.z[0] = xl + r * fs; m.chi[0] = 1.0; m.n = 1;
+      cudaError_t e = run_accumulate(po, ps, x + r * fo, m, s); c->launches++;
+      if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+      BlasArgs a = mkr(c, r, xl + r * fs); if ((rc = blas<OpZero>(c, ps, a, s))) return rc;
+    }
+    if ((rc = residual_mrhs(c, r_hi, b, x, nrhs, par, p.kappa, po, p.recon_outer, rn.data(), s))) return rc;
+    cnt.mat_outer += nrhs;
+    for (int r = 0; r < nrhs; ++r) {
+      if (done[r]) continue;
+      res[r].restarts++;
+      const bool nan = !(rn[r] == rn[r]);
+      if (rn[r] <= stop[r] || nan || capped) {
+        done[r] = 1; ++ndone;
+        status[r] = nan ? LQCD_EBREAKDOWN : (rn[r] <= stop[r] ? LQCD_OK : LQCD_ENOCONV);
+        if ((rc = set_done(c, r, 1.0, s))) return rc;
+      } else {
+        if ((rc = restart(r, status[r] == LQCD_EBREAKDOWN ? 0 : 1))) return rc;
+        status[r] = LQCD_OK;
+        maxr[r] = rn[r];
+        waiting[r] = 0;
+      }
+    }
+  }
+  for (int r = 0; r < nrhs; ++r) {
+    res[r].status = status[r];
+    res[r].iterated_residual = rn[r];
+    if ((rc = set_done(c, r, 0.0, s))) return rc;           // leave the scalar sets clean for the next call
+  }
+  return LQCD_OK;
+}
+
 int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
   if (!p) return fail(c, LQCD_EINVAL, "null params");
   if (!c->have_gauge || !c->have_clover) return fail(c, LQCD_ESTATE, "invert before load_gauge / build_clover");
@@ -506,6 +666,88 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   res->gflop = ((double)(cnt.mat_sloppy + cnt.mat_outer + cnt.mat_precond) * 3696.0 + cnt.blas_flop_sites) * (double)c->Vh * 1e-9;
   if (status == LQCD_ENOCONV) return fail(c, status, "max_iter reached");
   if (status == LQCD_EBREAKDOWN) return fail(c, status, "solver breakdown");
+  return LQCD_OK;
+}
+
+int lqcd_invert_mrhs(lqcd_ctx* c, void* x_can, const void* b_can, int nrhs, const lqcd_invert_params* p, lqcd_invert_result* res,
+                     void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!x_can || !b_can || !res || nrhs < 1 || nrhs > LQCD_MAX_RHS) return fail(c, LQCD_EINVAL, "invert_mrhs arguments");
+  int rc = check_params(c, p);
+  if (rc) return rc;
+  if (p->solver != LQCD_SOLVER_BICGSTAB || p->matpc_type != LQCD_MATPC_ASYMMETRIC)
+    return fail(c, LQCD_EINVAL, "invert_mrhs: BiCGstab on the asymmetric Schur system only");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  memset(res, 0, sizeof(*res) * nrhs);
+  const int po = p->prec_outer, par = p->parity;
+  const long long ns = c->nat.ns;
+  const size_t fo = spinor_bytes(po, ns), cb = (size_t)c->V * 24 * sizeof(double);
+  Work wk(c);
+  char *bp, *bq, *xp, *bhat, *t1;
+  for (char** q : {&bp, &bq, &xp, &bhat, &t1}) if ((rc = wk.get(q, fo * nrhs))) return rc;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  cudaEventRecord(e0, s);
+  struct Ev { cudaEvent_t a, b; ~Ev() { cudaEventDestroy(a); cudaEventDestroy(b); } } ev{e0, e1};
+  Counts cnt;
+  const char *A, *Ai;
+  if ((rc = get_clover(c, po, p->kappa, false, &A, &Ai, s))) return rc;
+  cudaError_t e = cudaSuccess;
+  for (int r = 0; r < nrhs && e == cudaSuccess; ++r) {
+    const double* bc = (const double*)((const char*)b_can + r * cb);
+    e = run_pack_spinor(po, bp + r * fo, bc, c->nat, par, 0, s); c->launches++;
+    if (e == cudaSuccess) { e = run_pack_spinor(po, bq + r * fo, bc, c->nat, 1 - par, 0, s); c->launches++; }
+    if (e == cudaSuccess) { e = run_clover_apply(po, t1 + r * fo, bq + r * fo, Ai, c->nat, 1 - par, s); c->launches++; }
+    if (e == cudaSuccess) {
+      if (p->use_initial_guess) { e = run_pack_spinor(po, xp + r * fo, (const double*)((const char*)x_can + r * cb), c->nat, par, 0, s); c->launches++; }
+      else { BlasArgs a = mk(c, false, xp + r * fo); if ((rc = blas<OpZero>(c, po, a, s))) return rc; }
+    }
+  }
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack / clover", e);
+  // ||b_r||: two norms per source on its own scalar set
+  std::vector<double> bnorm(nrhs), stop(nrhs);
+  for (int r = 0; r < nrhs; ++r) {
+    BlasArgs a = mkr(c, r, bp + r * fo); a.i0 = 0; if ((rc = blas<OpNorm2>(c, po, a, s))) return rc;
+    BlasArgs a2 = mkr(c, r, bq + r * fo); a2.i0 = 1; if ((rc = blas<OpNorm2>(c, po, a2, s))) return rc;
+  }
+  if ((rc = read_S_all(c, S_OUT, nrhs, s))) return rc;
+  for (int r = 0; r < nrhs; ++r) {
+    bnorm[r] = sqrt(c->hS[S_TOTAL + 2 * r] + c->hS[S_TOTAL + 2 * r + 1]);
+    stop[r] = p->tol * bnorm[r];                           // a zero source is "converged" at once with x = 0
+  }
+  // source preparation for all sources: bhat_p = b_p + kappa D A^-1 b_pbar   (R6)
+  if ((rc = op_dslash_mrhs(c, bhat, t1, bp, nrhs, par, 0, po, p->recon_outer, EPI_XPAY, p->kappa, p->kappa, s))) return rc;
+  rc = solve_bicgstab_mrhs(c, xp, bhat, nrhs, *p, stop.data(), res, cnt, s);
+  if (rc) return rc;
+  // true residuals, reconstruction x_pbar = A^-1 (b_pbar + kappa D x_p), unpack
+  std::vector<double> rn(nrhs);
+  if ((rc = residual_mrhs(c, t1, bhat, xp, nrhs, par, p->kappa, po, p->recon_outer, rn.data(), s))) return rc;
+  cnt.mat_outer += nrhs;
+  if ((rc = op_dslash_mrhs(c, t1, xp, bq, nrhs, 1 - par, 0, po, p->recon_outer, EPI_XPAY_CLOVOUT, p->kappa, p->kappa, s))) return rc;
+  for (int r = 0; r < nrhs && e == cudaSuccess; ++r) {
+    double* xc = (double*)((char*)x_can + r * cb);
+    e = run_pack_spinor(po, xp + r * fo, xc, c->nat, par, 1, s); c->launches++;
+    if (e == cudaSuccess) { e = run_pack_spinor(po, t1 + r * fo, xc, c->nat, 1 - par, 1, s); c->launches++; }
+  }
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "unpack", e);
+  cudaEventRecord(e1, s);
+  e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "invert_mrhs", e);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  int worst = LQCD_OK;
+  const double gflop = ((double)(cnt.mat_sloppy + cnt.mat_outer) * 3696.0 + cnt.blas_flop_sites) * (double)c->Vh * 1e-9;
+  for (int r = 0; r < nrhs; ++r) {
+    res[r].true_residual = bnorm[r] > 0 ? rn[r] / bnorm[r] : 0.0;
+    res[r].iterated_residual = bnorm[r] > 0 ? res[r].iterated_residual / bnorm[r] : 0.0;
+    res[r].seconds = ms * 1e-3;                            // the whole batch
+    res[r].gflop = gflop;                                  // the whole batch
+    res[r].matpc_sloppy = 2 * res[r].iterations; res[r].matpc_outer = res[r].restarts + 2;
+    if (res[r].status != LQCD_OK && worst == LQCD_OK) worst = res[r].status;
+  }
+  if (worst == LQCD_ENOCONV) return fail(c, worst, "max_iter reached for at least one right-hand side");
+  if (worst == LQCD_EBREAKDOWN) return fail(c, worst, "solver breakdown for at least one right-hand side");
   return LQCD_OK;
 }
 

@@ -25,7 +25,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_apply_host", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
 ]
 
@@ -88,6 +88,7 @@ def load_library():
             "lqcd_matpc_mrhs": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_schwarz": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, vp]),
             "lqcd_invert": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
+            "lqcd_invert_mrhs": (i, [vp, vp, vp, i, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_apply_host": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_invert_host": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_axpy_norm": (i, [vp, d, vp, vp, i, ctypes.POINTER(d), vp]),
@@ -238,6 +239,15 @@ class Context:
         rc = self.lib.lqcd_invert(self.h, _ptr(x), _ptr(b), ctypes.byref(params), ctypes.byref(r), _stream())
         self._check(rc, allow=(ENOCONV, EBREAKDOWN) if allow_fail else ())
         return r.as_dict()
+
+    def invert_mrhs(self, x, b, params, allow_fail=False):
+        """x, b: [nrhs, T, Z, Y, X, 4, 3] complex128 device tensors.  Returns one result dict per source."""
+        assert x.is_cuda and b.is_cuda and x.dtype == b.dtype == torch.complex128 and x.is_contiguous() and b.is_contiguous()
+        nrhs = b.shape[0]
+        r = (InvertResult * nrhs)()
+        rc = self.lib.lqcd_invert_mrhs(self.h, _ptr(x), _ptr(b), nrhs, ctypes.byref(params), r, _stream())
+        self._check(rc, allow=(ENOCONV, EBREAKDOWN) if allow_fail else ())
+        return [r[k].as_dict() for k in range(nrhs)]
 
     def apply_host(self, out_host, in_host, op, parity, dagger, kappa, prec, recon):
         """out_host, in_host: canonical complex128 HOST tensors (pinned for full-speed copies)."""

@@ -69,3 +69,50 @@ def test_mrhs_argument_errors(ragged):
     with pytest.raises(lq.LqcdError) as e:
         c.ctx.matpc_mrhs(f, f, 2, 0, False, 0.12, 1, 12)            # aliasing
     assert e.value.code == lq.EINVAL
+
+
+@pytest.mark.parametrize("sloppy", [0, 1, 2])
+def test_invert_mrhs(sloppy):
+    """lqcd_invert_mrhs: 5 sources (one zero, one 100x larger, one a point source) solved in lockstep;
+    every source meets its own full-system criterion by the ORACLE's operator and equals the
+    single-source lqcd_invert solution."""
+    c = Case((8, 8, 8, 16), 0.2)
+    lq = c.lqcd
+    kappa, nrhs = 0.124, 5
+    srcs = [inputs.gaussian_spinor(c.dims, 200 + r) for r in range(nrhs)]
+    srcs[1] = np.zeros_like(srcs[1])
+    srcs[2] = 100.0 * srcs[2]
+    srcs[3] = np.zeros_like(srcs[3])
+    srcs[3][5, 2, 1, 1, 2, 1] = 1.0 - 0.5j
+    b = torch.from_numpy(np.stack(srcs)).cuda()
+    x = torch.zeros_like(b)
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB, prec=(0, sloppy, sloppy), recon=(18, 12, 12))
+    infos = c.ctx.invert_mrhs(x, b, p)
+    xs = x.cpu().numpy()
+    for r in range(nrhs):
+        assert infos[r]["status"] == 0, r
+        if r == 1:
+            assert np.max(np.abs(xs[r])) == 0.0 and infos[r]["iterations"] == 0
+            continue
+        res = np.linalg.norm(srcs[r] - oracle.M(xs[r], c.U, c.T, c.bc, kappa)) / np.linalg.norm(srcs[r])
+        assert res <= 1.05e-10, (r, res)
+        assert abs(res - infos[r]["true_residual"]) <= 0.05 * res + 1e-14
+        x1 = torch.zeros_like(b[r])
+        c.ctx.invert(x1, b[r].contiguous(), p)
+        assert _rel(xs[r], x1.cpu().numpy()) <= 1e-8, r
+    # iteration cap: every unfinished source reports LQCD_ENOCONV with its true residual
+    p2 = c.ctx.make_params(kappa, 1.0, 1e-12, solver=lq.SOLVER_BICGSTAB, prec=(0, sloppy, sloppy), recon=(18, 12, 12), max_iter=3)
+    x.zero_()
+    infos = c.ctx.invert_mrhs(x, b, p2, allow_fail=True)
+    assert [i["status"] for i in infos] == [lq.ENOCONV, 0, lq.ENOCONV, lq.ENOCONV, lq.ENOCONV]
+    xs = x.cpu().numpy()
+    for r in (0, 2, 3, 4):
+        res = np.linalg.norm(srcs[r] - oracle.M(xs[r], c.U, c.T, c.bc, kappa)) / np.linalg.norm(srcs[r])
+        assert infos[r]["iterations"] == 3 and 1e-12 < res < 1.0 and abs(res - infos[r]["true_residual"]) <= 1e-6 * res
+    # the single-source solver still works on scalar set 0 afterwards, GCR-DD is refused in batched mode
+    x1 = torch.zeros_like(b[0])
+    assert c.ctx.invert(x1, b[0].contiguous(), p)["true_residual"] <= 1e-10
+    with pytest.raises(lq.LqcdError) as e:
+        c.ctx.invert_mrhs(x, b, c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, schwarz_block=(4, 4, 4, 8)))
+    assert e.value.code == lq.EINVAL
+    c.ctx.close()
