@@ -20,7 +20,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "wilson_clover_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_SRC_S = os.path.join(_HERE, "staggered_oracle.cpp")
+_LIB_S = os.path.join(_HERE, "liboracle_staggered.so")
 _lib = None
+_lib_s = None
 
 BICGSTAB, GCR_DD, CGNR = 0, 1, 2
 
@@ -30,7 +33,20 @@ def build(force=False):
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(
             ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC])
+    if force or not os.path.exists(_LIB_S) or os.path.getmtime(_LIB_S) < os.path.getmtime(_SRC_S):
+        subprocess.check_call(
+            ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", _LIB_S, _SRC_S])
     return _LIB
+
+
+def lib_s():
+    """The improved staggered oracle (staggered_oracle.cpp)."""
+    global _lib_s
+    if _lib_s is None:
+        build()
+        _lib_s = ctypes.CDLL(_LIB_S)
+        _lib_s.ors_cg.restype = ctypes.c_int
+    return _lib_s
 
 
 def lib():
@@ -195,3 +211,41 @@ def invert(b, U, Tcl, bc, kappa, parity=0, tol=1e-12, maxit=10000, solver=BICGST
                           ctypes.c_int(kmax), ctypes.c_double(delta), _blk(block), ctypes.c_int(n_mr),
                           ctypes.c_double(omega_mr), ctypes.byref(it), ctypes.byref(tr))
     return x, dict(status=st, iterations=it.value, true_residual=tr.value)
+
+
+# ---------------------------------------------------------------- improved staggered (staggered_oracle.cpp)
+def _sdims(chi):
+    T, Z, Y, X = chi.shape[:4]
+    return (X, Y, Z, T)
+
+
+def stag_dslash(chi, fat, lng, bc):
+    """D chi of PAPER.md Eq. 3 in the reading R13 (anti-Hermitian, staggered phases explicit)."""
+    chi, fat, lng = _c(chi), _c(fat), _c(lng)
+    out = np.empty_like(chi)
+    lib_s().ors_dslash(_p(out), _p(chi), _p(fat), _p(lng), _i4(_sdims(chi)), _i4(bc))
+    return out
+
+
+def stag_M(chi, fat, lng, bc, mass, dagger=False):
+    chi, fat, lng = _c(chi), _c(fat), _c(lng)
+    out = np.empty_like(chi)
+    lib_s().ors_M(_p(out), _p(chi), _p(fat), _p(lng), _i4(_sdims(chi)), _i4(bc), ctypes.c_double(mass), ctypes.c_int(int(dagger)))
+    return out
+
+
+def stag_MdagM(chi, fat, lng, bc, mass, sigma=0.0):
+    chi, fat, lng = _c(chi), _c(fat), _c(lng)
+    out = np.empty_like(chi)
+    lib_s().ors_MdagM(_p(out), _p(chi), _p(fat), _p(lng), _i4(_sdims(chi)), _i4(bc), ctypes.c_double(mass), ctypes.c_double(sigma))
+    return out
+
+
+def stag_cg(b, fat, lng, bc, mass, sigma=0.0, tol=1e-12, maxit=100000):
+    """x = (M^dag M + sigma)^-1 b by plain CG (Eq. 4, one shift).  Returns (x, info)."""
+    b, fat, lng = _c(b), _c(fat), _c(lng)
+    x = np.empty_like(b)
+    it, rr = ctypes.c_int(0), ctypes.c_double(0)
+    st = lib_s().ors_cg(_p(x), _p(b), _p(fat), _p(lng), _i4(_sdims(b)), _i4(bc), ctypes.c_double(mass), ctypes.c_double(sigma),
+                        ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.byref(it), ctypes.byref(rr))
+    return x, dict(status=st, iterations=it.value, true_residual=rr.value)

@@ -119,3 +119,26 @@ def gaussian_spinor_torch(dims, seed, device="cpu"):
     g.manual_seed(seed)
     a = torch.randn((T, Z, Y, X, 4, 3, 2), generator=g, dtype=torch.float64, device=device) / (2.0 ** 0.5)
     return torch.view_as_complex(a.contiguous())
+
+
+def staggered_links(dims, eps, seed, c1=1.125, c3=-1.0 / 24.0, smear=0.05):
+    """Synthetic fat and long link fields for the improved staggered operator: general
+    complex 3x3 matrices per link, as smeared links are.  fat = c1 * (random SU(3) + smear * complex
+    Gaussian noise) stands in for the asqtad fat links (sums of paths, not unitary); lng = c3 * (an
+    independent random SU(3)) for the three-link Naik term.  Both are inputs of the operator; no
+    smearing or link product is computed here.  Returns (fat, lng), each [mu][t][z][y][x][3][3]."""
+    X, Y, Z, T = dims
+    rng = np.random.default_rng(seed + 7919)
+    fat = c1 * random_gauge(dims, eps, seed)
+    n = rng.standard_normal((4, T, Z, Y, X, 3, 3, 2)) * (smear / np.sqrt(2.0))
+    fat = fat + c1 * (n[..., 0] + 1j * n[..., 1])
+    lng = c3 * random_gauge(dims, eps, seed + 104729)
+    return np.ascontiguousarray(fat), np.ascontiguousarray(lng)
+
+
+def gaussian_colour_vector(dims, seed):
+    """chi[t][z][y][x][3], re and im ~ N(0, 1/2): a staggered "spinor"."""
+    X, Y, Z, T = dims
+    rng = np.random.default_rng(seed)
+    a = rng.standard_normal((T, Z, Y, X, 3, 2)) / np.sqrt(2.0)
+    return np.ascontiguousarray(a[..., 0] + 1j * a[..., 1])
