@@ -71,6 +71,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_MATPC_SYMMETRIC  1
 
 #define LQCD_FIELD_SPINOR_PARITY 0
+#define LQCD_FIELD_STAGGERED_PARITY 1   /* 3-component colour vectors of one parity (fp64 / fp32 only) */
 
 /* Create a context for a lattice dims = (X,Y,Z,T), all even and >= 2, with per-direction
  * boundary condition boundary[mu] = +1 periodic / -1 antiperiodic (R5).  `device` is the
@@ -187,6 +188,25 @@ int lqcd_invert(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical,
  * LQCD_EBREAKDOWN if at least one source ended that way (see result[r].status).  Synchronises `stream`. */
 int lqcd_invert_mrhs(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical, int nrhs,
                      const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
+
+/* ---- improved staggered (asqtad) path: PAPER.md:114-122 Sec. 2.3 Eq. 3, :130-134 Eq. 4, :296 Sec. 8.2;
+ * SURVEY.md 8(f) NEXT-3; readings R13-R15 of DESIGN.md ------------------------------------------------
+ *   (D chi)(x) = sum_mu eta_mu(x) [ fat_mu(x) chi(x+mu) - fat_mu(x-mu)^dag chi(x-mu)
+ *                                 + lng_mu(x) chi(x+3mu) - lng_mu(x-3mu)^dag chi(x-3mu) ],   M = -D/2 + m,
+ *   eta_x = 1, eta_y = (-1)^x, eta_z = (-1)^(x+y), eta_t = (-1)^(x+y+z); boundary sign on hops that wrap.
+ * Canonical layouts (device, complex128): fat / lng [mu][t][z][y][x][3][3], general 3x3 (the fat links
+ * are not unitary; path coefficients are part of the links; NO phases, NO boundary signs);
+ * colour vectors chi[t][z][y][x][3].  Packed fields: lqcd_field_bytes(LQCD_FIELD_STAGGERED_PARITY),
+ * precisions LQCD_PREC_DOUBLE and LQCD_PREC_SINGLE (half is "not amenable", PAPER.md:298 fn. 3).
+ * Every extent must be >= 4 (three-hop term).  Errors as for the Wilson-clover calls. */
+int lqcd_load_staggered_links(lqcd_ctx* ctx, const void* fat_canonical, const void* lng_canonical, void* stream);
+int lqcd_pack_staggered(lqcd_ctx* ctx, void* packed, const void* canonical, int parity, int prec, void* stream);
+int lqcd_unpack_staggered(lqcd_ctx* ctx, void* canonical, const void* packed, int parity, int prec, void* stream);
+/* out_p = D_{p,pbar} in_pbar: 16 hops, 1146 flop per site.  out must not alias in. */
+int lqcd_staggered_dslash(lqcd_ctx* ctx, void* out, const void* in, int parity_out, int prec, void* stream);
+/* out = (M^dag M + sigma) in on `parity` = (m^2 + sigma) in - D_{p,pbar} D_{pbar,p} in / 4: two launches. */
+int lqcd_staggered_mdagm(lqcd_ctx* ctx, void* out, const void* in, int parity, double mass, double sigma,
+                         int prec, void* stream);
 
 /* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */
 /* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned for full PCIe speed;

@@ -103,6 +103,11 @@ struct lqcd_ctx {
   cudaStream_t hs_in, hs_out;
   cudaEvent_t hev_in[LQ_HOST_SLABS], hev_out[LQ_HOST_SLABS], hev_sync;
   bool have_hpipe;
+  // improved staggered path (staggered.cu): fp64 master links, fp32 copies, M^dag M temporaries
+  bool have_stag;
+  double *sfat64, *slng64;
+  char *sfat32, *slng32;
+  char* stmp[2];
   char* mtmp;             // multi-right-hand-side Mhat temporary (grow-only)
   size_t mtmp_bytes;
 };

@@ -19,7 +19,7 @@ PREC_DOUBLE, PREC_SINGLE, PREC_HALF = 0, 1, 2
 RECON_18, RECON_12, RECON_8 = 18, 12, 8
 SOLVER_BICGSTAB, SOLVER_GCR_DD, SOLVER_CGNR = 0, 1, 2
 MATPC_ASYMMETRIC, MATPC_SYMMETRIC = 0, 1
-FIELD_SPINOR_PARITY = 0
+FIELD_SPINOR_PARITY, FIELD_STAGGERED_PARITY = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = [
@@ -27,6 +27,7 @@ EXPORTS = [
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
     "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
+    "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm",
 ]
 
 
@@ -94,6 +95,11 @@ def load_library():
             "lqcd_axpy_norm": (i, [vp, d, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_cdot": (i, [vp, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_launch_count": (ctypes.c_longlong, [vp]),
+            "lqcd_load_staggered_links": (i, [vp, vp, vp, vp]),
+            "lqcd_pack_staggered": (i, [vp, vp, vp, i, i, vp]),
+            "lqcd_unpack_staggered": (i, [vp, vp, vp, i, i, vp]),
+            "lqcd_staggered_dslash": (i, [vp, vp, vp, i, i, vp]),
+            "lqcd_staggered_mdagm": (i, [vp, vp, vp, i, d, d, i, vp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(lib, name)
@@ -200,6 +206,34 @@ class Context:
     def schwarz(self, out, inp, parity, kappa, block, n_mr, omega_mr, prec, recon, prec_io):
         self._check(self.lib.lqcd_schwarz(self.h, _ptr(out), _ptr(inp), parity, kappa, _i4(block), n_mr, omega_mr,
                                           prec, recon, prec_io, _stream()))
+        return out
+
+    # -- improved staggered ------------------------------------------------------------------------
+    def load_staggered_links(self, fat, lng):
+        for t in (fat, lng):
+            assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()
+        self._check(self.lib.lqcd_load_staggered_links(self.h, _ptr(fat), _ptr(lng), _stream()))
+
+    def new_staggered_field(self, prec):
+        return torch.empty(self.lib.lqcd_field_bytes(self.h, FIELD_STAGGERED_PARITY, prec), dtype=torch.uint8, device=self.device)
+
+    def pack_staggered(self, canonical, parity, prec, out=None):
+        assert canonical.is_cuda and canonical.dtype == torch.complex128 and canonical.is_contiguous()
+        out = self.new_staggered_field(prec) if out is None else out
+        self._check(self.lib.lqcd_pack_staggered(self.h, _ptr(out), _ptr(canonical), parity, prec, _stream()))
+        return out
+
+    def unpack_staggered(self, canonical, packed, parity, prec):
+        assert canonical.is_cuda and canonical.dtype == torch.complex128 and canonical.is_contiguous()
+        self._check(self.lib.lqcd_unpack_staggered(self.h, _ptr(canonical), _ptr(packed), parity, prec, _stream()))
+        return canonical
+
+    def staggered_dslash(self, out, inp, parity_out, prec):
+        self._check(self.lib.lqcd_staggered_dslash(self.h, _ptr(out), _ptr(inp), parity_out, prec, _stream()))
+        return out
+
+    def staggered_mdagm(self, out, inp, parity, mass, sigma, prec):
+        self._check(self.lib.lqcd_staggered_mdagm(self.h, _ptr(out), _ptr(inp), parity, mass, sigma, prec, _stream()))
         return out
 
     # -- BLAS-1 ---------------------------------------------------------------------------------

@@ -1,0 +1,109 @@
+"""Improved staggered path on the GPU (-m gpu) against oracle/staggered_oracle.cpp on the same seeded
+inputs: pack/unpack round trip, the hopping term on both parities, M^dag M + sigma, free-field closed
+form, on a ragged lattice (Vh = 1440 sites = 11.25 CTAs) with mixed boundary conditions."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1109_2935_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+STOL = {0: 1e-13, 1: 1e-5}
+
+
+def _rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+class SCase:
+    def __init__(self, dims, eps, bc, seed=1, unit=False):
+        from paper_1109_2935_b200 import lqcd
+        self.lqcd, self.dims, self.bc = lqcd, dims, bc
+        if unit:
+            one = inputs.unit_gauge(dims)
+            self.fat, self.lng = 1.125 * one, (-1.0 / 24.0) * one
+        else:
+            self.fat, self.lng = inputs.staggered_links(dims, eps, seed)
+        self.ctx = lqcd.Context(dims, bc, 0)
+        self.ctx.load_staggered_links(torch.from_numpy(self.fat).cuda(), torch.from_numpy(self.lng).cuda())
+        self.par = inputs.parity_mask(dims)
+
+    def mask(self, p):
+        return (self.par == p)[..., None]
+
+    def op(self, fn, chi, p_in, p_out, prec):
+        d = torch.from_numpy(np.ascontiguousarray(chi)).cuda()
+        fin = self.ctx.pack_staggered(d, p_in, prec)
+        fout = self.ctx.new_staggered_field(prec)
+        fn(fout, fin)
+        res = torch.zeros_like(d)
+        self.ctx.unpack_staggered(res, fout, p_out, prec)
+        torch.cuda.synchronize()
+        return res.cpu().numpy()
+
+
+@pytest.fixture(scope="module")
+def ragged():
+    return SCase((6, 4, 10, 12), 0.4, (-1, 1, 1, -1))
+
+
+def test_pack_unpack_roundtrip(ragged):
+    c = ragged
+    chi = inputs.gaussian_colour_vector(c.dims, 2)
+    for prec in (0, 1):
+        for p in (0, 1):
+            got = c.op(lambda o, i: o.copy_(i), chi, p, p, prec)
+            want = chi * c.mask(p)
+            if prec == 0:
+                assert np.array_equal(got, want)
+            else:
+                assert _rel(got, want) <= 1e-7 and np.max(np.abs(got[c.par != p])) == 0.0
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_dslash_and_mdagm(ragged, prec):
+    c = ragged
+    chi = inputs.gaussian_colour_vector(c.dims, 3)
+    for p in (0, 1):
+        want = oracle.stag_dslash(chi * c.mask(1 - p), c.fat, c.lng, c.bc) * c.mask(p)
+        got = c.op(lambda o, i: c.ctx.staggered_dslash(o, i, p, prec), chi, 1 - p, p, prec)
+        assert _rel(got, want) <= STOL[prec], ("dslash", p)
+        assert np.max(np.abs(got[c.par != p])) == 0.0
+        for mass, sigma in ((0.05, 0.0), (0.3, 0.7)):
+            want = oracle.stag_MdagM(chi * c.mask(p), c.fat, c.lng, c.bc, mass, sigma) * c.mask(p)
+            got = c.op(lambda o, i: c.ctx.staggered_mdagm(o, i, p, mass, sigma, prec), chi, p, p, prec)
+            assert _rel(got, want) <= STOL[prec], ("mdagm", p, mass, sigma)
+
+
+def test_free_field_closed_form_on_gpu():
+    dims, bc, n = (8, 4, 6, 12), (1, -1, 1, -1), (3, 1, 2, 5)
+    c = SCase(dims, 0.0, bc, unit=True)
+    X, Y, Z, T = dims
+    p = 2 * np.pi * (np.array(n) + np.where(np.array(bc) < 0, 0.5, 0.0)) / np.array(dims)
+    t, z, y, x = np.meshgrid(np.arange(T), np.arange(Z), np.arange(Y), np.arange(X), indexing="ij")
+    phase = np.exp(1j * (p[0] * x + p[1] * y + p[2] * z + p[3] * t))
+    chi = phase[..., None] * np.array([0.3 - 1.0j, 2.0, -0.5 + 0.25j])
+    m, sigma = 0.07, 0.4
+    lam = m * m + sigma + np.sum((1.125 * np.sin(p) - np.sin(3 * p) / 24.0) ** 2)
+    for par in (0, 1):
+        got = c.op(lambda o, i: c.ctx.staggered_mdagm(o, i, par, m, sigma, 0), chi, par, par, 0)
+        assert _rel(got, lam * chi * c.mask(par)) <= 1e-13
+    c.ctx.close()
+
+
+def test_staggered_errors():
+    from paper_1109_2935_b200 import lqcd
+    ctx = lqcd.Context((4, 4, 4, 4), (1, 1, 1, -1), 0)
+    f, g = ctx.new_staggered_field(1), ctx.new_staggered_field(1)
+    with pytest.raises(lqcd.LqcdError) as e:
+        ctx.staggered_dslash(f, g, 0, 1)                        # links not loaded
+    assert e.value.code == lqcd.ESTATE
+    assert ctx.lib.lqcd_field_bytes(ctx.h, lqcd.FIELD_STAGGERED_PARITY, 2) == 0     # no half-precision staggered fields
+    ctx.close()
+    ctx = lqcd.Context((2, 4, 4, 4), (1, 1, 1, -1), 0)
+    one = torch.from_numpy(inputs.unit_gauge((2, 4, 4, 4))).cuda()
+    with pytest.raises(lqcd.LqcdError) as e:
+        ctx.load_staggered_links(one, one)                      # extent 2 < 4
+    assert e.value.code == lqcd.EINVAL
+    ctx.close()
