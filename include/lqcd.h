@@ -208,6 +208,18 @@ int lqcd_staggered_dslash(lqcd_ctx* ctx, void* out, const void* in, int parity_o
 int lqcd_staggered_mdagm(lqcd_ctx* ctx, void* out, const void* in, int parity, double mass, double sigma,
                          int prec, void* stream);
 
+/* Solve (M^dag M + sigma_i) x_i = b on `parity` for nshift (1..32) shifts 0 <= sigma_0 < sigma_1 < ... (Eq. 4,
+ * PAPER.md:130-134) with the paper's strategy: a pure single-precision multi-shift CG for all
+ * shifts at once, then sequential mixed-precision CG (fp64 outer with reliable updates, fp32 inner) refining
+ * every x_i until ||b - (M^dag M + sigma_i) x_i|| <= tol ||b|| in fp64.  b_canonical: chi-shaped DEVICE array
+ * (only the sites of `parity` are read); x_canonical: nshift such arrays back to back (sites of the other
+ * parity are set to zero).  result[i]: iterations / restarts / matpc_sloppy / matpc_outer of shift i's
+ * refinement, true_residual; result[0].matpc_precond = iterations of the multi-shift phase; seconds and gflop
+ * are those of the whole call.  max_iter bounds each phase.  Synchronises `stream`. */
+int lqcd_staggered_multishift(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical, int parity, double mass,
+                              const double* sigma, int nshift, double tol, int max_iter,
+                              lqcd_invert_result* result, void* stream);
+
 /* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */
 /* out_host/in_host: canonical full-lattice complex128 HOST arrays (pinned for full PCIe speed;
  * pageable works), owned by the caller, not overlapping.

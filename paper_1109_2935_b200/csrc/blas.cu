@@ -27,6 +27,7 @@ LQ_INST(OpZero) LQ_INST(OpNorm2) LQ_INST(OpCdot) LQ_INST(OpAxpyNorm) LQ_INST(OpX
 LQ_INST(OpBicgInit) LQ_INST(OpBicgP) LQ_INST(OpBicgAlpha) LQ_INST(OpBicgS) LQ_INST(OpBicgOmega) LQ_INST(OpBicgXR)
 LQ_INST(OpGcrScale)
 LQ_INST(OpCgInit) LQ_INST(OpCgP) LQ_INST(OpCgAlpha) LQ_INST(OpCgXR)
+LQ_INST(OpCgPAp) LQ_INST(OpCgXRB) LQ_INST(OpMsR)
 typedef OpMrUpdate<true, false> OpMrFirst;
 typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;

@@ -234,6 +234,79 @@ struct OpCgXR {            // v0 = x, v1 = p, v2 = r, v3 = w : x += alpha p ; r 
   LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) { a.S[S_RR] = s[0]; }
 };
 
+// ---- CG on a Hermitian positive definite operator, and its multi-shift form (staggered path) -----
+// (M^dag M + sigma_i) x_i = b, Eq. 4, solver of PAPER.md:296.  Scalars: rr = <r,r> in
+// S_RHO, alpha in S_ALPHA, beta in S_BETA (real).  Multi-shift state (Jegerlehner's recurrences; the
+// shifted residuals are zeta_i r): per shift i at S_MS + LQ_MS_STRIDE*i: zeta, zeta_old, alpha_i, beta_i,
+// sigma_i - sigma_0; S_MS_AOLD, S_MS_BOLD the previous alpha, beta of the base system; S_MS_N shifts.
+enum { S_MS = S_GCR_BETA, LQ_MS_STRIDE = 8, LQ_MS_MAX = 32, S_MS_AOLD = S_MS + LQ_MS_STRIDE * LQ_MS_MAX, S_MS_BOLD, S_MS_N };
+static_assert(S_MS_N < S_GCR_GAMMAS, "multi-shift scalars must fit the GCR beta region they reuse");
+
+struct OpCgPAp {           // v0 = p, v1 = A p : alpha = rr / Re<p, A p>
+  static constexpr int NV = 1, READ = 3, WRITE = 0;
+  typedef NoCoef Coef;
+  LQ_DEV static void prepare(Coef&, const BlasArgs&, int) {}
+  template <typename R> LQ_DEV static void site(const Coef&, R* p, R* ap, R*, R*, R*, double* red) {
+    R s = 0;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) s = fma_(p[k], ap[k], s);
+    red[0] += (double)s;
+  }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+    double* S = a.S;
+    if (!(s[0] > 0.0)) { S[S_FLAG] = 1; S[S_ALPHA] = 0; return; }
+    S[S_ALPHA] = S[S_RHO] / s[0];
+  }
+};
+
+struct OpCgXRB {           // v0 = x, v1 = p, v2 = r, v3 = A p : x += alpha p ; r -= alpha A p ; rr' = ||r||^2 ; beta = rr'/rr
+  static constexpr int NV = 1, READ = 15, WRITE = 5;
+  struct Coef { double a; };
+  LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int) { c.a = a.S[S_ALPHA]; }
+  template <typename R> LQ_DEV static void site(const Coef& c, R* x, R* p, R* r, R* ap, R*, double* red) {
+    const R al = (R)c.a;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) { x[k] = fma_(al, p[k], x[k]); r[k] = fma_(-al, ap[k], r[k]); }
+    site_norm2(r, red[0]);
+  }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+    double* S = a.S;
+    S[S_BETA] = (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;
+    S[S_RHO] = s[0]; S[S_RR] = s[0];
+  }
+};
+
+struct OpMsR {             // v0 = r, v1 = A p (base system): r -= alpha A p ; rr' ; beta ; all shifted scalars
+  static constexpr int NV = 1, READ = 3, WRITE = 1;
+  struct Coef { double a; };
+  LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int) { c.a = a.S[S_ALPHA]; }
+  template <typename R> LQ_DEV static void site(const Coef& c, R* r, R* ap, R*, R*, R*, double* red) {
+    const R al = (R)c.a;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) r[k] = fma_(-al, ap[k], r[k]);
+    site_norm2(r, red[0]);
+  }
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+    double* S = a.S;
+    const double al = S[S_ALPHA], be = (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;
+    const double a_old = S[S_MS_AOLD], b_old = S[S_MS_BOLD];
+    const int n = (int)S[S_MS_N];
+    for (int i = 0; i < n; ++i) {
+      double* m = S + S_MS + LQ_MS_STRIDE * i;
+      const double z = m[0], zo = m[1], d = m[4];
+      // zeta_{n+1} = zeta_n zeta_{n-1} a_{n-1} / ( a_n b_{n-1} (zeta_{n-1} - zeta_n) + zeta_{n-1} a_{n-1} (1 + d a_n) )
+      const double den = al * b_old * (zo - z) + zo * a_old * (1.0 + d * al);
+      const double zn = (den != 0.0) ? z * zo * a_old / den : 0.0;
+      const double ratio = (z != 0.0) ? zn / z : 0.0;
+      m[2] = al * ratio;                 // alpha_i of this step
+      m[3] = be * ratio * ratio;         // beta_i
+      m[1] = z; m[0] = zn;
+    }
+    S[S_MS_AOLD] = al; S[S_MS_BOLD] = be;
+    S[S_BETA] = be; S[S_RHO] = s[0]; S[S_RR] = s[0];
+  }
+};
+
 // ---- GCR (Algorithm 1) --------------------------------------------------------------------------
 struct OpGcrScale {        // v0 = z_k, v1 = rhat : z_k /= gamma ; rhat -= alpha z_k ; rr = ||rhat||^2
   static constexpr int NV = 1, READ = 3, WRITE = 3;

@@ -97,6 +97,80 @@ int op_stag_mdagm(lqcd_ctx* c, char* out, const char* in, int p, double mass, do
   return op_stag_dslash(c, out, tmp, in, mass * mass + sigma, -0.25, p, prec, s);
 }
 
+// ---------------------------------------------------------------- solver for Eq. 4
+struct MsArgs {
+  const char* r;
+  char* x[LQ_MS_MAX];
+  char* p[LQ_MS_MAX];
+  const double* S;
+  long long ns;         // records (= Vh/4)
+  int n;                // active shifts (a prefix: shifts are sorted ascending, larger ones converge first)
+};
+
+// one pass over r: x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i for every active shift
+template <class P>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) ms_update_kernel(const MsArgs m) {
+  typedef typename P::real R;
+  const long long i = (long long)blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x;
+  if (i >= m.ns) return;
+  R r[24];
+  load_site<P, 24>(r, m.r, m.ns, i);
+  for (int k = 0; k < m.n; ++k) {
+    const double* sc = m.S + S_MS + LQ_MS_STRIDE * k;
+    const R z = (R)sc[0], al = (R)sc[2], be = (R)sc[3];
+    R x[24], p[24];
+    load_site<P, 24>(x, m.x[k], m.ns, i);
+    load_site<P, 24>(p, m.p[k], m.ns, i);
+#pragma unroll
+    for (int j = 0; j < 24; ++j) { x[j] = fma_(al, p[j], x[j]); p[j] = fma_(be, p[j], z * r[j]); }
+    store_site<P, 24>(x, m.x[k], m.ns, i);
+    store_site<P, 24>(p, m.p[k], m.ns, i);
+  }
+}
+
+BlasArgs mks(lqcd_ctx* c, char* v0 = nullptr, char* v1 = nullptr, char* v2 = nullptr, char* v3 = nullptr) {
+  BlasArgs a;
+  memset(&a, 0, sizeof(a));
+  a.v[0] = v0; a.v[1] = v1; a.v[2] = v2; a.v[3] = v3;
+  a.ns = c->Vh / 4; a.vh = (int)(c->Vh / 4); a.nb = 1;      // quad-site records (staggered.cuh)
+  a.S = c->S; a.partials = c->partials; a.counters = c->counters;
+  return a;
+}
+template <class Op> int sblas(lqcd_ctx* c, int prec, const BlasArgs& a, cudaStream_t s) {
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s, 1);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "staggered blas launch", e);
+}
+int sread(lqcd_ctx* c, int off, int n, cudaStream_t s) {
+  cudaError_t e = cudaMemcpyAsync(c->hS + off, c->S + off, n * sizeof(double), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "scalar read-back", e);
+}
+int sconvert(lqcd_ctx* c, int pa, int pb, char* dst, const char* src, cudaStream_t s) {
+  BlockMap bm = c->bm;
+  bm.nat.ns = c->Vh / 4; bm.nat.vh = (int)(c->Vh / 4);
+  cudaError_t e = run_convert(pa, pb, dst, src, bm, 0, 0, s);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "convert", e);
+}
+// y (fp64) += x (fp32)
+int saccumulate(lqcd_ctx* c, char* y, char* x, cudaStream_t s) {
+  MultiArgs m; memset(&m, 0, sizeof(m));
+  m.b = mks(c); m.z[0] = x; m.chi[0] = 1.0; m.n = 1;
+  cudaError_t e = run_accumulate(0, 1, y, m, s); c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "accumulate", e);
+}
+// r = b - (M^dag M + sigma) x in fp64 ; *rn = ||r||
+int sresidual(lqcd_ctx* c, char* r, const char* b, const char* x, int par, double mass, double sigma, double* rn, cudaStream_t s) {
+  int rc = op_stag_mdagm(c, r, x, par, mass, sigma, 0, s);
+  if (rc) return rc;
+  BlasArgs a = mks(c, const_cast<char*>(b), r);
+  if ((rc = sblas<OpXmyNorm>(c, 0, a, s))) return rc;
+  if ((rc = sread(c, S_OUT, 1, s))) return rc;
+  *rn = sqrt(c->hS[S_OUT]);
+  return LQCD_OK;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -154,6 +228,173 @@ int lqcd_staggered_mdagm(lqcd_ctx* c, void* out, const void* in, int parity, dou
   if (rc) return rc;
   cudaSetDevice(c->device);
   return op_stag_mdagm(c, (char*)out, (const char*)in, parity, mass, sigma, prec, (cudaStream_t)stream);
+}
+
+// (M^dag M + sigma_i) x_i = b on one parity, i < nshift (Eq. 4), by the paper's strategy
+// (PAPER.md:296): a pure single-precision multi-shift CG for all shifts at once, then sequential
+// mixed-precision CG (fp64 outer with reliable updates, fp32 inner) refining every x_i to `tol`.
+int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int parity, double mass, const double* sigma,
+                              int nshift, double tol, int max_iter, lqcd_invert_result* res, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!x_can || !b_can || !sigma || !res || (parity | 1) != 1 || nshift < 1 || nshift > LQ_MS_MAX || !(tol > 0) || max_iter < 1)
+    return fail(c, LQCD_EINVAL, "staggered_multishift arguments");
+  for (int i = 0; i < nshift; ++i) if (!(sigma[i] >= 0.0)) return fail(c, LQCD_EINVAL, "shifts must be >= 0");
+  for (int i = 1; i < nshift; ++i) if (!(sigma[i] > sigma[i - 1])) return fail(c, LQCD_EINVAL, "shifts must be strictly ascending");
+  int rc = stag_check(c, 0);
+  if (rc) return rc;
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  memset(res, 0, sizeof(*res) * nshift);
+  const size_t f64 = colour_bytes(0, c->Vh), f32 = colour_bytes(1, c->Vh), cbytes = (size_t)c->V * 6 * sizeof(double);
+  struct Bufs { std::vector<void*> v; ~Bufs() { for (void* p : v) cudaFree(p); } } bufs;
+  auto get = [&](char** out, size_t bytes) -> int {
+    void* p = nullptr;
+    int rc2 = dev_alloc(c, &p, bytes);
+    if (rc2) return rc2;
+    bufs.v.push_back(p); *out = (char*)p;
+    return LQCD_OK;
+  };
+  char *b_hi, *x_hi, *r_hi, *r, *ap, *xs, *ps;
+  if ((rc = get(&b_hi, f64)) || (rc = get(&x_hi, f64)) || (rc = get(&r_hi, f64)) || (rc = get(&r, f32)) || (rc = get(&ap, f32)) ||
+      (rc = get(&xs, f32 * nshift)) || (rc = get(&ps, f32 * nshift))) return rc;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  struct Ev { cudaEvent_t a, b; ~Ev() { cudaEventDestroy(a); cudaEventDestroy(b); } } ev{e0, e1};
+  cudaEventRecord(e0, s);
+  cudaError_t e = run_pack_colour(0, b_hi, (const double*)b_can, c->nat, parity, 0, s); c->launches++;
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack", e);
+  double bn;
+  { BlasArgs a = mks(c, b_hi); a.i0 = 0; if ((rc = sblas<OpNorm2>(c, 0, a, s))) return rc; }
+  if ((rc = sread(c, S_OUT, 1, s))) return rc;
+  bn = sqrt(c->hS[S_OUT]);
+  e = cudaMemsetAsync(x_can, 0, cbytes * nshift, s);
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "memset", e);
+  long long n_lo = 0, n_hi = 0;
+  double blas_sites = 0;
+  int ms_iters = 0, worst = LQCD_OK;
+  if (bn > 0.0) {
+    // ---- phase 1: multi-shift CG in single precision, all x_i = 0, r = p_i = b
+    if ((rc = sconvert(c, 0, 1, r, b_hi, s))) return rc;
+    for (int i = 0; i < nshift; ++i) {
+      if ((rc = sconvert(c, 1, 1, ps + i * f32, r, s))) return rc;
+      BlasArgs a = mks(c, xs + i * f32); if ((rc = sblas<OpZero>(c, 1, a, s))) return rc;
+    }
+    { BlasArgs a = mks(c, r); a.i0 = 0; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }      // rr -> S_RHO, flag = 0
+    {
+      double* h = c->hS;                                  // initial multi-shift state
+      for (int i = 0; i < nshift; ++i) {
+        double* m = h + S_MS + LQ_MS_STRIDE * i;
+        m[0] = 1; m[1] = 1; m[2] = 0; m[3] = 0; m[4] = sigma[i] - sigma[0];
+      }
+      h[S_MS_AOLD] = 1; h[S_MS_BOLD] = 0; h[S_MS_N] = nshift;
+      e = cudaMemcpyAsync(c->S + S_MS, h + S_MS, (S_MS_N + 1 - S_MS) * sizeof(double), cudaMemcpyHostToDevice, s);
+      if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "multi-shift state", e);
+    }
+    // single precision cannot resolve more than ~1e-6 of the source; the refinement takes over from there
+    const double ms_stop = (tol > 2e-6 ? tol : 2e-6) * bn;
+    int active = nshift;
+    double rn = bn, best = bn;
+    int stall = 0;
+    while (rn > ms_stop && ms_iters < max_iter) {
+      if ((rc = op_stag_mdagm(c, ap, ps, parity, mass, sigma[0], 1, s))) return rc;
+      { BlasArgs a = mks(c, ps, ap); if ((rc = sblas<OpCgPAp>(c, 1, a, s))) return rc; }
+      { BlasArgs a = mks(c, r, ap); if ((rc = sblas<OpMsR>(c, 1, a, s))) return rc; }
+      MsArgs m; memset(&m, 0, sizeof(m));
+      m.r = r; m.S = c->S; m.ns = c->Vh / 4; m.n = active;
+      for (int i = 0; i < active; ++i) { m.x[i] = xs + i * f32; m.p[i] = ps + i * f32; }
+      ms_update_kernel<PrecS><<<(unsigned)((m.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK), LQ_BLAS_BLOCK, 0, s>>>(m);
+      c->launches++;
+      if ((e = cudaGetLastError()) != cudaSuccess) return fail(c, LQCD_ECUDA, "ms_update", e);
+      ++ms_iters; ++n_lo; blas_sites += 6.0 * (2 + 3 + 5 * active);
+      if ((rc = sread(c, 0, S_MS_N + 1, s))) return rc;
+      const double rr = c->hS[S_RR];
+      if (!(rr == rr) || c->hS[S_FLAG] != 0.0) { worst = LQCD_EBREAKDOWN; break; }
+      rn = sqrt(rr);
+      // a shift whose own residual |zeta_i| ||r|| is below the target is finished: drop it (it is a suffix)
+      while (active > 1 && fabs(c->hS[S_MS + LQ_MS_STRIDE * (active - 1)]) * rn <= ms_stop) --active;
+      if (rn < 0.999 * best) { best = rn; stall = 0; } else if (++stall > 50) break;     // fp32 floor reached
+    }
+  }
+  // ---- phase 2: sequential mixed-precision CG refinement of every shift (fp64 outer, fp32 inner)
+  const double stop = tol * bn, delta = 0.1;
+  worst = LQCD_OK;                                         // a breakdown of the single-precision phase is repaired below
+  char *xl = r, *rl = ap;                                  // fp32 work fields reused: x_l, r_l ; p and A p below
+  char *pl, *apl;
+  if ((rc = get(&pl, f32)) || (rc = get(&apl, f32))) return rc;
+  for (int i = 0; i < nshift; ++i) {
+    lqcd_invert_result& R = res[i];
+    if (bn == 0.0) { R.status = LQCD_OK; continue; }
+    if ((rc = sconvert(c, 1, 0, x_hi, xs + i * f32, s))) return rc;
+    double rn;
+    if ((rc = sresidual(c, r_hi, b_hi, x_hi, parity, mass, sigma[i], &rn, s))) return rc;
+    ++n_hi; R.matpc_outer++;
+    int status = LQCD_OK;
+    if (!(rn == rn)) {                                     // the single-precision phase broke down: start from zero
+      BlasArgs a = mks(c, x_hi); if ((rc = sblas<OpZero>(c, 0, a, s))) return rc;
+      if ((rc = sresidual(c, r_hi, b_hi, x_hi, parity, mass, sigma[i], &rn, s))) return rc;
+      ++n_hi; R.matpc_outer++; status = LQCD_OK;
+    }
+    int it = 0;
+    bool fresh = true;                                      // start (or restart) the direction p = r
+    double maxr = rn;
+    while (rn > stop) {
+      if (fresh) {
+        if ((rc = sconvert(c, 0, 1, rl, r_hi, s))) return rc;
+        { BlasArgs a = mks(c, xl); if ((rc = sblas<OpZero>(c, 1, a, s))) return rc; }
+        { BlasArgs a = mks(c, pl); if ((rc = sblas<OpZero>(c, 1, a, s))) return rc; }
+        { BlasArgs a = mks(c, rl); a.i0 = 0; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }
+        { BlasArgs a = mks(c, pl, rl); if ((rc = sblas<OpCgP>(c, 1, a, s))) return rc; }
+        fresh = false;
+      }
+      if (it >= max_iter) { status = LQCD_ENOCONV; break; }
+      if ((rc = op_stag_mdagm(c, apl, pl, parity, mass, sigma[i], 1, s))) return rc;
+      { BlasArgs a = mks(c, pl, apl); if ((rc = sblas<OpCgPAp>(c, 1, a, s))) return rc; }
+      { BlasArgs a = mks(c, xl, pl, rl, apl); if ((rc = sblas<OpCgXRB>(c, 1, a, s))) return rc; }
+      { BlasArgs a = mks(c, pl, rl); if ((rc = sblas<OpCgP>(c, 1, a, s))) return rc; }
+      ++it; ++n_lo; R.matpc_sloppy++; blas_sites += 6.0 * (2 + 6 + 3);
+      if ((rc = sread(c, S_RR, 2, s))) return rc;
+      const double rr = c->hS[S_RR];
+      const bool bad = !(rr == rr) || c->hS[S_FLAG] != 0.0;
+      const double rln = sqrt(rr);
+      if (rln > maxr) maxr = rln;
+      if (bad || rln <= stop || rln < delta * maxr) {
+        // reliable update: x += x_l, true residual in fp64; the direction is kept (beta from the new residual)
+        if ((rc = saccumulate(c, x_hi, xl, s))) return rc;
+        { BlasArgs a = mks(c, xl); if ((rc = sblas<OpZero>(c, 1, a, s))) return rc; }
+        if ((rc = sresidual(c, r_hi, b_hi, x_hi, parity, mass, sigma[i], &rn, s))) return rc;
+        ++n_hi; R.matpc_outer++; R.restarts++;
+        if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
+        if (rn <= stop) break;
+        maxr = rn;
+        if (bad) { fresh = true; continue; }
+        if ((rc = sconvert(c, 0, 1, rl, r_hi, s))) return rc;
+        { BlasArgs a = mks(c, rl); a.i0 = 1; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }
+        { BlasArgs a = mks(c, pl, rl); if ((rc = sblas<OpCgP>(c, 1, a, s))) return rc; }
+      }
+    }
+    if (status == LQCD_ENOCONV) {                          // fold what the inner iteration has and report its true residual
+      if ((rc = saccumulate(c, x_hi, xl, s))) return rc;
+      if ((rc = sresidual(c, r_hi, b_hi, x_hi, parity, mass, sigma[i], &rn, s))) return rc;
+      ++n_hi; R.matpc_outer++;
+    }
+    R.status = status; R.iterations = it;
+    R.true_residual = rn / bn; R.iterated_residual = rn / bn;
+    if (status != LQCD_OK && worst == LQCD_OK) worst = status;
+    e = run_pack_colour(0, x_hi, (const double*)((const char*)x_can + i * cbytes), c->nat, parity, 1, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "unpack", e);
+  }
+  res[0].matpc_sloppy += ms_iters;
+  res[0].matpc_precond = ms_iters;                          // iterations of the multi-shift phase
+  cudaEventRecord(e1, s);
+  e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "staggered_multishift", e);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  const double gflop = ((double)(n_lo + n_hi) * (2.0 * 1146 + 12) + blas_sites) * (double)c->Vh * 1e-9;
+  for (int i = 0; i < nshift; ++i) { res[i].seconds = ms * 1e-3; res[i].gflop = gflop; }
+  if (worst == LQCD_ENOCONV) return fail(c, worst, "max_iter reached for at least one shift");
+  if (worst == LQCD_EBREAKDOWN) return fail(c, worst, "breakdown for at least one shift");
+  return LQCD_OK;
 }
 
 }  // extern "C"

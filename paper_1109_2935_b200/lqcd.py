@@ -27,7 +27,7 @@ EXPORTS = [
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
     "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
-    "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm",
+    "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm", "lqcd_staggered_multishift",
 ]
 
 
@@ -100,6 +100,7 @@ def load_library():
             "lqcd_unpack_staggered": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_staggered_dslash": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_staggered_mdagm": (i, [vp, vp, vp, i, d, d, i, vp]),
+            "lqcd_staggered_multishift": (i, [vp, vp, vp, i, d, ctypes.POINTER(d), i, d, i, ctypes.POINTER(InvertResult), vp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(lib, name)
@@ -235,6 +236,16 @@ class Context:
     def staggered_mdagm(self, out, inp, parity, mass, sigma, prec):
         self._check(self.lib.lqcd_staggered_mdagm(self.h, _ptr(out), _ptr(inp), parity, mass, sigma, prec, _stream()))
         return out
+
+    def staggered_multishift(self, x, b, parity, mass, sigmas, tol, max_iter=10000, allow_fail=False):
+        """x: [nshift, T, Z, Y, X, 3], b: [T, Z, Y, X, 3] complex128 device tensors.  One result dict per shift."""
+        n = len(sigmas)
+        assert x.is_cuda and b.is_cuda and x.dtype == b.dtype == torch.complex128 and x.is_contiguous() and x.shape[0] == n
+        sg = (ctypes.c_double * n)(*[float(v) for v in sigmas])
+        r = (InvertResult * n)()
+        rc = self.lib.lqcd_staggered_multishift(self.h, _ptr(x), _ptr(b), parity, mass, sg, n, tol, max_iter, r, _stream())
+        self._check(rc, allow=(ENOCONV, EBREAKDOWN) if allow_fail else ())
+        return [r[k].as_dict() for k in range(n)]
 
     # -- BLAS-1 ---------------------------------------------------------------------------------
     def axpy_norm(self, a, x, y, prec):

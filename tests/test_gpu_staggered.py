@@ -107,3 +107,47 @@ def test_staggered_errors():
         ctx.load_staggered_links(one, one)                      # extent 2 < 4
     assert e.value.code == lqcd.EINVAL
     ctx.close()
+
+
+@pytest.mark.parametrize("parity", [0, 1])
+def test_multishift_solver(ragged, parity):
+    """lqcd_staggered_multishift (single-precision multi-shift CG + mixed-precision refinement):
+    every x_i equals the oracle's own CG solution of (M^dag M + sigma_i) x = b on that parity, and the true
+    residual recomputed with the ORACLE's operator meets the tolerance."""
+    c = ragged
+    mass, sigmas, tol = 0.08, [0.0, 0.01, 0.1, 0.5, 2.0], 1e-10
+    b = inputs.gaussian_colour_vector(c.dims, 5) * c.mask(parity)
+    x = torch.zeros((len(sigmas),) + b.shape, dtype=torch.complex128, device="cuda")
+    infos = c.ctx.staggered_multishift(x, torch.from_numpy(b).cuda(), parity, mass, sigmas, tol)
+    xs = x.cpu().numpy()
+    assert infos[0]["matpc_precond"] > 0                    # the multi-shift phase ran
+    for i, sg in enumerate(sigmas):
+        assert infos[i]["status"] == 0 and infos[i]["true_residual"] <= tol
+        assert np.max(np.abs(xs[i][c.par != parity])) == 0.0
+        res = np.linalg.norm(b - oracle.stag_MdagM(xs[i], c.fat, c.lng, c.bc, mass, sg)) / np.linalg.norm(b)
+        assert res <= 1.05 * tol, (i, res)
+        xo, io = oracle.stag_cg(b, c.fat, c.lng, c.bc, mass, sg, tol=1e-13)
+        assert io["status"] == 0 and _rel(xs[i], xo) <= 1e-8, i
+    # larger shifts are better conditioned: their refinement needs no more iterations than the smallest shift's
+    assert infos[-1]["iterations"] <= infos[0]["iterations"]
+
+
+def test_multishift_edges(ragged):
+    c = ragged
+    lq = c.lqcd
+    b = torch.from_numpy(inputs.gaussian_colour_vector(c.dims, 6)).cuda()
+    x = torch.zeros((2,) + tuple(b.shape), dtype=torch.complex128, device="cuda")
+    for bad in ([0.5, 0.1], [-0.1, 0.2], [0.3, 0.3]):         # not ascending / negative / repeated
+        with pytest.raises(lq.LqcdError) as e:
+            c.ctx.staggered_multishift(x, b, 0, 0.1, bad, 1e-8)
+        assert e.value.code == lq.EINVAL
+    # zero source: x = 0 at once
+    infos = c.ctx.staggered_multishift(x, torch.zeros_like(b), 0, 0.1, [0.0, 1.0], 1e-10)
+    assert all(i["status"] == 0 and i["iterations"] == 0 for i in infos) and float(x.abs().max()) == 0.0
+    # a single shift and a loose tolerance that the single-precision phase meets by itself
+    x1 = torch.zeros((1,) + tuple(b.shape), dtype=torch.complex128, device="cuda")
+    infos = c.ctx.staggered_multishift(x1, b, 1, 0.2, [0.0], 1e-4)
+    assert infos[0]["status"] == 0 and infos[0]["true_residual"] <= 1e-4 and infos[0]["iterations"] == 0
+    # iteration cap
+    infos = c.ctx.staggered_multishift(x, b, 0, 0.01, [0.0, 0.5], 1e-12, max_iter=3, allow_fail=True)
+    assert infos[0]["status"] == lq.ENOCONV and 0 < infos[0]["true_residual"] < 1.0
