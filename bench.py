@@ -45,7 +45,7 @@ def matpc_bytes(prec, recon):
 
 # ncu --set full captures of one launch at 32^3x64 (profiles/r1_dslash_*.md): DRAM bytes read + written,
 # and executed warp instructions (the half-precision kernels are issue-bound)
-NCU_TRAFFIC = {("fp32", 12): 595.03e6, ("half", 12): 298.28e6}
+NCU_TRAFFIC = {("fp32", 12): 595.03e6, ("half", 12): 298.28e6, ("staggered", "fp32"): 1238.6e6}
 NCU_WARP_INST = {("half", 12): 76.15e6}
 N_SCHEDULERS = 148 * 4      # one warp instruction per scheduler per clock (B200: 148 SMs x 4 SMSPs)
 
@@ -212,6 +212,8 @@ def main():
     ap.add_argument("--full", action="store_true", help="also run config 5 (48^3x96 GCR-DD vs BiCGstab)")
     ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
+    ap.add_argument("--op", default="dslash", choices=["dslash", "staggered"],
+                    help="dslash: the BASELINE metric (Wilson-clover Dslash); staggered: the improved staggered Dslash (SURVEY NEXT-3)")
     ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"], help="storage precision of the timed Dslash")
     ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8], help="link compression of the timed Dslash")
     ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per launch (>1: lqcd_dslash_mrhs; the BASELINE metric is 1)")
@@ -226,6 +228,9 @@ def main():
         run_reference(args, rank)
         return
     args.warmup = max(args.warmup, 3)
+    if args.op == "staggered":
+        run_staggered(args, rank, world, local)
+        return
 
     import torch
     import torch.distributed as dist
@@ -348,6 +353,126 @@ def main():
             out["parity_rel_l2_vs_oracle"] = float(torch.linalg.vector_norm(got - want) / torch.linalg.vector_norm(want))
     elif rank == 0:
         out["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_staggered(args, rank, world, local):
+    """Improved staggered (asqtad) Dslash at 32^3x64: a step = D on both parities
+    (2 launches), 1146 flop/site, compulsory bytes 16 links + 2 colour vectors per site; plus M^dag M and the
+    multi-shift solve (single-precision multi-shift CG + mixed-precision refinement) as extras."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1109_2935_b200 import inputs, lqcd
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    V = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3]
+    Vh = V // 2
+    pk, pk_kind = peaks()
+    if args.prec == "half":
+        raise SystemExit("staggered fields are fp64 or fp32")
+    prec = 0 if args.prec == "fp64" else 1
+    flop, by = 1146, (16 * 18 + 2 * 6) * (8 if prec == 0 else 4)
+    # synthetic fat / long links: scaled random SU(3) plus noise (inputs.staggered_links recipe, torch path)
+    fat = inputs.random_gauge_torch(DIMS, EPS, 31 + rank, device=dev) * 1.125
+    g = torch.Generator(device=dev)
+    g.manual_seed(32 + rank)
+    fat = fat + 1.125 * 0.05 * torch.view_as_complex(torch.randn(fat.shape + (2,), generator=g, dtype=torch.float64, device=dev)) / 2 ** 0.5
+    lng = inputs.random_gauge_torch(DIMS, EPS, 33 + rank, device=dev) * (-1.0 / 24.0)
+    chi = torch.view_as_complex(torch.randn((DIMS[3], DIMS[2], DIMS[1], DIMS[0], 3, 2), generator=g, dtype=torch.float64, device=dev) / 2 ** 0.5).contiguous()
+    ctx = lqcd.Context(DIMS, BC, local)
+    ctx.load_staggered_links(fat, lng)
+    f = [ctx.pack_staggered(chi, p, prec) for p in (0, 1)]
+    o = [ctx.new_staggered_field(prec) for _ in (0, 1)]
+
+    def step():
+        ctx.staggered_dslash(o[0], f[1], 0, prec)
+        ctx.staggered_dslash(o[1], f[0], 1, prec)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = ctx.launch_count()
+    ms = max_over_ranks(time_region(step, args.steps), dev)
+    launches = ctx.launch_count() - l0
+    # e2e through the public calls with host buffers: H2D, pack, D, unpack, D2H
+    h_in = chi.cpu().pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    d_in, d_out = torch.empty_like(chi), torch.empty_like(chi)
+
+    def e2e():
+        d_in.copy_(h_in, non_blocking=True)
+        for p in (0, 1):
+            ctx.pack_staggered(d_in, p, prec, out=f[p])
+        step()
+        for p in (0, 1):
+            ctx.unpack_staggered(d_out, o[p], p, prec)
+        h_out.copy_(d_out, non_blocking=True)
+    e2e()
+    e2e_steps = 5
+    e2e_ms = max_over_ranks(time_region(e2e, e2e_steps), dev)
+    clocks = sampler.stop() if rank == 0 else None
+    ms_step = ms / args.steps
+    kern_ms = ms / launches
+    achieved = by * Vh / (kern_ms * 1e-3) / 1e9
+    out = {
+        "metric": "staggered_dslash_gflops", "value": whole_job_gflops(flop * V, world, ms_step), "unit": "GFLOP/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if prec == 0 else "f32", "data": "synthetic",
+        "config": {"workload": "32^3x64 improved staggered (asqtad) Dslash, fat + long links, both parities (SURVEY NEXT-3; not the BASELINE metric)",
+                   "precision": args.prec, "flop_per_site": flop, "l2": "inputs larger than L2 (links %d MB per step)" % (16 * 18 * (8 if prec == 0 else 4) * V // 2 // 10 ** 6 * 2 // 2),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": achieved / pk["hbm_gbs"],
+                     "traffic": NCU_TRAFFIC.get(("staggered", args.prec)), "peak_kind": pk_kind, "kernel": "stag_dslash_kernel<%s>" % args.prec,
+                     "algorithmic_bytes_per_launch": by * Vh, "frac_of_8TBs_nominal": achieved / 8000.0},
+        "e2e": {"value": whole_job_gflops(flop * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
+                "h2d_bytes_per_step": V * 3 * 16, "d2h_bytes_per_step": V * 3 * 16, "steps": e2e_steps},
+        "gpu_launches": launches, "clocks": clocks, "cpu_baseline": None,
+    }
+    if rank == 0 and not args.quick:
+        import oracle
+        fn, ln, cn = fat.cpu().numpy(), lng.cpu().numpy(), chi.cpu().numpy()
+        oracle.stag_dslash(cn, fn, ln, BC)
+        t0 = time.time()
+        for _ in range(5):
+            want = oracle.stag_dslash(cn, fn, ln, BC)
+        dt = time.time() - t0
+        out["cpu_baseline"] = {"value": flop * V * 5 / dt / 1e9, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle",
+                               "sample": "5 full-lattice staggered D applications at 32^3x64 in %.1f s (fp64, OpenMP)" % dt}
+        got = torch.zeros_like(chi)
+        for p in (0, 1):
+            ctx.unpack_staggered(got, o[p], p, prec)
+        w = torch.from_numpy(want).to(dev)
+        out["parity_rel_l2_vs_oracle"] = float(torch.linalg.vector_norm(got - w) / torch.linalg.vector_norm(w))
+        ex = {}
+        m = lambda: ctx.staggered_mdagm(o[0], f[0], 0, 0.05, 0.0, prec)
+        for _ in range(3):
+            m()
+        bursts = sorted(time_region(m, 10) / 10.0 for _ in range(5))
+        ex["mdagm_us"] = bursts[2] * 1e3
+        ex["mdagm_gbs"] = (2 * by + 6 * (8 if prec == 0 else 4)) * Vh / (bursts[2] * 1e-3) / 1e9
+        b = chi * torch.from_numpy((inputs.parity_mask(DIMS) == 0)[..., None]).to(dev)
+        sig = [0.0, 0.002, 0.01, 0.05, 0.25, 1.0]
+        x = torch.zeros((len(sig),) + tuple(chi.shape), dtype=torch.complex128, device=dev)
+        for mass in (0.1, 0.02):
+            ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True)
+            infos = min((ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True) for _ in range(2)), key=lambda r: r[0]["seconds"])
+            ex["multishift_mass_%g" % mass] = {
+                "shifts": sig, "tol": 1e-10, "seconds": infos[0]["seconds"], "multishift_iterations_fp32": infos[0]["matpc_precond"],
+                "refinement_iterations": [i["iterations"] for i in infos], "reliable_updates": [i["restarts"] for i in infos],
+                "true_residual_max": max(i["true_residual"] for i in infos), "status": [i["status"] for i in infos],
+                "effective_gflops": infos[0]["gflop"] / infos[0]["seconds"]}
+        out["extra"] = ex
     if rank == 0:
         print(json.dumps(out))
     ctx.close()
