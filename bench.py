@@ -214,6 +214,7 @@ def main():
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
     ap.add_argument("--op", default="dslash", choices=["dslash", "staggered"],
                     help="dslash: the BASELINE metric (Wilson-clover Dslash); staggered: the improved staggered Dslash (SURVEY NEXT-3)")
+    ap.add_argument("--long12", action="store_true", help="--op staggered: long links declared c3 x SU(3) and stored as 12 reals")
     ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"], help="storage precision of the timed Dslash")
     ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8], help="link compression of the timed Dslash")
     ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per launch (>1: lqcd_dslash_mrhs; the BASELINE metric is 1)")
@@ -378,7 +379,7 @@ def run_staggered(args, rank, world, local):
     if args.prec == "half":
         raise SystemExit("staggered fields are fp64 or fp32")
     prec = 0 if args.prec == "fp64" else 1
-    flop, by = 1146, (16 * 18 + 2 * 6) * (8 if prec == 0 else 4)
+    flop, by = 1146, (8 * 18 + 8 * (12 if args.long12 else 18) + 2 * 6) * (8 if prec == 0 else 4)
     # synthetic fat / long links: scaled random SU(3) plus noise (inputs.staggered_links recipe, torch path)
     fat = inputs.random_gauge_torch(DIMS, EPS, 31 + rank, device=dev) * 1.125
     g = torch.Generator(device=dev)
@@ -387,7 +388,8 @@ def run_staggered(args, rank, world, local):
     lng = inputs.random_gauge_torch(DIMS, EPS, 33 + rank, device=dev) * (-1.0 / 24.0)
     chi = torch.view_as_complex(torch.randn((DIMS[3], DIMS[2], DIMS[1], DIMS[0], 3, 2), generator=g, dtype=torch.float64, device=dev) / 2 ** 0.5).contiguous()
     ctx = lqcd.Context(DIMS, BC, local)
-    ctx.load_staggered_links(fat, lng)
+    long_scale = (-1.0 / 24.0) if args.long12 else 0.0
+    ctx.load_staggered_links(fat, lng, long_scale)
     f = [ctx.pack_staggered(chi, p, prec) for p in (0, 1)]
     o = [ctx.new_staggered_field(prec) for _ in (0, 1)]
 
@@ -430,10 +432,10 @@ def run_staggered(args, rank, world, local):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64" if prec == 0 else "f32", "data": "synthetic",
         "config": {"workload": "32^3x64 improved staggered (asqtad) Dslash, fat + long links, both parities (SURVEY NEXT-3; not the BASELINE metric)",
-                   "precision": args.prec, "flop_per_site": flop, "l2": "inputs larger than L2 (links %d MB per step)" % (16 * 18 * (8 if prec == 0 else 4) * V // 2 // 10 ** 6 * 2 // 2),
+                   "precision": args.prec, "long_link_reals": 12 if args.long12 else 18, "flop_per_site": flop, "l2": "inputs larger than L2 (links %d MB per step)" % (16 * 18 * (8 if prec == 0 else 4) * V // 2 // 10 ** 6 * 2 // 2),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": achieved / pk["hbm_gbs"],
-                     "traffic": NCU_TRAFFIC.get(("staggered", args.prec)), "peak_kind": pk_kind, "kernel": "stag_dslash_kernel<%s>" % args.prec,
+                     "traffic": None if args.long12 else NCU_TRAFFIC.get(("staggered", args.prec)), "peak_kind": pk_kind, "kernel": "stag_dslash_kernel<%s>" % args.prec,
                      "algorithmic_bytes_per_launch": by * Vh, "frac_of_8TBs_nominal": achieved / 8000.0},
         "e2e": {"value": whole_job_gflops(flop * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
                 "h2d_bytes_per_step": V * 3 * 16, "d2h_bytes_per_step": V * 3 * 16, "steps": e2e_steps},

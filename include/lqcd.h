@@ -199,7 +199,11 @@ int lqcd_invert_mrhs(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical, 
  * colour vectors chi[t][z][y][x][3].  Packed fields: lqcd_field_bytes(LQCD_FIELD_STAGGERED_PARITY),
  * precisions LQCD_PREC_DOUBLE and LQCD_PREC_SINGLE (half is "not amenable", PAPER.md:298 fn. 3).
  * Every extent must be >= 4 (three-hop term).  Errors as for the Wilson-clover calls. */
-int lqcd_load_staggered_links(lqcd_ctx* ctx, const void* fat_canonical, const void* lng_canonical, void* stream);
+/* long_scale != 0 declares every long link to be long_scale x SU(3) (the three-link Naik term of asqtad is
+ * c3 x a product of three SU(3) links): the library verifies it (LQCD_EINVAL otherwise) and stores 12 reals per
+ * long link, third row = conj(row0 x row1) / long_scale (PAPER.md:164 (a)); long_scale = 0: general 3x3, 18 reals. */
+int lqcd_load_staggered_links(lqcd_ctx* ctx, const void* fat_canonical, const void* lng_canonical, double long_scale,
+                              void* stream);
 int lqcd_pack_staggered(lqcd_ctx* ctx, void* packed, const void* canonical, int parity, int prec, void* stream);
 int lqcd_unpack_staggered(lqcd_ctx* ctx, void* canonical, const void* packed, int parity, int prec, void* stream);
 /* out_p = D_{p,pbar} in_pbar: 16 hops, 1146 flop per site.  out must not alias in. */

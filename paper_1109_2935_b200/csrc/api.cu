@@ -215,9 +215,9 @@ int op_matpc_mrhs(lqcd_ctx* c, char* out, const char* in, int nrhs, int parity, 
   const size_t need = spinor_bytes(prec, c->nat.ns) * (size_t)nrhs;
   if (c->mtmp_bytes < need) {
     if (c->mtmp) cudaFree(c->mtmp);
-  for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfat32, (void*)c->slng32, (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);                   // synchronises: no launch still uses the old buffer
+  for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfatp[0], (void*)c->sfatp[1], (void*)c->slngp[0], (void*)c->slngp[1], (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);                   // synchronises: no launch still uses the old buffer
     c->mtmp = nullptr; c->mtmp_bytes = 0;
-  c->have_stag = false; c->sfat64 = c->slng64 = nullptr; c->sfat32 = c->slng32 = nullptr; c->stmp[0] = c->stmp[1] = nullptr;
+  c->have_stag = false; c->sfat64 = c->slng64 = nullptr; c->sfatp[0] = c->sfatp[1] = c->slngp[0] = c->slngp[1] = nullptr; c->slong_scale = 0; c->stmp[0] = c->stmp[1] = nullptr;
     int rc = dev_alloc(c, (void**)&c->mtmp, need);
     if (rc) return rc;
     c->mtmp_bytes = need;
@@ -263,7 +263,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
   c->have_hpipe = false;
   c->mtmp = nullptr; c->mtmp_bytes = 0;
-  c->have_stag = false; c->sfat64 = c->slng64 = nullptr; c->sfat32 = c->slng32 = nullptr; c->stmp[0] = c->stmp[1] = nullptr;
+  c->have_stag = false; c->sfat64 = c->slng64 = nullptr; c->sfatp[0] = c->sfatp[1] = c->slngp[0] = c->slngp[1] = nullptr; c->slong_scale = 0; c->stmp[0] = c->stmp[1] = nullptr;
   cudaDeviceProp prop;
   cudaGetDeviceProperties(&prop, device);
   c->n_sm = prop.multiProcessorCount;
@@ -296,7 +296,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   for (void* p : c->pool) cudaFree(p);
   for (void* p : c->hws) if (p) cudaFree(p);
   if (c->mtmp) cudaFree(c->mtmp);
-  for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfat32, (void*)c->slng32, (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);
+  for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfatp[0], (void*)c->sfatp[1], (void*)c->slngp[0], (void*)c->slngp[1], (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);
   if (c->have_hpipe) {
     cudaStreamDestroy(c->hs_in); cudaStreamDestroy(c->hs_out); cudaEventDestroy(c->hev_sync);
     for (int i = 0; i < LQ_HOST_SLABS; ++i) { cudaEventDestroy(c->hev_in[i]); cudaEventDestroy(c->hev_out[i]); }

@@ -106,7 +106,8 @@ struct lqcd_ctx {
   // improved staggered path (staggered.cu): fp64 master links, fp32 copies, M^dag M temporaries
   bool have_stag;
   double *sfat64, *slng64;
-  char *sfat32, *slng32;
+  char *sfatp[2], *slngp[2];   // per precision: fat (fp32 copy; fp64 uses the master), long (18 or 12 reals)
+  double slong_scale;          // != 0: every long link is slong_scale x SU(3) and is stored as 12 reals
   char* stmp[2];
   char* mtmp;             // multi-right-hand-side Mhat temporary (grow-only)
   size_t mtmp_bytes;

@@ -45,11 +45,45 @@ cudaError_t run_pack_colour(int prec, char* packed, const double* canonical, con
 }
 
 template <class P>
-cudaError_t launch_stag(const StagArgs& a, bool xpay, cudaStream_t s) {
+cudaError_t launch_stag(const StagArgs& a, bool xpay, bool long12, cudaStream_t s) {
   dim3 grid((a.g.vh + LQ_STAG_BLOCK - 1) / LQ_STAG_BLOCK), block(LQ_STAG_BLOCK);
-  if (xpay) stag_dslash_kernel<P, true><<<grid, block, 0, s>>>(a);
-  else stag_dslash_kernel<P, false><<<grid, block, 0, s>>>(a);
+  if (long12) {
+    if (xpay) stag_dslash_kernel<P, true, 12><<<grid, block, 0, s>>>(a);
+    else stag_dslash_kernel<P, false, 12><<<grid, block, 0, s>>>(a);
+  } else {
+    if (xpay) stag_dslash_kernel<P, true, 18><<<grid, block, 0, s>>>(a);
+    else stag_dslash_kernel<P, false, 18><<<grid, block, 0, s>>>(a);
+  }
   return cudaGetLastError();
+}
+
+// max over links of || L L^dag / scale^2 - 1 ||_max and |det L / scale^3 - 1| : is every long link scale x SU(3)?
+__global__ void long_link_check_kernel(const double* __restrict__ lng, long long nlinks, double inv2, double inv3, double* out) {
+  double worst = 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nlinks; i += (long long)gridDim.x * blockDim.x) {
+    const double* u = lng + i * 18;
+    for (int r = 0; r < 3; ++r)
+      for (int q = 0; q < 3; ++q) {
+        double re = 0, im = 0;
+        for (int k = 0; k < 3; ++k) {
+          re += u[6 * r + 2 * k] * u[6 * q + 2 * k] + u[6 * r + 2 * k + 1] * u[6 * q + 2 * k + 1];
+          im += u[6 * r + 2 * k + 1] * u[6 * q + 2 * k] - u[6 * r + 2 * k] * u[6 * q + 2 * k + 1];
+        }
+        worst = fmax(worst, fmax(fabs(re * inv2 - (r == q ? 1.0 : 0.0)), fabs(im * inv2)));
+      }
+    // det L = scale^3 (row 2 = conj(row0 x row1) / scale needs det = 1 as well as unitarity)
+    double dr = 0, di = 0;
+    for (int c0 = 0; c0 < 3; ++c0) {
+      const int j = (c0 + 1) % 3, k = (c0 + 2) % 3;
+      const double cr = u[6 + 2 * j] * u[12 + 2 * k] - u[6 + 2 * j + 1] * u[12 + 2 * k + 1] - u[6 + 2 * k] * u[12 + 2 * j] + u[6 + 2 * k + 1] * u[12 + 2 * j + 1];
+      const double ci = u[6 + 2 * j] * u[12 + 2 * k + 1] + u[6 + 2 * j + 1] * u[12 + 2 * k] - u[6 + 2 * k] * u[12 + 2 * j + 1] - u[6 + 2 * k + 1] * u[12 + 2 * j];
+      dr += u[2 * c0] * cr - u[2 * c0 + 1] * ci;
+      di += u[2 * c0] * ci + u[2 * c0 + 1] * cr;
+    }
+    worst = fmax(worst, fmax(fabs(dr * inv3 - 1.0), fabs(di * inv3)));
+  }
+  for (int o = 16; o > 0; o >>= 1) worst = fmax(worst, __shfl_down_sync(0xffffffffu, worst, o));
+  if ((threadIdx.x & 31) == 0 && worst > 0) atomicMax((unsigned long long*)out, (unsigned long long)__double_as_longlong(worst));
 }
 
 size_t colour_bytes(int prec, long long vh) { return (size_t)vh * 6 * (prec == 0 ? 8 : 4); }
@@ -61,17 +95,24 @@ int stag_check(lqcd_ctx* c, int prec) {
 }
 
 // fp64 masters -> links of precision prec (recon-18 records), on first use
+// (the long links are 12-real records when the caller declared them long_scale x SU(3))
 int stag_links(lqcd_ctx* c, int prec, const char** fat, const char** lng, cudaStream_t s) {
-  if (prec == 0) { *fat = (const char*)c->sfat64; *lng = (const char*)c->slng64; return LQCD_OK; }
-  if (!c->sfat32) {
-    int rc = dev_alloc(c, (void**)&c->sfat32, gauge_bytes(1, 18, c->nat.ns));
-    if (!rc) rc = dev_alloc(c, (void**)&c->slng32, gauge_bytes(1, 18, c->nat.ns));
+  const int lr = c->slong_scale != 0.0 ? 12 : 18;
+  if (prec == 0 && lr == 18) { *fat = (const char*)c->sfat64; *lng = (const char*)c->slng64; return LQCD_OK; }
+  char*& f = c->sfatp[prec];
+  char*& l = c->slngp[prec];
+  if (!l) {
+    int rc = LQCD_OK;
+    if (prec == 1) rc = dev_alloc(c, (void**)&f, gauge_bytes(1, 18, c->nat.ns));
+    if (!rc) rc = dev_alloc(c, (void**)&l, gauge_bytes(prec, lr, c->nat.ns));
     if (rc) return rc;
-    cudaError_t e = run_convert_gauge(1, 18, c->sfat32, c->sfat64, c->bm, 0, s); c->launches++;
-    if (e == cudaSuccess) { e = run_convert_gauge(1, 18, c->slng32, c->slng64, c->bm, 0, s); c->launches++; }
+    cudaError_t e = cudaSuccess;
+    if (prec == 1) { e = run_convert_gauge(1, 18, f, c->sfat64, c->bm, 0, s); c->launches++; }
+    if (e == cudaSuccess) { e = run_convert_gauge(prec, lr, l, c->slng64, c->bm, 0, s); c->launches++; }
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "convert staggered links", e);
   }
-  *fat = c->sfat32; *lng = c->slng32;
+  *fat = prec == 0 ? (const char*)c->sfat64 : f;
+  *lng = l;
   return LQCD_OK;
 }
 
@@ -83,7 +124,9 @@ int op_stag_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, double
   d.out = out; d.in = in; d.y = y; d.a = a; d.b = b; d.parity = p;
   int rc = stag_links(c, prec, &d.fat, &d.lng, s);
   if (rc) return rc;
-  cudaError_t e = prec == 0 ? launch_stag<PrecD>(d, y != nullptr, s) : launch_stag<PrecS>(d, y != nullptr, s);
+  const bool l12 = c->slong_scale != 0.0;
+  d.linv = l12 ? 1.0 / c->slong_scale : 0.0;
+  cudaError_t e = prec == 0 ? launch_stag<PrecD>(d, y != nullptr, l12, s) : launch_stag<PrecS>(d, y != nullptr, l12, s);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "staggered dslash launch", e);
 }
@@ -176,7 +219,7 @@ int sresidual(lqcd_ctx* c, char* r, const char* b, const char* x, int par, doubl
 // ================================================================================================
 extern "C" {
 
-int lqcd_load_staggered_links(lqcd_ctx* c, const void* fat, const void* lng, void* stream) {
+int lqcd_load_staggered_links(lqcd_ctx* c, const void* fat, const void* lng, double long_scale, void* stream) {
   if (!c) return LQCD_EINVAL;
   if (!fat || !lng) return fail(c, LQCD_EINVAL, "null link pointer");
   for (int m = 0; m < 4; ++m) if (c->dims[m] < 4) return fail(c, LQCD_EINVAL, "the three-hop term needs every extent >= 4");
@@ -185,11 +228,27 @@ int lqcd_load_staggered_links(lqcd_ctx* c, const void* fat, const void* lng, voi
   int rc;
   if (!c->sfat64 && (rc = dev_alloc(c, (void**)&c->sfat64, gauge_bytes(0, 18, c->nat.ns)))) return rc;
   if (!c->slng64 && (rc = dev_alloc(c, (void**)&c->slng64, gauge_bytes(0, 18, c->nat.ns)))) return rc;
-  if (c->sfat32) { cudaFree(c->sfat32); c->sfat32 = nullptr; }
-  if (c->slng32) { cudaFree(c->slng32); c->slng32 = nullptr; }
+  for (int i = 0; i < 2; ++i) {
+    if (c->sfatp[i]) { cudaFree(c->sfatp[i]); c->sfatp[i] = nullptr; }
+    if (c->slngp[i]) { cudaFree(c->slngp[i]); c->slngp[i] = nullptr; }
+  }
+  c->have_stag = false;
+  if (long_scale != 0.0) {
+    // the caller says every long link is long_scale x SU(3): check it before trusting a 12-real encoding
+    cudaError_t e = cudaMemsetAsync(c->S + S_OUT, 0, sizeof(double), s);
+    if (e == cudaSuccess) {
+      long_link_check_kernel<<<c->n_sm * 4, 256, 0, s>>>((const double*)lng, 4 * c->V, 1.0 / (long_scale * long_scale), 1.0 / (long_scale * long_scale * long_scale), c->S + S_OUT);
+      c->launches++;
+      e = cudaMemcpyAsync(c->hS + S_OUT, c->S + S_OUT, sizeof(double), cudaMemcpyDeviceToHost, s);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "long link check", e);
+    if (!(c->hS[S_OUT] <= 1e-10)) return fail(c, LQCD_EINVAL, "long links are not long_scale x SU(3); pass long_scale = 0");
+  }
   cudaError_t e = run_pack_gauge(c->sfat64, (const double*)fat, c->nat, s); c->launches++;
   if (e == cudaSuccess) { e = run_pack_gauge(c->slng64, (const double*)lng, c->nat, s); c->launches++; }
   if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack staggered links", e);
+  c->slong_scale = long_scale;
   c->have_stag = true;
   return LQCD_OK;
 }

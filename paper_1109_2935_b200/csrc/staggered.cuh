@@ -16,7 +16,8 @@
 // (fp64) or 8-byte (fp32) loads; a warp's loads cover whole 128-byte lines.
 //
 // One thread per output site, 16 hops, each link read exactly once per application: compulsory
-// bytes per site = 16 links + 2 vectors = 16*72 + 48 = 1200 B in fp32 (2400 B in fp64), 1146 flop
+// bytes per site = 16 links + 2 vectors = 16*72 + 48 = 1200 B in fp32 (2400 B in fp64; 1008 / 2016 B when the long
+// links are stored as 12 reals), 1146 flop
 // (16 x 66 for the 3x3 complex matvecs + 15 x 6 adds): HBM-bound at ~1 flop/byte.
 #pragma once
 #include "core.cuh"
@@ -31,6 +32,7 @@ struct StagArgs {
   const char* fat;      // [parity][mu] x 18 reals
   const char* lng;
   double a, b;          // XPAY: out = a*y + b*(D in); else out = D in
+  double linv;          // LRECON == 12: 1 / long_scale (third row of a long link = conj(row0 x row1) * linv)
   int parity;           // output parity
 };
 
@@ -87,7 +89,30 @@ LQ_DEV void su3_mac(R* __restrict__ acc, const R* __restrict__ u, const R* __res
 
 #define LQ_STAG_BLOCK 128
 
-template <class P, bool XPAY>
+// 18 reals of a link: as stored (N == 18), or rows 0,1 stored and row 2 = conj(row0 x row1) * linv (N == 12;
+// long links that are long_scale x SU(3), as the three-link Naik term of asqtad is: PAPER.md:164 (a), :122)
+template <typename R, int N>
+LQ_DEV void load_stag_link(R* __restrict__ u, const char* __restrict__ f, long long ns, long long i, R linv) {
+  Rec<R, N>::template load<LQ_GAUGE_STREAM>(u, f, ns, i);
+  if constexpr (N == 12) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int j = (c + 1) % 3, k = (c + 2) % 3;
+      R re = u[2 * j] * u[6 + 2 * k];
+      re = fma_(-u[2 * j + 1], u[6 + 2 * k + 1], re);
+      re = fma_(-u[2 * k], u[6 + 2 * j], re);
+      re = fma_(u[2 * k + 1], u[6 + 2 * j + 1], re);
+      R im = u[2 * k] * u[6 + 2 * j + 1];
+      im = fma_(u[2 * k + 1], u[6 + 2 * j], im);
+      im = fma_(-u[2 * j], u[6 + 2 * k + 1], im);
+      im = fma_(-u[2 * j + 1], u[6 + 2 * k], im);
+      u[12 + 2 * c] = re * linv;
+      u[12 + 2 * c + 1] = im * linv;
+    }
+  }
+}
+
+template <class P, bool XPAY, int LRECON>
 __global__ void __launch_bounds__(LQ_STAG_BLOCK) stag_dslash_kernel(const StagArgs a) {
   typedef typename P::real R;
   const Geom& g = a.g;
@@ -97,7 +122,8 @@ __global__ void __launch_bounds__(LQ_STAG_BLOCK) stag_dslash_kernel(const StagAr
   const long long ns4 = g.ns >> 2;
   int c[4];
   cb_to_coords(g, cb, p, c);
-  const long long link_bytes = 18ll * sizeof(R) * g.ns;
+  const long long fat_bytes = 18ll * sizeof(R) * g.ns, lng_bytes = (long long)LRECON * sizeof(R) * g.ns;
+  const R linv = (R)a.linv;
   R acc[6] = {0, 0, 0, 0, 0, 0};
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
@@ -109,6 +135,7 @@ __global__ void __launch_bounds__(LQ_STAG_BLOCK) stag_dslash_kernel(const StagAr
     for (int kind = 0; kind < 2; ++kind) {               // 0: fat link, one hop; 1: long link, three hops
       const int step = kind ? 3 : 1;
       const char* links = kind ? a.lng : a.fat;
+      const long long link_bytes = kind ? lng_bytes : fat_bytes;
       int d[4] = {c[0], c[1], c[2], c[3]};
       {                                                   // forward: link of this site, chi(x + step mu)
         int v = c[mu] + step;
@@ -117,7 +144,8 @@ __global__ void __launch_bounds__(LQ_STAG_BLOCK) stag_dslash_kernel(const StagAr
         d[mu] = v;
         const int nb = coords_to_cb(g, d);
         R u[18], chi[6];
-        Rec<R, 18>::template load<LQ_GAUGE_STREAM>(u, links + (long long)(p * 4 + mu) * link_bytes, g.ns, cb);
+        if (kind) load_stag_link<R, LRECON>(u, links + (long long)(p * 4 + mu) * link_bytes, g.ns, cb, linv);
+        else load_stag_link<R, 18>(u, links + (long long)(p * 4 + mu) * link_bytes, g.ns, cb, linv);
         Colour<P>::load(chi, a.in, ns4, nb);
         su3_mac<true, R>(acc, u, chi, sg);
       }
@@ -128,7 +156,8 @@ __global__ void __launch_bounds__(LQ_STAG_BLOCK) stag_dslash_kernel(const StagAr
         d[mu] = v;
         const int nb = coords_to_cb(g, d);
         R u[18], chi[6];
-        Rec<R, 18>::template load<LQ_GAUGE_STREAM>(u, links + (long long)((1 - p) * 4 + mu) * link_bytes, g.ns, nb);
+        if (kind) load_stag_link<R, LRECON>(u, links + (long long)((1 - p) * 4 + mu) * link_bytes, g.ns, nb, linv);
+        else load_stag_link<R, 18>(u, links + (long long)((1 - p) * 4 + mu) * link_bytes, g.ns, nb, linv);
         Colour<P>::load(chi, a.in, ns4, nb);
         su3_mac<false, R>(acc, u, chi, sg);
       }

@@ -95,7 +95,7 @@ def load_library():
             "lqcd_axpy_norm": (i, [vp, d, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_cdot": (i, [vp, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_launch_count": (ctypes.c_longlong, [vp]),
-            "lqcd_load_staggered_links": (i, [vp, vp, vp, vp]),
+            "lqcd_load_staggered_links": (i, [vp, vp, vp, d, vp]),
             "lqcd_pack_staggered": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_unpack_staggered": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_staggered_dslash": (i, [vp, vp, vp, i, i, vp]),
@@ -210,10 +210,11 @@ class Context:
         return out
 
     # -- improved staggered ------------------------------------------------------------------------
-    def load_staggered_links(self, fat, lng):
+    def load_staggered_links(self, fat, lng, long_scale=0.0):
+        """long_scale != 0: every long link is long_scale x SU(3) (checked) and is stored as 12 reals."""
         for t in (fat, lng):
             assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()
-        self._check(self.lib.lqcd_load_staggered_links(self.h, _ptr(fat), _ptr(lng), _stream()))
+        self._check(self.lib.lqcd_load_staggered_links(self.h, _ptr(fat), _ptr(lng), float(long_scale), _stream()))
 
     def new_staggered_field(self, prec):
         return torch.empty(self.lib.lqcd_field_bytes(self.h, FIELD_STAGGERED_PARITY, prec), dtype=torch.uint8, device=self.device)

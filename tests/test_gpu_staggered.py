@@ -17,7 +17,7 @@ def _rel(a, b):
 
 
 class SCase:
-    def __init__(self, dims, eps, bc, seed=1, unit=False):
+    def __init__(self, dims, eps, bc, seed=1, unit=False, long_scale=0.0):
         from paper_1109_2935_b200 import lqcd
         self.lqcd, self.dims, self.bc = lqcd, dims, bc
         if unit:
@@ -26,7 +26,7 @@ class SCase:
         else:
             self.fat, self.lng = inputs.staggered_links(dims, eps, seed)
         self.ctx = lqcd.Context(dims, bc, 0)
-        self.ctx.load_staggered_links(torch.from_numpy(self.fat).cuda(), torch.from_numpy(self.lng).cuda())
+        self.ctx.load_staggered_links(torch.from_numpy(self.fat).cuda(), torch.from_numpy(self.lng).cuda(), long_scale)
         self.par = inputs.parity_mask(dims)
 
     def mask(self, p):
@@ -151,3 +151,29 @@ def test_multishift_edges(ragged):
     # iteration cap
     infos = c.ctx.staggered_multishift(x, b, 0, 0.01, [0.0, 0.5], 1e-12, max_iter=3, allow_fail=True)
     assert infos[0]["status"] == lq.ENOCONV and 0 < infos[0]["true_residual"] < 1.0
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_long_links_stored_as_12_reals(prec):
+    """long_scale = c3 declares the long links c3 x SU(3): 12 reals per long link, third row reconstructed.
+    Same operator as the 18-real storage, against the oracle; a field that is not c3 x SU(3) is refused."""
+    dims, bc = (6, 4, 10, 12), (-1, 1, 1, -1)
+    c = SCase(dims, 0.4, bc, long_scale=-1.0 / 24.0)
+    chi = inputs.gaussian_colour_vector(dims, 3)
+    for p in (0, 1):
+        want = oracle.stag_dslash(chi * c.mask(1 - p), c.fat, c.lng, c.bc) * c.mask(p)
+        got = c.op(lambda o, i: c.ctx.staggered_dslash(o, i, p, prec), chi, 1 - p, p, prec)
+        assert _rel(got, want) <= STOL[prec]
+        want = oracle.stag_MdagM(chi * c.mask(p), c.fat, c.lng, c.bc, 0.1, 0.3) * c.mask(p)
+        got = c.op(lambda o, i: c.ctx.staggered_mdagm(o, i, p, 0.1, 0.3, prec), chi, p, p, prec)
+        assert _rel(got, want) <= STOL[prec]
+    lq = c.lqcd
+    fat, lng = torch.from_numpy(c.fat).cuda(), torch.from_numpy(c.lng).cuda()
+    for bad_lng, scale in ((lng, -1.0 / 20.0), (fat, 1.125), (lng * np.exp(0.3j), -1.0 / 24.0)):   # wrong scale / not unitary / det != 1
+        with pytest.raises(lq.LqcdError) as e:
+            c.ctx.load_staggered_links(fat, bad_lng.contiguous(), scale)
+        assert e.value.code == lq.EINVAL
+    with pytest.raises(lq.LqcdError) as e:
+        c.ctx.staggered_dslash(c.ctx.new_staggered_field(1), c.ctx.new_staggered_field(1), 0, 1)      # a refused load leaves no links
+    assert e.value.code == lq.ESTATE
+    c.ctx.close()
