@@ -177,3 +177,61 @@ def test_long_links_stored_as_12_reals(prec):
         c.ctx.staggered_dslash(c.ctx.new_staggered_field(1), c.ctx.new_staggered_field(1), 0, 1)      # a refused load leaves no links
     assert e.value.code == lq.ESTATE
     c.ctx.close()
+
+
+def test_extent_four_three_hop_wraps_to_the_backward_neighbour():
+    """L_mu = 4: x + 3 mu and x - mu are the same site (and x - 3 mu = x + mu), reached once through the long
+    link with the wrap's boundary sign and once through the fat link; every hop of a 4^4 lattice wraps
+    somewhere.  Operator and a full multi-shift solve against the oracle."""
+    dims, bc = (4, 4, 4, 4), (-1, 1, -1, -1)
+    c = SCase(dims, 0.5, bc, seed=9)
+    chi = inputs.gaussian_colour_vector(dims, 3)
+    for prec in (0, 1):
+        for p in (0, 1):
+            want = oracle.stag_dslash(chi * c.mask(1 - p), c.fat, c.lng, c.bc) * c.mask(p)
+            got = c.op(lambda o, i: c.ctx.staggered_dslash(o, i, p, prec), chi, 1 - p, p, prec)
+            assert _rel(got, want) <= STOL[prec]
+    b = chi * c.mask(1)
+    sig = [0.0, 0.3]
+    x = torch.zeros((2,) + b.shape, dtype=torch.complex128, device="cuda")
+    infos = c.ctx.staggered_multishift(x, torch.from_numpy(b).cuda(), 1, 0.1, sig, 1e-11)
+    for i, sg in enumerate(sig):
+        xo, _ = oracle.stag_cg(b, c.fat, c.lng, c.bc, 0.1, sg, tol=1e-13)
+        assert infos[i]["status"] == 0 and _rel(x[i].cpu().numpy(), xo) <= 1e-9
+    c.ctx.close()
+
+
+def test_full_size_32x64_operator_and_solve():
+    """32^3x64 (the size bench.py --op staggered times): Dslash fp32/fp64 with 18- and 12-real long links
+    against the oracle on the full lattice, and a 3-shift solve whose true residuals are recomputed by
+    the oracle's operator."""
+    from paper_1109_2935_b200 import lqcd
+    dims, bc = (32, 32, 32, 64), (1, 1, 1, -1)
+    fat = (inputs.random_gauge_torch(dims, 0.3, 31, device="cuda") * 1.125).contiguous()
+    lng = (inputs.random_gauge_torch(dims, 0.3, 33, device="cuda") * (-1.0 / 24.0)).contiguous()
+    g = torch.Generator(device="cuda")
+    g.manual_seed(5)
+    chi = torch.view_as_complex(torch.randn((64, 32, 32, 32, 3, 2), generator=g, dtype=torch.float64, device="cuda")).contiguous()
+    fn, ln, cn = fat.cpu().numpy(), lng.cpu().numpy(), chi.cpu().numpy()
+    want = torch.from_numpy(oracle.stag_dslash(cn, fn, ln, bc)).cuda()
+    ctx = lqcd.Context(dims, bc, 0)
+    for long_scale in (0.0, -1.0 / 24.0):
+        ctx.load_staggered_links(fat, lng, long_scale)
+        for prec in (0, 1):
+            got = torch.zeros_like(chi)
+            for p in (0, 1):
+                o = ctx.new_staggered_field(prec)
+                ctx.staggered_dslash(o, ctx.pack_staggered(chi, 1 - p, prec), p, prec)
+                ctx.unpack_staggered(got, o, p, prec)
+            err = float(torch.linalg.vector_norm(got - want) / torch.linalg.vector_norm(want))
+            assert err <= STOL[prec], (long_scale, prec, err)
+    par = torch.from_numpy(inputs.parity_mask(dims) == 0).cuda()[..., None]
+    b = (chi * par).contiguous()
+    sig, mass, tol = [0.0, 0.02, 0.5], 0.05, 1e-10
+    x = torch.zeros((3,) + tuple(chi.shape), dtype=torch.complex128, device="cuda")
+    infos = ctx.staggered_multishift(x, b, 0, mass, sig, tol)
+    bn = b.cpu().numpy()
+    for i, sg in enumerate(sig):
+        res = np.linalg.norm(bn - oracle.stag_MdagM(x[i].cpu().numpy(), fn, ln, bc, mass, sg)) / np.linalg.norm(bn)
+        assert infos[i]["status"] == 0 and res <= 1.05 * tol, (i, res)
+    ctx.close()
