@@ -22,7 +22,10 @@ static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
   constexpr int NST = sizeof(typename P::real) == 8 ? ((CLOVX || CLOVOUT) ? 0 : LQ_PIPE_FP64) : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
   constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
   auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST>;
-  static bool configured = false;         // per instantiation
+  static bool configured_dev[64] = {};    // per instantiation and device (function attributes are per device)
+  int dev = 0;
+  cudaGetDevice(&dev);
+  bool& configured = configured_dev[dev & 63];
   if (!configured) {
     if (NST > 0) {
       cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
