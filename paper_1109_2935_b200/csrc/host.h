@@ -7,7 +7,9 @@
 #include "blas.cuh"
 #include "../../include/lqcd.h"
 
+#ifndef LQ_HOST_SLABS
 #define LQ_HOST_SLABS 16    /* max t-slabs of the host-buffer pipeline (host_api.cu) */
+#endif
 
 namespace lq {
 
