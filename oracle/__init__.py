@@ -25,7 +25,7 @@ _LIB_S = os.path.join(_HERE, "liboracle_staggered.so")
 _lib = None
 _lib_s = None
 
-BICGSTAB, GCR_DD, CGNR = 0, 1, 2
+BICGSTAB, GCR_DD, CGNR, CGNE = 0, 1, 2, 3
 
 
 def build(force=False):

@@ -416,6 +416,36 @@ int cgnr(cplx* x, const cplx* bhat, const Op& op, int p, double stop, int maxit,
   return status;
 }
 
+// CGNE (Craig's method): CG on Mhat Mhat^dag y = bhat with x = Mhat^dag y carried directly (PAPER.md:128,
+// "CGNE or CGNR").  r = bhat - Mhat x;  p = Mhat^dag r;  repeat { alpha = <r,r>/<p,p>; x += alpha p;
+// r -= alpha Mhat p; beta = <r',r'>/<r,r>; p = Mhat^dag r' + beta p }.  Stops when ||r|| <= stop (absolute).
+int cgne(cplx* x, const cplx* bhat, const Op& op, int p, double stop, int maxit, int* iters, double* rnorm) {
+  const long n = op.n();
+  std::vector<cplx> r(n), z(n), pv(n), w(n);
+  apply_matpc(r.data(), x, op, p, 0);
+  for (long i = 0; i < n; ++i) r[i] = bhat[i] - r[i];
+  mask_parity(r.data(), op.lat, p);
+  apply_matpc(pv.data(), r.data(), op, p, 1);
+  double rr = norm2(r.data(), n);
+  int it = 0, status = 0;
+  while (std::sqrt(rr) > stop) {
+    if (it >= maxit) { status = 1; break; }
+    const double pp = norm2(pv.data(), n);
+    if (pp == 0.0) { status = 2; break; }
+    const double alpha = rr / pp;
+    apply_matpc(w.data(), pv.data(), op, p, 0);
+    for (long i = 0; i < n; ++i) { x[i] += alpha * pv[i]; r[i] -= alpha * w[i]; }
+    const double rr1 = norm2(r.data(), n);
+    const double beta = rr1 / rr;
+    apply_matpc(z.data(), r.data(), op, p, 1);
+    for (long i = 0; i < n; ++i) pv[i] = z[i] + beta * pv[i];
+    rr = rr1;
+    ++it;
+  }
+  *iters = it; *rnorm = std::sqrt(rr);
+  return status;
+}
+
 // c.8  Schwarz preconditioner K: n_mr MR steps on Mhat_D from x = 0,
 // one alpha per block, sums over the block's parity-p sites.
 void schwarz_K(cplx* out, const cplx* rin, const Op& opD, int p, int n_mr, double omega_mr) {
@@ -638,7 +668,7 @@ int orc_invert_sym(cplx* x, const cplx* b, const cplx* U, const cplx* T, const i
 }
 
 // Full solve of M x = b (Eq. 1): prepare -> parity solve -> reconstruct.
-// solver: 0 BiCGstab, 1 GCR-DD, 2 CGNR.  Stops on ||bhat - Mhat x_p|| <= tol*||b||  (= ||b - M x||, c.5).
+// solver: 0 BiCGstab, 1 GCR-DD, 2 CGNR, 3 CGNE.  Stops on ||bhat - Mhat x_p|| <= tol*||b||  (= ||b - M x||, c.5).
 int orc_invert(cplx* x, const cplx* b, const cplx* U, const cplx* T, const int* dims, const int* bc,
                double kappa, int parity, double tol, int maxit, int solver,
                int kmax, double delta, const int* block, int n_mr, double omega_mr,
@@ -651,6 +681,7 @@ int orc_invert(cplx* x, const cplx* b, const cplx* U, const cplx* T, const int* 
   int restarts = 0; double rn = 0; int st;
   if (solver == 0) st = bicgstab(xp.data(), bhat.data(), op, parity, tol * bn, maxit, iters, &rn);
   else if (solver == 2) st = cgnr(xp.data(), bhat.data(), op, parity, tol * bn, maxit, iters, &rn);
+  else if (solver == 3) st = cgne(xp.data(), bhat.data(), op, parity, tol * bn, maxit, iters, &rn);
   else {
     Op opD(U, T, dims, bc, kappa, block);
     st = gcr_dd(xp.data(), bhat.data(), op, opD, parity, tol * bn, maxit, kmax, delta, 1, n_mr, omega_mr, iters, &restarts, &rn);

@@ -336,6 +336,25 @@ def test_dense_lu_cgnr(four):
     assert abs(rnorm.value - stop3) <= 1e-12 * stop3
 
 
+def test_dense_lu_cgne(four):
+    """CGNE / Craig's method: dense-LU solution on both parities; its iterates minimise the
+    ERROR over the Krylov space of Mhat^dag (Mhat Mhat^dag)^k r0, so the error norm against the dense solution
+    decreases monotonically (the residual need not) -- checked on the first 12 iterations."""
+    dims, U, Tcl, b, kappa = four
+    Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
+    x_lu = np.linalg.solve(Md, b.ravel()).reshape(b.shape)
+    for parity in (0, 1):
+        x, info = oracle.invert(b, U, Tcl, BC, kappa, parity=parity, tol=1e-12, solver=oracle.CGNE)
+        assert info["status"] == 0 and info["true_residual"] < 2e-12
+        assert _rel(x, x_lu) < 1e-10
+    errs = []
+    for k in range(1, 13):
+        x, info = oracle.invert(b, U, Tcl, BC, kappa, parity=0, tol=1e-30, maxit=k, solver=oracle.CGNE)
+        assert info["iterations"] == k
+        errs.append(np.linalg.norm((x - x_lu)[inputs.parity_mask(dims) == 0]))
+    assert all(e1 < e0 for e0, e1 in zip(errs, errs[1:]))
+
+
 def test_symmetric_even_odd_form(four):
     """Mhat_s = A_pp^-1 Mhat as dense matrices; the dagger flag is the true adjoint; solving through the
     symmetric system gives the dense-LU solution of M x = b with the full-system criterion met."""
