@@ -65,6 +65,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 
 #define LQCD_SOLVER_BICGSTAB 0
 #define LQCD_SOLVER_GCR_DD   1
+#define LQCD_SOLVER_CGNE     3   /* Craig's method: CG on Mhat Mhat^dag y = bhat, x = Mhat^dag y */
 #define LQCD_SOLVER_CGNR     2   /* CG on Mhat^dag Mhat x = Mhat^dag bhat, mixed precision, reliable updates */
 
 #define LQCD_MATPC_ASYMMETRIC 0
@@ -159,7 +160,7 @@ typedef struct {
   int    precondition;    /* GCR: 1 = Schwarz/MR preconditioner, 0 = plain GCR */
   int    matpc_type;      /* LQCD_MATPC_ASYMMETRIC (default, R6) or LQCD_MATPC_SYMMETRIC: the Krylov iteration runs on
                              Mhat_s x_p = A_pp^-1 bhat; the stopping test stays ||b - M x|| <= tol ||b|| (fp64, at
-                             reliable updates).  BiCGstab and CGNR only. */
+                             reliable updates).  BiCGstab, CGNR and CGNE only. */
 } lqcd_invert_params;
 
 typedef struct {

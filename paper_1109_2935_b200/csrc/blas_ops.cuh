@@ -185,6 +185,7 @@ struct OpBicgXR {          // v0 = x, v1 = p, v2 = s->r, v3 = t, v4 = rtilde
 // Device scalars: zz = <z,z> in S_RHO, alpha in S_ALPHA, beta in S_BETA (all real), rr in S_RR.
 struct OpCgInit {          // v0 = z, v1 = p : p = z ; zz = ||z||^2          (start, i0 = 0)
   //                          i0 = 1 (after a reliable update): beta = ||z||^2 / zz_old ; p = z + beta p is done by OpCgP
+  //                          i0 = 2: the same when S_RHO and beta were already advanced by OpCgXRB (CGNE, plain CG)
   static constexpr int NV = 1, READ = 1, WRITE = 0;
   typedef NoCoef Coef;
   LQ_DEV static void prepare(Coef&, const BlasArgs&, int) {}
@@ -192,8 +193,9 @@ struct OpCgInit {          // v0 = z, v1 = p : p = z ; zz = ||z||^2          (st
   LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
     double* S = a.S;
     if (a.i0 == 0) { S[S_BETA] = 0; S[S_FLAG] = 0; }
-    else S[S_BETA] = (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;
-    S[S_RHO] = s[0];
+    else if (a.i0 == 1) S[S_BETA] = (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;
+    else S[S_BETA] *= (S[S_RHO] > 0.0) ? s[0] / S[S_RHO] : 0.0;     // i0 == 2: the residual whose norm gave beta (OpCgXRB:
+    S[S_RHO] = s[0];                                                  // beta = rr'/rr, S_RHO = rr') was replaced: beta = rr_new/rr
   }
 };
 

@@ -310,6 +310,100 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
   return status;
 }
 
+// ---------------------------------------------------------------- CGNE (Craig's method) with reliable updates
+// CG on Mhat Mhat^dag y = bhat with x = Mhat^dag y carried directly ("CGNE or CGNR"):
+// alpha = <r,r>/<p,p>; x += alpha p; r -= alpha Mhat p; beta = <r',r'>/<r,r>; p = Mhat^dag r' + beta p.
+// Minimises the error instead of the residual.  Same precision scheme and BLAS-1 passes as CGNR.
+int solve_cgne(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
+               lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
+  const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
+  const long long ns = c->nat.ns;
+  Work wk(c);
+  char *r_hi, *xl, *rl, *z, *pv, *w;
+  int rc;
+  if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
+  char** lo[] = {&xl, &rl, &z, &pv, &w};
+  for (char** q : lo) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
+  const int sym = p.matpc_type == LQCD_MATPC_SYMMETRIC;
+  double rn, rin, istop = stop;
+  auto true_residual = [&]() -> int {      // as in solve_bicgstab
+    int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
+    if (rc2) return rc2;
+    cnt.mat_outer++;
+    rin = rn;
+    if (sym && rn > stop) {
+      if ((rc2 = to_symmetric_residual(c, r_hi, par, p.kappa, po, &rin, s))) return rc2;
+      istop = stop * (rin / rn);
+    }
+    return LQCD_OK;
+  };
+  if ((rc = true_residual())) return rc;
+  res->iterations = 0; res->restarts = 0;
+  const double delta = p.delta > 0 ? p.delta : 0.1;
+  int status = LQCD_OK;
+  auto fold = [&]() -> int {
+    MultiArgs m; memset(&m, 0, sizeof(m));
+    m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
+    cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+    BlasArgs a = mk(c, false, xl);
+    return blas<OpZero>(c, ps, a, s);
+  };
+  // (re)start or continue the direction from the low-precision residual r_l: rr (and beta) on the device,
+  // z = Mhat^dag r_l, p = z + beta p.   keep = 0: beta = 0
+  auto direction = [&](int keep) -> int {
+    BlasArgs a = mk(c, false, rl); a.i0 = keep;
+    int rc2 = blas<OpCgInit>(c, ps, a, s);
+    if (rc2) return rc2;
+    if ((rc2 = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc2;
+    cnt.mat_sloppy++;
+    BlasArgs a2 = mk(c, false, pv, z);
+    return blas<OpCgP>(c, ps, a2, s);
+  };
+  if (rn > stop) {
+    if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+    for (char* q : {xl, pv}) { BlasArgs a = mk(c, false, q); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+    if ((rc = direction(0))) return rc;
+    double maxr = rin;
+    int it = 0;
+    while (true) {
+      if (it >= p.max_iter) { if ((rc = fold())) return rc; status = LQCD_ENOCONV; break; }
+      { BlasArgs a = mk(c, false, pv); if ((rc = blas<OpCgAlpha>(c, ps, a, s))) return rc; }          // alpha = rr / ||p||^2
+      if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
+      { BlasArgs a = mk(c, false, xl, pv, rl, w); if ((rc = blas<OpCgXRB>(c, ps, a, s))) return rc; }   // x, r, rr', beta
+      cnt.mat_sloppy++; cnt.blas_flop_sites += 24.0 * (2 + 4 + 2); ++it;
+      if ((rc = read_S(c, S_RR, 2, s))) return rc;
+      const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
+      const bool bad = !(rr == rr) || flag != 0.0;
+      const double rln = sqrt(rr);
+      if (rln > maxr) maxr = rln;
+      bool replaced = false;
+      if (bad || rln <= istop || rln < delta * maxr) {
+        if ((rc = fold())) return rc;
+        if ((rc = true_residual())) return rc;
+        res->restarts++;
+        if (rn <= stop) { status = LQCD_OK; break; }
+        if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
+        if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+        maxr = rin;
+        replaced = true;
+      }
+      if (replaced) {
+        if ((rc = direction(bad ? 0 : 2))) return rc;       // beta rescaled to the new residual (0 after a breakdown)
+      } else {
+        if ((rc = op_matpc(c, z, rl, par, 1, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
+        cnt.mat_sloppy++;
+        BlasArgs a = mk(c, false, pv, z);
+        if ((rc = blas<OpCgP>(c, ps, a, s))) return rc;
+      }
+      cnt.blas_flop_sites += 24.0 * 2;
+    }
+    res->iterations = it;
+  }
+  res->iterated_residual = rn;
+  return status;
+}
+
 // ---------------------------------------------------------------- GCR-DD (Algorithm 1)
 int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, double stop,
               lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
@@ -560,11 +654,11 @@ int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
   if ((p->parity | 1) != 1) return fail(c, LQCD_EINVAL, "parity");
   for (int pr : {p->prec_outer, p->prec_sloppy, p->prec_precond}) if (pr < 0 || pr > 2) return fail(c, LQCD_EINVAL, "precision");
   for (int r : {p->recon_outer, p->recon_sloppy, p->recon_precond}) if (recon_index(r) < 0) return fail(c, LQCD_EINVAL, "recon");
-  if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD && p->solver != LQCD_SOLVER_CGNR) return fail(c, LQCD_EINVAL, "solver");
+  if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD && p->solver != LQCD_SOLVER_CGNR && p->solver != LQCD_SOLVER_CGNE) return fail(c, LQCD_EINVAL, "solver");
   if (!(p->tol > 0) || p->max_iter < 1) return fail(c, LQCD_EINVAL, "tol / max_iter");
   if (p->solver == LQCD_SOLVER_GCR_DD && p->precondition && p->mr_steps < 1) return fail(c, LQCD_EINVAL, "mr_steps");
   if (p->matpc_type != LQCD_MATPC_ASYMMETRIC && p->matpc_type != LQCD_MATPC_SYMMETRIC) return fail(c, LQCD_EINVAL, "matpc_type");
-  if (p->matpc_type == LQCD_MATPC_SYMMETRIC && p->solver == LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "symmetric form: BiCGstab and CGNR only");
+  if (p->matpc_type == LQCD_MATPC_SYMMETRIC && p->solver == LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "symmetric form: BiCGstab, CGNR and CGNE only");
   return LQCD_OK;
 }
 
@@ -641,6 +735,7 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   int status;
   if (p->solver == LQCD_SOLVER_BICGSTAB) status = solve_bicgstab(c, xp, bhat, *p, stop, res, cnt, s);
   else if (p->solver == LQCD_SOLVER_CGNR) status = solve_cgnr(c, xp, bhat, *p, stop, res, cnt, s);
+  else if (p->solver == LQCD_SOLVER_CGNE) status = solve_cgne(c, xp, bhat, *p, stop, res, cnt, s);
   else status = solve_gcr(c, xp, bhat, *p, stop, res, cnt, s);
   if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) { cudaEventDestroy(e0); cudaEventDestroy(e1); return status; }
   // true residual of the Schur system in the outer precision = ||b - M x|| (R6)

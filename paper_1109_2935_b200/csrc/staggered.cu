@@ -427,7 +427,7 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
         maxr = rn;
         if (bad) { fresh = true; continue; }
         if ((rc = sconvert(c, 0, 1, rl, r_hi, s))) return rc;
-        { BlasArgs a = mks(c, rl); a.i0 = 1; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }
+        { BlasArgs a = mks(c, rl); a.i0 = 2; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }   // beta = rr_new / rr_old
         { BlasArgs a = mks(c, pl, rl); if ((rc = sblas<OpCgP>(c, 1, a, s))) return rc; }
       }
     }

@@ -17,7 +17,7 @@ LIB_PATH = os.environ.get("LQCD_B200_LIB") or os.path.join(_HERE, "liblqcd_b200.
 
 PREC_DOUBLE, PREC_SINGLE, PREC_HALF = 0, 1, 2
 RECON_18, RECON_12, RECON_8 = 18, 12, 8
-SOLVER_BICGSTAB, SOLVER_GCR_DD, SOLVER_CGNR = 0, 1, 2
+SOLVER_BICGSTAB, SOLVER_GCR_DD, SOLVER_CGNR, SOLVER_CGNE = 0, 1, 2, 3
 MATPC_ASYMMETRIC, MATPC_SYMMETRIC = 0, 1
 FIELD_SPINOR_PARITY, FIELD_STAGGERED_PARITY = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6

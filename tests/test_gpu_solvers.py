@@ -250,3 +250,24 @@ def test_symmetric_even_odd_form(mid):
     with pytest.raises(lq.LqcdError) as e:
         _solve(c, b, p)
     assert e.value.code == lq.EINVAL
+
+
+@pytest.mark.parametrize("prec", [(0, 0, 0), (0, 1, 1), (0, 2, 2)])
+def test_cgne(mid, prec):
+    """CGNE / Craig's method (PAPER.md:128), fp64 and mixed precision, both even-odd forms: the oracle's
+    solution and the full-system residual by the oracle's operator; in fp64 the iteration count of the
+    oracle's CGNE (+-1)."""
+    c = mid
+    lq = c.lqcd
+    kappa = 0.124
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-10, solver=oracle.CGNE)
+    for mt in (lq.MATPC_ASYMMETRIC, lq.MATPC_SYMMETRIC):
+        p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_CGNE, prec=prec, recon=(18, 12, 12), matpc_type=mt)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-10
+        res = np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+        assert res <= 1.05e-10
+        assert _rel(x, xo) <= 1e-8
+        if prec == (0, 0, 0) and mt == lq.MATPC_ASYMMETRIC:
+            assert abs(info["iterations"] - io["iterations"]) <= 1
