@@ -229,6 +229,10 @@ def main():
         run_reference(args, rank)
         return
     args.warmup = max(args.warmup, 3)
+    if world > 1:
+        # replicas: every rank times the headline and the e2e leg; the sweep, the solvers and the CPU baseline
+        # are rank-0-at-N=1 material and would leave the other ranks waiting in the process-group teardown
+        args.quick, args.solvers_only, args.full = True, False, False
     if args.op == "staggered":
         run_staggered(args, rank, world, local)
         return
@@ -358,6 +362,7 @@ def main():
         print(json.dumps(out))
     ctx.close()
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
 
 
@@ -479,6 +484,7 @@ def run_staggered(args, rank, world, local):
         print(json.dumps(out))
     ctx.close()
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
 
 
