@@ -7,7 +7,10 @@ namespace lq {
 
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int NR>
 static cudaError_t launch_mrhs_nr(const DslashArgs& a, int nrhs, cudaStream_t s) {
-  constexpr int NST = P::HALF ? 4 : 2;              // depth of the spinor cp.async ring
+#ifndef LQ_MRHS_PIPE
+#define LQ_MRHS_PIPE 3   /* measured: 2 -> 200, 3 -> 195, 4 -> 214 us per source for the fp32/r12 Mhat at 32^3x64 */
+#endif
+  constexpr int NST = P::HALF ? 4 : LQ_MRHS_PIPE;   // depth of the spinor cp.async ring
   constexpr int SMEM = LinkTile<typename P::real>::BYTES + NST * SpinStage<P, NR>::BYTES;
   dim3 grid((a.range.cb1 - a.range.cb0 + 31) / 32, a.g.nb, (nrhs + NR - 1) / NR);
   auto kern = dslash_mrhs_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, NST, NR>;
