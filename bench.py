@@ -471,11 +471,11 @@ def run_staggered(args, rank, world, local):
         b = chi * torch.from_numpy((inputs.parity_mask(DIMS) == 0)[..., None]).to(dev)
         sig = [0.0, 0.002, 0.01, 0.05, 0.25, 1.0]
         x = torch.zeros((len(sig),) + tuple(chi.shape), dtype=torch.complex128, device=dev)
-        for mass in (0.1, 0.02):
-            ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True)
-            infos = min((ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True) for _ in range(2)), key=lambda r: r[0]["seconds"])
-            ex["multishift_mass_%g" % mass] = {
-                "shifts": sig, "tol": 1e-10, "seconds": infos[0]["seconds"], "multishift_iterations_fp32": infos[0]["matpc_precond"],
+        for mass, msp in ((0.1, 1), (0.02, 1), (0.1, 0), (0.02, 0)):
+            ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True, multishift_prec=msp)
+            infos = min((ctx.staggered_multishift(x, b, 0, mass, sig, 1e-10, allow_fail=True, multishift_prec=msp) for _ in range(2)), key=lambda r: r[0]["seconds"])
+            ex["multishift_mass_%g_%s" % (mass, "fp32_then_refine" if msp else "fp64")] = {
+                "shifts": sig, "tol": 1e-10, "seconds": infos[0]["seconds"], "multishift_iterations": infos[0]["matpc_precond"],
                 "refinement_iterations": [i["iterations"] for i in infos], "reliable_updates": [i["restarts"] for i in infos],
                 "true_residual_max": max(i["true_residual"] for i in infos), "status": [i["status"] for i in infos],
                 "effective_gflops": infos[0]["gflop"] / infos[0]["seconds"]}

@@ -220,9 +220,12 @@ int lqcd_staggered_mdagm(lqcd_ctx* ctx, void* out, const void* in, int parity, d
  * (only the sites of `parity` are read); x_canonical: nshift such arrays back to back (sites of the other
  * parity are set to zero).  result[i]: iterations / restarts / matpc_sloppy / matpc_outer of shift i's
  * refinement, true_residual; result[0].matpc_precond = iterations of the multi-shift phase; seconds and gflop
- * are those of the whole call.  max_iter bounds each phase.  Synchronises `stream`. */
+ * are those of the whole call.  max_iter bounds each phase.  multishift_prec: LQCD_PREC_SINGLE = the paper's
+ * strategy; LQCD_PREC_DOUBLE = the multi-shift phase itself in fp64 down to tol (what PAPER.md:294-296 rules out
+ * for memory and fp64 rate on 2011 GPUs; on B200 it is the faster of the two); the refinement
+ * then only confirms.  Synchronises `stream`. */
 int lqcd_staggered_multishift(lqcd_ctx* ctx, void* x_canonical, const void* b_canonical, int parity, double mass,
-                              const double* sigma, int nshift, double tol, int max_iter,
+                              const double* sigma, int nshift, double tol, int max_iter, int multishift_prec,
                               lqcd_invert_result* result, void* stream);
 
 /* ---- host-buffer entry points (end-to-end path: host<->device copies inside the call) ---- */

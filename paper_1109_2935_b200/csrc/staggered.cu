@@ -292,10 +292,13 @@ int lqcd_staggered_mdagm(lqcd_ctx* c, void* out, const void* in, int parity, dou
 // (M^dag M + sigma_i) x_i = b on one parity, i < nshift (Eq. 4), by the paper's strategy
 // (PAPER.md:296): a pure single-precision multi-shift CG for all shifts at once, then sequential
 // mixed-precision CG (fp64 outer with reliable updates, fp32 inner) refining every x_i to `tol`.
+// multishift_prec = LQCD_PREC_DOUBLE runs the multi-shift phase in fp64 to `tol` instead (the memory and
+// fp64 rate that ruled it out on the paper's GPUs, are not a constraint on B200).
 int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int parity, double mass, const double* sigma,
-                              int nshift, double tol, int max_iter, lqcd_invert_result* res, void* stream) {
+                              int nshift, double tol, int max_iter, int multishift_prec, lqcd_invert_result* res, void* stream) {
   if (!c) return LQCD_EINVAL;
-  if (!x_can || !b_can || !sigma || !res || (parity | 1) != 1 || nshift < 1 || nshift > LQ_MS_MAX || !(tol > 0) || max_iter < 1)
+  if (!x_can || !b_can || !sigma || !res || (parity | 1) != 1 || nshift < 1 || nshift > LQ_MS_MAX || !(tol > 0) || max_iter < 1 ||
+      (multishift_prec != LQCD_PREC_SINGLE && multishift_prec != LQCD_PREC_DOUBLE))
     return fail(c, LQCD_EINVAL, "staggered_multishift arguments");
   for (int i = 0; i < nshift; ++i) if (!(sigma[i] >= 0.0)) return fail(c, LQCD_EINVAL, "shifts must be >= 0");
   for (int i = 1; i < nshift; ++i) if (!(sigma[i] > sigma[i - 1])) return fail(c, LQCD_EINVAL, "shifts must be strictly ascending");
@@ -314,8 +317,10 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
     return LQCD_OK;
   };
   char *b_hi, *x_hi, *r_hi, *r, *ap, *xs, *ps;
-  if ((rc = get(&b_hi, f64)) || (rc = get(&x_hi, f64)) || (rc = get(&r_hi, f64)) || (rc = get(&r, f32)) || (rc = get(&ap, f32)) ||
-      (rc = get(&xs, f32 * nshift)) || (rc = get(&ps, f32 * nshift))) return rc;
+  const int pm = multishift_prec;
+  const size_t fm = pm == 0 ? f64 : f32;
+  if ((rc = get(&b_hi, f64)) || (rc = get(&x_hi, f64)) || (rc = get(&r_hi, f64)) || (rc = get(&r, fm)) || (rc = get(&ap, fm)) ||
+      (rc = get(&xs, fm * nshift)) || (rc = get(&ps, fm * nshift))) return rc;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
   struct Ev { cudaEvent_t a, b; ~Ev() { cudaEventDestroy(a); cudaEventDestroy(b); } } ev{e0, e1};
@@ -332,13 +337,13 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
   double blas_sites = 0;
   int ms_iters = 0, worst = LQCD_OK;
   if (bn > 0.0) {
-    // ---- phase 1: multi-shift CG in single precision, all x_i = 0, r = p_i = b
-    if ((rc = sconvert(c, 0, 1, r, b_hi, s))) return rc;
+    // ---- phase 1: multi-shift CG in precision pm (single = the paper's strategy), all x_i = 0, r = p_i = b
+    if ((rc = sconvert(c, 0, pm, r, b_hi, s))) return rc;
     for (int i = 0; i < nshift; ++i) {
-      if ((rc = sconvert(c, 1, 1, ps + i * f32, r, s))) return rc;
-      BlasArgs a = mks(c, xs + i * f32); if ((rc = sblas<OpZero>(c, 1, a, s))) return rc;
+      if ((rc = sconvert(c, pm, pm, ps + i * fm, r, s))) return rc;
+      BlasArgs a = mks(c, xs + i * fm); if ((rc = sblas<OpZero>(c, pm, a, s))) return rc;
     }
-    { BlasArgs a = mks(c, r); a.i0 = 0; if ((rc = sblas<OpCgInit>(c, 1, a, s))) return rc; }      // rr -> S_RHO, flag = 0
+    { BlasArgs a = mks(c, r); a.i0 = 0; if ((rc = sblas<OpCgInit>(c, pm, a, s))) return rc; }      // rr -> S_RHO, flag = 0
     {
       double* h = c->hS;                                  // initial multi-shift state
       for (int i = 0; i < nshift; ++i) {
@@ -350,28 +355,29 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
       if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "multi-shift state", e);
     }
     // single precision cannot resolve more than ~1e-6 of the source; the refinement takes over from there
-    const double ms_stop = (tol > 2e-6 ? tol : 2e-6) * bn;
+    const double ms_stop = (pm == 0 ? tol : (tol > 2e-6 ? tol : 2e-6)) * bn;
     int active = nshift;
     double rn = bn, best = bn;
     int stall = 0;
     while (rn > ms_stop && ms_iters < max_iter) {
-      if ((rc = op_stag_mdagm(c, ap, ps, parity, mass, sigma[0], 1, s))) return rc;
-      { BlasArgs a = mks(c, ps, ap); if ((rc = sblas<OpCgPAp>(c, 1, a, s))) return rc; }
-      { BlasArgs a = mks(c, r, ap); if ((rc = sblas<OpMsR>(c, 1, a, s))) return rc; }
+      if ((rc = op_stag_mdagm(c, ap, ps, parity, mass, sigma[0], pm, s))) return rc;
+      { BlasArgs a = mks(c, ps, ap); if ((rc = sblas<OpCgPAp>(c, pm, a, s))) return rc; }
+      { BlasArgs a = mks(c, r, ap); if ((rc = sblas<OpMsR>(c, pm, a, s))) return rc; }
       MsArgs m; memset(&m, 0, sizeof(m));
       m.r = r; m.S = c->S; m.ns = c->Vh / 4; m.n = active;
-      for (int i = 0; i < active; ++i) { m.x[i] = xs + i * f32; m.p[i] = ps + i * f32; }
-      ms_update_kernel<PrecS><<<(unsigned)((m.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK), LQ_BLAS_BLOCK, 0, s>>>(m);
+      for (int i = 0; i < active; ++i) { m.x[i] = xs + i * fm; m.p[i] = ps + i * fm; }
+      if (pm == 0) ms_update_kernel<PrecD><<<(unsigned)((m.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK), LQ_BLAS_BLOCK, 0, s>>>(m);
+      else ms_update_kernel<PrecS><<<(unsigned)((m.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK), LQ_BLAS_BLOCK, 0, s>>>(m);
       c->launches++;
       if ((e = cudaGetLastError()) != cudaSuccess) return fail(c, LQCD_ECUDA, "ms_update", e);
-      ++ms_iters; ++n_lo; blas_sites += 6.0 * (2 + 3 + 5 * active);
+      ++ms_iters; if (pm == 0) ++n_hi; else ++n_lo; blas_sites += 6.0 * (2 + 3 + 5 * active);
       if ((rc = sread(c, 0, S_MS_N + 1, s))) return rc;
       const double rr = c->hS[S_RR];
       if (!(rr == rr) || c->hS[S_FLAG] != 0.0) { worst = LQCD_EBREAKDOWN; break; }
       rn = sqrt(rr);
       // a shift whose own residual |zeta_i| ||r|| is below the target is finished: drop it (it is a suffix)
       while (active > 1 && fabs(c->hS[S_MS + LQ_MS_STRIDE * (active - 1)]) * rn <= ms_stop) --active;
-      if (rn < 0.999 * best) { best = rn; stall = 0; } else if (++stall > 50) break;     // fp32 floor reached
+      if (rn < 0.999 * best) { best = rn; stall = 0; } else if (++stall > 50) break;     // precision floor reached
     }
   }
   // ---- phase 2: sequential mixed-precision CG refinement of every shift (fp64 outer, fp32 inner)
@@ -383,7 +389,7 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
   for (int i = 0; i < nshift; ++i) {
     lqcd_invert_result& R = res[i];
     if (bn == 0.0) { R.status = LQCD_OK; continue; }
-    if ((rc = sconvert(c, 1, 0, x_hi, xs + i * f32, s))) return rc;
+    if ((rc = sconvert(c, pm, 0, x_hi, xs + i * fm, s))) return rc;
     double rn;
     if ((rc = sresidual(c, r_hi, b_hi, x_hi, parity, mass, sigma[i], &rn, s))) return rc;
     ++n_hi; R.matpc_outer++;

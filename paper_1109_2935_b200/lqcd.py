@@ -100,7 +100,7 @@ def load_library():
             "lqcd_unpack_staggered": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_staggered_dslash": (i, [vp, vp, vp, i, i, vp]),
             "lqcd_staggered_mdagm": (i, [vp, vp, vp, i, d, d, i, vp]),
-            "lqcd_staggered_multishift": (i, [vp, vp, vp, i, d, ctypes.POINTER(d), i, d, i, ctypes.POINTER(InvertResult), vp]),
+            "lqcd_staggered_multishift": (i, [vp, vp, vp, i, d, ctypes.POINTER(d), i, d, i, i, ctypes.POINTER(InvertResult), vp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(lib, name)
@@ -238,13 +238,13 @@ class Context:
         self._check(self.lib.lqcd_staggered_mdagm(self.h, _ptr(out), _ptr(inp), parity, mass, sigma, prec, _stream()))
         return out
 
-    def staggered_multishift(self, x, b, parity, mass, sigmas, tol, max_iter=10000, allow_fail=False):
+    def staggered_multishift(self, x, b, parity, mass, sigmas, tol, max_iter=10000, allow_fail=False, multishift_prec=PREC_SINGLE):
         """x: [nshift, T, Z, Y, X, 3], b: [T, Z, Y, X, 3] complex128 device tensors.  One result dict per shift."""
         n = len(sigmas)
         assert x.is_cuda and b.is_cuda and x.dtype == b.dtype == torch.complex128 and x.is_contiguous() and x.shape[0] == n
         sg = (ctypes.c_double * n)(*[float(v) for v in sigmas])
         r = (InvertResult * n)()
-        rc = self.lib.lqcd_staggered_multishift(self.h, _ptr(x), _ptr(b), parity, mass, sg, n, tol, max_iter, r, _stream())
+        rc = self.lib.lqcd_staggered_multishift(self.h, _ptr(x), _ptr(b), parity, mass, sg, n, tol, max_iter, multishift_prec, r, _stream())
         self._check(rc, allow=(ENOCONV, EBREAKDOWN) if allow_fail else ())
         return [r[k].as_dict() for k in range(n)]
 

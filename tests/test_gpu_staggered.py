@@ -109,8 +109,9 @@ def test_staggered_errors():
     ctx.close()
 
 
+@pytest.mark.parametrize("ms_prec", [1, 0])
 @pytest.mark.parametrize("parity", [0, 1])
-def test_multishift_solver(ragged, parity):
+def test_multishift_solver(ragged, parity, ms_prec):
     """lqcd_staggered_multishift (single-precision multi-shift CG + mixed-precision refinement):
     every x_i equals the oracle's own CG solution of (M^dag M + sigma_i) x = b on that parity, and the true
     residual recomputed with the ORACLE's operator meets the tolerance."""
@@ -118,7 +119,7 @@ def test_multishift_solver(ragged, parity):
     mass, sigmas, tol = 0.08, [0.0, 0.01, 0.1, 0.5, 2.0], 1e-10
     b = inputs.gaussian_colour_vector(c.dims, 5) * c.mask(parity)
     x = torch.zeros((len(sigmas),) + b.shape, dtype=torch.complex128, device="cuda")
-    infos = c.ctx.staggered_multishift(x, torch.from_numpy(b).cuda(), parity, mass, sigmas, tol)
+    infos = c.ctx.staggered_multishift(x, torch.from_numpy(b).cuda(), parity, mass, sigmas, tol, multishift_prec=ms_prec)
     xs = x.cpu().numpy()
     assert infos[0]["matpc_precond"] > 0                    # the multi-shift phase ran
     for i, sg in enumerate(sigmas):
@@ -130,6 +131,8 @@ def test_multishift_solver(ragged, parity):
         assert io["status"] == 0 and _rel(xs[i], xo) <= 1e-8, i
     # larger shifts are better conditioned: their refinement needs no more iterations than the smallest shift's
     assert infos[-1]["iterations"] <= infos[0]["iterations"]
+    if ms_prec == 0:      # the fp64 multi-shift phase reaches the tolerance by itself: the refinement only confirms
+        assert sum(i["iterations"] for i in infos) <= 3 * len(sigmas)
 
 
 def test_multishift_edges(ragged):
