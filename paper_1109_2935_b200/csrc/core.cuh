@@ -185,6 +185,22 @@ LQ_DEV void load_site_raw(typename P::real* __restrict__ v, typename P::real& sc
   }
 }
 
+// half precision only: the N stored values as floats m = 2^23 + 32768 + q (no decoding FADD), for consumers that
+// combine pairs of them exactly (fixed_project in dslash.cuh); scale as in load_site_raw
+template <class P, int N, int MODE = 0>
+LQ_DEV void load_site_magic(float* __restrict__ m, float& scale, const char* __restrict__ f, long long ns, long long i) {
+  static_assert(P::HALF, "magic-float form exists for the 16-bit fixed-point storage only");
+  alignas(16) unsigned w[N / 2];
+  Rec<unsigned, N / 2>::template load<MODE>(w, f, ns, i);
+  const int* np = reinterpret_cast<const int*>(f + (long long)(2 * N) * ns) + i;
+  scale = __int_as_float(MODE == 2 ? ld_shared(np) : ld_nc(np)) * LQ_FIXED_INV;
+#pragma unroll
+  for (int k = 0; k < N / 2; ++k) {
+    m[2 * k] = __uint_as_float(__byte_perm(w[k], 0x4B000000u, 0x7610));
+    m[2 * k + 1] = __uint_as_float(__byte_perm(w[k], 0x4B000000u, 0x7632));
+  }
+}
+
 template <class P, int N>
 LQ_DEV void load_site(typename P::real* __restrict__ v, const char* __restrict__ f, long long ns, long long i) {
   typename P::real sc;

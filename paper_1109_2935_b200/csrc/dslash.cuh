@@ -61,6 +61,9 @@ template <> struct GammaRow<3> { static constexpr int j0 = 2, c0 = 0, j1 = 3, c1
 // coef carries the boundary sign and, in half precision, the spinor norm and the link scale.
 // All multiply-adds are written as explicit FMAs (nvcc does not re-associate a*b - c*d + e).
 template <int MU, bool FWD, typename R>
+LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef);
+
+template <int MU, bool FWD, typename R>
 LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restrict__ u, R sigma, R coef) {
   typedef GammaRow<MU> G;
   // project: h0 = psi_0 + sigma*c0*psi_j0, h1 = psi_1 + sigma*c1*psi_j1   (3 colours each)
@@ -72,6 +75,44 @@ LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restr
     h[0][c] = {fma_(sigma, q0.re, psi[2 * c]), fma_(sigma, q0.im, psi[2 * c + 1])};
     h[1][c] = {fma_(sigma, q1.re, psi[6 + 2 * c]), fma_(sigma, q1.im, psi[6 + 2 * c + 1])};
   }
+  hop_tail<MU, FWD, R>(acc, h, u, sigma, coef);
+}
+
+// ---- 16-bit fixed point: projection fused with the decode (compile-time sigma) -----------------------
+// A stored value q in [-32767, 32767] arrives as the float m = 2^23 + 32768 + q (one PRMT, core.cuh).  The
+// projected component q_a + s q_b (s = +-1) is formed on these floats directly, exactly:
+//   s = -1:  m_a - m_b                         (one FADD; both offsets cancel)
+//   s = +1:  (m_a - 2(2^23 + 32768)) + m_b     (two FADDs; every intermediate is an integer below 2^24)
+// instead of two decoding FADDs and one FFMA: 1.5 instead of 3 instructions per projected real.  Which
+// of the two applies to a component depends on sigma, so the dagger flag is a template parameter of the
+// half-precision kernels.  Results are bit-identical to decode-then-project.
+template <int S> LQ_DEV float fixed_sum(float ma, float mb) {
+  if (S < 0) return ma - mb;
+  return (ma - 2.0f * LQ_MAGIC_DEC) + mb;
+}
+// (a + SG * unit<C>(b)) on magic floats: unit<0> = 1, <1> = i, <2> = -1, <3> = -i
+template <int C, int SG> LQ_DEV cx<float> fixed_project(float ar, float ai, float br, float bi) {
+  constexpr int SRE = SG * ((C == 0 || C == 3) ? 1 : -1);
+  constexpr int SIM = SG * ((C == 0 || C == 1) ? 1 : -1);
+  const float xr = (C == 0 || C == 2) ? br : bi;
+  const float xi = (C == 0 || C == 2) ? bi : br;
+  return {fixed_sum<SRE>(ar, xr), fixed_sum<SIM>(ai, xi)};
+}
+template <int MU, bool FWD, int SG>
+LQ_DEV void hop_fixed(float* __restrict__ acc, const float* __restrict__ m, const float* __restrict__ u, float coef) {
+  typedef GammaRow<MU> G;
+  cx<float> h[2][3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    h[0][c] = fixed_project<G::c0, SG>(m[2 * c], m[2 * c + 1], m[6 * G::j0 + 2 * c], m[6 * G::j0 + 2 * c + 1]);
+    h[1][c] = fixed_project<G::c1, SG>(m[6 + 2 * c], m[6 + 2 * c + 1], m[6 * G::j1 + 2 * c], m[6 * G::j1 + 2 * c + 1]);
+  }
+  hop_tail<MU, FWD, float>(acc, h, u, (float)SG, coef);
+}
+
+template <int MU, bool FWD, typename R>
+LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef) {
+  typedef GammaRow<MU> G;
   // colour multiply: 6 FMA per real output
   cx<R> w[2][3];
 #pragma unroll
@@ -269,9 +310,12 @@ template <class P, int RECON> struct HopStage {
 // memory filled by cp.async: while hop h is computed, the loads of hops h+1 .. h+NST-1 are in
 // flight without holding registers.  The slots are private to a thread, so no CTA barrier is
 // needed: cp.async.wait_group orders a thread's own copies.
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST>
+// DAG: -1 = dagger read from the arguments at run time (fp64, fp32); 0 / 1 = compile-time dagger (half precision:
+// the fixed-point projection fused with the decode needs the sign of every combination at compile time).
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST, int DAG = -1>
 __global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? LQ_DSLASH_MINB64 : LQ_DSLASH_MINB))
 dslash_kernel(const DslashArgs a) {
+  static_assert(P::HALF ? (DAG == 0 || DAG == 1) : DAG == -1, "compile-time dagger for half precision only");
   typedef typename P::real R;
   const Geom& g = a.g;
   const int cb = (DOTS ? 0 : a.range.cb0) + blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
@@ -357,11 +401,13 @@ dslash_kernel(const DslashArgs a) {
         const char* sb_ = lq_stage + ((H) % NST) * HS::BYTES;                                              \
         R u[18], psi[24], us, ps;                                                                          \
         load_link<P, RECON, 2>(u, us, sb_, LQ_DSLASH_BLOCK, tid);                                          \
-        load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);        \
+        if constexpr (P::HALF) load_site_magic<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid); \
+        else load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);   \
         if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                       \
         cp_async_commit();                                                                                 \
         const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
-        hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, P::HALF ? sg_ * us * ps : sg_);                \
+        if constexpr (P::HALF) hop_fixed<MU_, FW_, (FW_ == (DAG == 1)) ? 1 : -1>(acc, psi, u, sg_ * us * ps); \
+        else hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, sg_);                                     \
       }
 #pragma unroll
       for (int h = 0; h < NST; ++h) {

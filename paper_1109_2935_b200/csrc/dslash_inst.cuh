@@ -17,11 +17,11 @@ namespace lq {
 #define LQ_PIPE_HALF 4
 #endif
 
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
-static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int DAG>
+static void launch_dag(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
   constexpr int NST = sizeof(typename P::real) == 8 ? ((CLOVX || CLOVOUT) ? 0 : LQ_PIPE_FP64) : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
   constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
-  auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST>;
+  auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST, DAG>;
   static bool configured_dev[64] = {};    // per instantiation and device (function attributes are per device)
   int dev = 0;
   cudaGetDevice(&dev);
@@ -38,6 +38,17 @@ static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
     configured = true;
   }
   kern<<<grid, block, SMEM, s>>>(a);
+}
+
+// half precision: the dagger flag selects one of two instantiations (dslash.cuh, hop_fixed)
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
+  if constexpr (P::HALF) {
+    if (a.dagger) launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, 1>(a, grid, block, s);
+    else launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, 0>(a, grid, block, s);
+  } else {
+    launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, -1>(a, grid, block, s);
+  }
 }
 
 template <class P, int RECON>

@@ -73,10 +73,12 @@ template <class P> struct MrhsMinB { static constexpr int V = sizeof(typename P:
 
 // a.in / a.out / a.y hold nrhs packed fields back to back (field r at r * bytes of one field);
 // a.dagger carries nrhs in bits 8.. (the argument struct must stay 128 bytes, dslash.cuh).
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int NST, int NR>
+// DAG: as in dslash_kernel (-1 run-time dagger for fp64 / fp32, 0 / 1 compile-time for half precision)
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int NST, int NR, int DAG = -1>
 __global__ void __launch_bounds__(32 * NR, MrhsMinB<P>::V)
 dslash_mrhs_kernel(const DslashArgs a) {
   typedef typename P::real R;
+  static_assert(P::HALF ? (DAG == 0 || DAG == 1) : DAG == -1, "compile-time dagger for half precision only");
   static_assert(NST >= 1 && NST <= 4, "spinor ring depth");
   static_assert(NR == 4, "right-hand sides per CTA = directions");
   constexpr int LQ_MRHS_BLOCK = 32 * NR;
@@ -171,11 +173,13 @@ dslash_mrhs_kernel(const DslashArgs a) {
       const char* ss_ = ring + ((H) % NST) * SpinStage<P, NR>::BYTES;                                      \
       R u[18], psi[24], ps;                                                                                \
       LinkTile<R>::get(tile, (H), lane, u);                                                                \
-      load_site_raw<P, 24, 2>(psi, ps, ss_, LQ_MRHS_BLOCK, tid);                                           \
+      if constexpr (P::HALF) load_site_magic<P, 24, 2>(psi, ps, ss_, LQ_MRHS_BLOCK, tid);                  \
+      else load_site_raw<P, 24, 2>(psi, ps, ss_, LQ_MRHS_BLOCK, tid);                                      \
       if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                         \
       cp_async_commit();                                                                                   \
       const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
-      hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, P::HALF ? sg_ * USCALE * ps : sg_);              \
+      if constexpr (P::HALF) hop_fixed<MU_, FW_, (FW_ == (DAG == 1)) ? 1 : -1>(acc, psi, u, sg_ * USCALE * ps); \
+      else hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, sg_);                                       \
     }
     LQ_PHOP(0) LQ_PHOP(1) LQ_PHOP(2) LQ_PHOP(3) LQ_PHOP(4) LQ_PHOP(5) LQ_PHOP(6) LQ_PHOP(7)
 #undef LQ_PHOP

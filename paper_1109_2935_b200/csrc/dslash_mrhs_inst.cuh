@@ -5,7 +5,7 @@
 
 namespace lq {
 
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int NR>
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int NR, int DAG>
 static cudaError_t launch_mrhs_nr(const DslashArgs& a, int nrhs, cudaStream_t s) {
 #ifndef LQ_MRHS_PIPE
 #define LQ_MRHS_PIPE 3   /* measured: 2 -> 200, 3 -> 195, 4 -> 214 us per source for the fp32/r12 Mhat at 32^3x64 */
@@ -13,7 +13,7 @@ static cudaError_t launch_mrhs_nr(const DslashArgs& a, int nrhs, cudaStream_t s)
   constexpr int NST = P::HALF ? 4 : LQ_MRHS_PIPE;   // depth of the spinor cp.async ring
   constexpr int SMEM = LinkTile<typename P::real>::BYTES + NST * SpinStage<P, NR>::BYTES;
   dim3 grid((a.range.cb1 - a.range.cb0 + 31) / 32, a.g.nb, (nrhs + NR - 1) / NR);
-  auto kern = dslash_mrhs_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, NST, NR>;
+  auto kern = dslash_mrhs_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, NST, NR, DAG>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
   if (e != cudaSuccess) return e;
   cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -23,7 +23,12 @@ static cudaError_t launch_mrhs_nr(const DslashArgs& a, int nrhs, cudaStream_t s)
 
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT>
 static cudaError_t launch_mrhs_one(const DslashArgs& a, int nrhs, cudaStream_t s) {
-  return launch_mrhs_nr<P, RECON, XPAY, CLOVX, CLOVOUT, 4>(a, nrhs, s);
+  if constexpr (P::HALF) {
+    if (a.dagger & 1) return launch_mrhs_nr<P, RECON, XPAY, CLOVX, CLOVOUT, 4, 1>(a, nrhs, s);
+    return launch_mrhs_nr<P, RECON, XPAY, CLOVX, CLOVOUT, 4, 0>(a, nrhs, s);
+  } else {
+    return launch_mrhs_nr<P, RECON, XPAY, CLOVX, CLOVOUT, 4, -1>(a, nrhs, s);
+  }
 }
 
 template <class P, int RECON>
