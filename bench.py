@@ -45,8 +45,8 @@ def matpc_bytes(prec, recon):
 
 # ncu --set full captures of one launch at 32^3x64 (profiles/r1_dslash_*.md): DRAM bytes read + written,
 # and executed warp instructions (the half-precision kernels are issue-bound)
-NCU_TRAFFIC = {("fp32", 12): 593.75e6, ("half", 12): 300.73e6, ("staggered", "fp32"): 1238.6e6}
-NCU_WARP_INST = {("half", 12): 74.78e6}
+NCU_TRAFFIC = {("fp32", 12): 593.75e6, ("half", 12): 301.72e6, ("staggered", "fp32"): 1238.6e6}
+NCU_WARP_INST = {("half", 12): 69.50e6}
 N_SCHEDULERS = 148 * 4      # one warp instruction per scheduler per clock (B200: 148 SMs x 4 SMSPs)
 
 
