@@ -238,3 +238,19 @@ def test_full_size_32x64_operator_and_solve():
         res = np.linalg.norm(bn - oracle.stag_MdagM(x[i].cpu().numpy(), fn, ln, bc, mass, sg)) / np.linalg.norm(bn)
         assert infos[i]["status"] == 0 and res <= 1.05 * tol, (i, res)
     ctx.close()
+
+
+@pytest.mark.parametrize("ms_prec", [1, 0])
+def test_multishift_wide_shift_range_and_small_mass(ms_prec):
+    """Eight shifts over six decades (0 ... 100) at mass 0.005: the zeta recurrences of the converged (large)
+    shifts underflow while the small ones still iterate; every solution meets 1e-11 by the oracle's operator."""
+    dims, bc = (8, 8, 8, 16), (1, 1, 1, -1)
+    c = SCase(dims, 0.4, bc, seed=3, long_scale=-1.0 / 24.0)
+    b = inputs.gaussian_colour_vector(dims, 4) * c.mask(0)
+    sig = [0.0, 1e-4, 1e-3, 1e-2, 0.1, 1.0, 10.0, 100.0]
+    x = torch.zeros((len(sig),) + b.shape, dtype=torch.complex128, device="cuda")
+    infos = c.ctx.staggered_multishift(x, torch.from_numpy(b).cuda(), 0, 0.005, sig, 1e-11, max_iter=20000, multishift_prec=ms_prec)
+    for i, sg in enumerate(sig):
+        res = np.linalg.norm(b - oracle.stag_MdagM(x[i].cpu().numpy(), c.fat, c.lng, c.bc, 0.005, sg)) / np.linalg.norm(b)
+        assert infos[i]["status"] == 0 and res <= 1.05e-11, (i, res)
+    c.ctx.close()
