@@ -171,6 +171,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
     for (char* z : {xl, pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
     { BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc; }
     double maxr = rin;
+    const double r_start = rn;                // divergence guard: BiCGstab can blow up on an indefinite operator (kappa > kappa_c)
     int it = 0;
     while (true) {
       if (it >= p.max_iter) {
@@ -206,6 +207,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
         if ((rc = true_residual())) return rc;
         res->restarts++;
         if (rn <= stop) { status = LQCD_OK; break; }
+        if (rn > 1e5 * r_start) { status = LQCD_EBREAKDOWN; break; }      // the true residual has grown 1e5-fold: give up
         if (status == LQCD_EBREAKDOWN) {
           // restart the recurrence from the true residual
           status = LQCD_OK;

@@ -271,3 +271,31 @@ def test_cgne(mid, prec):
         assert _rel(x, xo) <= 1e-8
         if prec == (0, 0, 0) and mt == lq.MATPC_ASYMMETRIC:
             assert abs(info["iterations"] - io["iterations"]) <= 1
+
+
+def test_beyond_critical_kappa_cgnr_converges_where_bicgstab_does_not():
+    """kappa = 0.138 on these rough links is beyond kappa_c: M is indefinite.  BiCGstab (the oracle's plain fp64
+    one as well) does not converge there; it must end with LQCD_ENOCONV or LQCD_EBREAKDOWN and an honest true
+    residual, never with a false success.  CGNR and GCR-DD converge to the oracle's solution."""
+    c = Case((8, 8, 8, 16), 0.2)
+    lq = c.lqcd
+    kappa = 0.138
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-10, solver=oracle.CGNR)
+    assert io["status"] == 0
+    for solver, kw in ((lq.SOLVER_CGNR, {}), (lq.SOLVER_CGNE, {}), (lq.SOLVER_GCR_DD, dict(schwarz_block=(4, 4, 4, 8), mr_steps=4))):
+        p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=solver, prec=(0, 1, 2), recon=(18, 12, 12), max_iter=5000, **kw)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0
+        assert np.linalg.norm(b - oracle.M(x, c.U, c.T, c.bc, kappa)) / np.linalg.norm(b) <= 1.05e-10
+        assert _rel(x, xo) <= 1e-7
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB, prec=(0, 2, 2), recon=(18, 12, 12), max_iter=400)
+    x = torch.zeros(b.shape, dtype=torch.complex128, device="cuda")
+    info = c.ctx.invert(x, torch.from_numpy(b).cuda(), p, allow_fail=True)
+    if info["status"] == 0:
+        assert info["true_residual"] <= 1e-10
+    else:
+        assert info["status"] in (lq.ENOCONV, lq.EBREAKDOWN)
+        res = np.linalg.norm(b - oracle.M(x.cpu().numpy(), c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
+        assert abs(res - info["true_residual"]) <= 1e-6 * res       # the reported residual is the real one
+    c.ctx.close()
