@@ -80,6 +80,9 @@ typedef struct lqcd_ctx lqcd_ctx;
 int lqcd_create(lqcd_ctx** ctx, const int dims[4], const int boundary[4], int device);
 int lqcd_destroy(lqcd_ctx* ctx);
 const char* lqcd_last_error(const lqcd_ctx* ctx);
+/* Solver and host-pipeline workspace is cached in the context between calls (allocating ~1 GB per solve costs
+ * milliseconds); this frees the cache (lqcd_destroy does it too).  Synchronises the device. */
+int lqcd_release_workspace(lqcd_ctx* ctx);
 
 /* Load the gauge field (canonical layout, device pointer, 4*V*9 complex128).  Packs the
  * checkerboarded fp64 / recon-18 copy immediately; other precision x compression copies are

@@ -32,6 +32,29 @@ int dev_alloc(lqcd_ctx* c, void** p, size_t bytes) {
   return LQCD_OK;
 }
 
+int ws_get(lqcd_ctx* c, void** p, size_t bytes, cudaStream_t s) {
+  for (size_t i = 0; i < c->pool.size(); ++i) {
+    if (c->pool[i].bytes != bytes) continue;
+    lqcd_ctx::WsBuf b = c->pool[i];
+    c->pool.erase(c->pool.begin() + i);
+    if (b.last != s) cudaStreamSynchronize(b.last);     // handed back on another stream: let its work finish first
+    *p = b.p;
+    return LQCD_OK;
+  }
+  int rc = dev_alloc(c, p, bytes);
+  if (rc && !c->pool.empty()) {                          // out of memory: drop the cache and try once more
+    cudaDeviceSynchronize();
+    for (auto& b : c->pool) cudaFree(b.p);
+    c->pool.clear();
+    rc = dev_alloc(c, p, bytes);
+  }
+  return rc;
+}
+
+void ws_put(lqcd_ctx* c, void* p, size_t bytes, cudaStream_t s) {
+  if (p) c->pool.push_back(lqcd_ctx::WsBuf{p, bytes, s});
+}
+
 static void free_p(char*& p) { if (p) cudaFree(p); p = nullptr; }
 
 static void drop_clover_copies(lqcd_ctx* c) {
@@ -293,7 +316,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->counters) cudaFree(c->counters);
   if (c->boxdots) cudaFree(c->boxdots);
   if (c->hS) cudaFreeHost(c->hS);
-  for (void* p : c->pool) cudaFree(p);
+  for (auto& b : c->pool) cudaFree(b.p);
   for (void* p : c->hws) if (p) cudaFree(p);
   if (c->mtmp) cudaFree(c->mtmp);
   for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfatp[0], (void*)c->sfatp[1], (void*)c->slngp[0], (void*)c->slngp[1], (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);
@@ -302,6 +325,15 @@ int lqcd_destroy(lqcd_ctx* c) {
     for (int i = 0; i < LQ_HOST_SLABS; ++i) { cudaEventDestroy(c->hev_in[i]); cudaEventDestroy(c->hev_out[i]); }
   }
   delete c;
+  return LQCD_OK;
+}
+
+int lqcd_release_workspace(lqcd_ctx* c) {
+  if (!c) return LQCD_EINVAL;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  for (auto& b : c->pool) cudaFree(b.p);
+  c->pool.clear();
   return LQCD_OK;
 }
 

@@ -98,7 +98,11 @@ struct lqcd_ctx {
   double* boxdots;        // MR per-box partial dots
   size_t boxdots_doubles;
   double* hS;             // pinned host mirror of S
-  std::vector<void*> pool; // solver workspace allocations released at the end of lqcd_invert
+  // workspace cache: buffers handed back by finished calls, reused by the next call that asks for the same size
+  // (cudaMalloc / cudaFree of ~1 GB per solve cost milliseconds and, after a free, occasionally 100 ms);
+  // released by lqcd_release_workspace and lqcd_destroy
+  struct WsBuf { void* p; size_t bytes; cudaStream_t last; };
+  std::vector<WsBuf> pool;
   // lqcd_apply_host: cached staging buffers, copy streams and events of the slab pipeline
   void* hws[8];
   size_t hws_bytes[8];

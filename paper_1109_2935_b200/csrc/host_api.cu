@@ -16,11 +16,6 @@
 using namespace lq;
 
 namespace {
-struct DevBuf {
-  void* p = nullptr;
-  ~DevBuf() { if (p) cudaFree(p); }
-};
-
 // grow-only staging buffer `slot` of the context (freed by lqcd_destroy)
 int hbuf(lqcd_ctx* c, int slot, size_t bytes, void** out) {
   if (c->hws_bytes[slot] < bytes) {
@@ -141,10 +136,10 @@ int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const lqcd_i
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
   const size_t cbytes = (size_t)c->V * 24 * sizeof(double);
-  DevBuf xb, bb;
+  struct Ws { lqcd_ctx* c; cudaStream_t s; size_t n; void* p = nullptr; ~Ws() { ws_put(c, p, n, s); } } xb{c, s, cbytes}, bb{c, s, cbytes};
   int rc;
-  if ((rc = dev_alloc(c, &xb.p, cbytes))) return rc;
-  if ((rc = dev_alloc(c, &bb.p, cbytes))) return rc;
+  if ((rc = ws_get(c, &xb.p, cbytes, s))) return rc;
+  if ((rc = ws_get(c, &bb.p, cbytes, s))) return rc;
   cudaError_t e = cudaMemcpyAsync(bb.p, b_host, cbytes, cudaMemcpyHostToDevice, s);
   if (e == cudaSuccess && p->use_initial_guess) e = cudaMemcpyAsync(xb.p, x_host, cbytes, cudaMemcpyHostToDevice, s);
   if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "H2D", e);

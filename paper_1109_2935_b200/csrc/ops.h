@@ -6,6 +6,11 @@ namespace lq {
 
 int fail(lqcd_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess);
 int dev_alloc(lqcd_ctx* c, void** p, size_t bytes);
+// workspace of a call: taken from the context's cache when a buffer of that size is there, else allocated;
+// ws_put hands it back (its pending work on stream `s` is ordered before any reuse on the same stream, and
+// waited for before a reuse on another stream)
+int ws_get(lqcd_ctx* c, void** p, size_t bytes, cudaStream_t s);
+void ws_put(lqcd_ctx* c, void* p, size_t bytes, cudaStream_t s);
 int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, cudaStream_t s);
 int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A, const char** Ainv, cudaStream_t s);
 int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out);

@@ -22,16 +22,17 @@ typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;
 typedef OpMrUpdate<true, true> OpMrOnly;
 
-struct Work {                      // solver workspace, freed when it goes out of scope
+struct Work {                      // workspace of one call; goes back to the context's cache when it leaves scope
   lqcd_ctx* c;
-  std::vector<void*> ptrs;
-  explicit Work(lqcd_ctx* c_) : c(c_) {}
-  ~Work() { for (void* p : ptrs) cudaFree(p); }
+  cudaStream_t s;
+  std::vector<std::pair<void*, size_t>> bufs;
+  Work(lqcd_ctx* c_, cudaStream_t s_) : c(c_), s(s_) {}
+  ~Work() { for (auto& b : bufs) ws_put(c, b.first, b.second, s); }
   int get(char** out, size_t bytes) {
     void* p = nullptr;
-    int rc = dev_alloc(c, &p, bytes);
+    int rc = ws_get(c, &p, bytes, s);
     if (rc) return rc;
-    ptrs.push_back(p);
+    bufs.push_back({p, bytes});
     *out = (char*)p;
     return LQCD_OK;
   }
@@ -141,7 +142,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
                    lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
   const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
   const long long ns = c->nat.ns;
-  Work wk(c);
+  Work wk(c, s);
   char *r_hi, *xl, *rl, *rt, *pv, *v, *t;
   int rc;
   if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
@@ -238,7 +239,7 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
                lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
   const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
   const long long ns = c->nat.ns;
-  Work wk(c);
+  Work wk(c, s);
   char *r_hi, *xl, *rl, *z, *pv, *w;
   int rc;
   if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
@@ -320,7 +321,7 @@ int solve_cgne(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
                lqcd_invert_result* res, Counts& cnt, cudaStream_t s) {
   const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
   const long long ns = c->nat.ns;
-  Work wk(c);
+  Work wk(c, s);
   char *r_hi, *xl, *rl, *z, *pv, *w;
   int rc;
   if ((rc = wk.get(&r_hi, spinor_bytes(po, ns)))) return rc;
@@ -414,7 +415,7 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
   const int kmax = p.gcr_kmax > 0 ? p.gcr_kmax : 16;
   if (kmax > LQ_GCR_KMAX) return fail(c, LQCD_EINVAL, "gcr_kmax too large");
   const double delta = p.delta > 0 ? p.delta : 0.1;
-  Work wk(c);
+  Work wk(c, s);
   int rc;
   char *r0, *rh, *rho = nullptr, *w = nullptr, *xk = nullptr;
   std::vector<char*> ph(kmax), zh(kmax);
@@ -548,7 +549,7 @@ int solve_bicgstab_mrhs(lqcd_ctx* c, char* x, const char* b, int nrhs, const lqc
   const int po = p.prec_outer, ps = p.prec_sloppy, par = p.parity;
   const long long ns = c->nat.ns;
   const size_t fo = spinor_bytes(po, ns), fs = spinor_bytes(ps, ns);
-  Work wk(c);
+  Work wk(c, s);
   char *r_hi, *xl, *rl, *rt, *pv, *v, *t;
   int rc;
   if ((rc = wk.get(&r_hi, fo * nrhs))) return rc;
@@ -678,7 +679,7 @@ int lqcd_schwarz(lqcd_ctx* c, void* out, const void* in, int parity, double kapp
   cudaStream_t s = (cudaStream_t)stream;
   int rc = set_blocks(c, block);
   if (rc) return rc;
-  Work wk(c);
+  Work wk(c, s);
   char *rho, *w, *xk;
   for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->nat.ns)))) return rc;
   rc = schwarz_apply(c, (char*)out, (const char*)in, parity, kappa, n_mr, omega_mr, prec, recon, prec_io, rho, w, xk, s);
@@ -696,7 +697,7 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   memset(res, 0, sizeof(*res));
   const int po = p->prec_outer, par = p->parity;
   const long long ns = c->nat.ns;
-  Work wk(c);
+  Work wk(c, s);
   char *bp, *bq, *xp, *xq, *t1;
   for (char** q : {&bp, &bq, &xp, &xq, &t1}) if ((rc = wk.get(q, spinor_bytes(po, ns)))) return rc;
   cudaEvent_t e0, e1;
@@ -780,7 +781,7 @@ int lqcd_invert_mrhs(lqcd_ctx* c, void* x_can, const void* b_can, int nrhs, cons
   const int po = p->prec_outer, par = p->parity;
   const long long ns = c->nat.ns;
   const size_t fo = spinor_bytes(po, ns), cb = (size_t)c->V * 24 * sizeof(double);
-  Work wk(c);
+  Work wk(c, s);
   char *bp, *bq, *xp, *bhat, *t1;
   for (char** q : {&bp, &bq, &xp, &bhat, &t1}) if ((rc = wk.get(q, fo * nrhs))) return rc;
   cudaEvent_t e0, e1;

@@ -308,12 +308,15 @@ int lqcd_staggered_multishift(lqcd_ctx* c, void* x_can, const void* b_can, int p
   cudaStream_t s = (cudaStream_t)stream;
   memset(res, 0, sizeof(*res) * nshift);
   const size_t f64 = colour_bytes(0, c->Vh), f32 = colour_bytes(1, c->Vh), cbytes = (size_t)c->V * 6 * sizeof(double);
-  struct Bufs { std::vector<void*> v; ~Bufs() { for (void* p : v) cudaFree(p); } } bufs;
+  struct Bufs {                                           // workspace from / back to the context's cache
+    lqcd_ctx* c; cudaStream_t s; std::vector<std::pair<void*, size_t>> v;
+    ~Bufs() { for (auto& b : v) ws_put(c, b.first, b.second, s); }
+  } bufs{c, s, {}};
   auto get = [&](char** out, size_t bytes) -> int {
     void* p = nullptr;
-    int rc2 = dev_alloc(c, &p, bytes);
+    int rc2 = ws_get(c, &p, bytes, s);
     if (rc2) return rc2;
-    bufs.v.push_back(p); *out = (char*)p;
+    bufs.v.push_back({p, bytes}); *out = (char*)p;
     return LQCD_OK;
   };
   char *b_hi, *x_hi, *r_hi, *r, *ap, *xs, *ps;

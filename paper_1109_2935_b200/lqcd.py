@@ -23,7 +23,7 @@ FIELD_SPINOR_PARITY, FIELD_STAGGERED_PARITY = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = [
-    "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_load_gauge", "lqcd_build_clover",
+    "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_release_workspace", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
     "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
@@ -75,6 +75,7 @@ def load_library():
         sig = {
             "lqcd_create": (i, [ctypes.POINTER(vp), ctypes.POINTER(i), ctypes.POINTER(i), i]),
             "lqcd_destroy": (i, [vp]),
+            "lqcd_release_workspace": (i, [vp]),
             "lqcd_last_error": (ctypes.c_char_p, [vp]),
             "lqcd_load_gauge": (i, [vp, vp, vp]),
             "lqcd_build_clover": (i, [vp, d, vp]),
@@ -138,6 +139,9 @@ class Context:
         if getattr(self, "h", None):
             self.lib.lqcd_destroy(self.h)
             self.h = None
+
+    def release_workspace(self):
+        self._check(self.lib.lqcd_release_workspace(self.h))
 
     def __del__(self):
         try:
