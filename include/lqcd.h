@@ -8,8 +8,9 @@
  *   problem           M x = b                                    PAPER.md:88-92  Sec. 2.1 Eq. 1
  *   operator          M = A(kappa) - kappa D,  A = 1 + kappa T   PAPER.md:98-108 Sec. 2.2 Eq. 2 (R1-R4)
  *   even-odd          Mhat = A_pp - kappa^2 D A^-1 D             PAPER.md:128    Sec. 3.1     (R6)
- *   solvers           mixed-precision BiCGstab, CGNR
+ *   solvers           mixed-precision BiCGstab, CGNR, CGNE
  *                     GCR-DD (Algorithm 1) + additive Schwarz/MR PAPER.md:146, :248-292 Sec. 8.1
+ *   improved staggered D, M^dag M + sigma, multi-shift CG         PAPER.md:114-134, :296 (lqcd_staggered_*)
  *
  * Conventions
  *   - Unless a function says "host", every field pointer is a DEVICE pointer owned by the
@@ -65,8 +66,8 @@ typedef struct lqcd_ctx lqcd_ctx;
 
 #define LQCD_SOLVER_BICGSTAB 0
 #define LQCD_SOLVER_GCR_DD   1
-#define LQCD_SOLVER_CGNE     3   /* Craig's method: CG on Mhat Mhat^dag y = bhat, x = Mhat^dag y (PAPER.md:128) */
 #define LQCD_SOLVER_CGNR     2   /* CG on Mhat^dag Mhat x = Mhat^dag bhat, mixed precision, reliable updates */
+#define LQCD_SOLVER_CGNE     3   /* Craig's method: CG on Mhat Mhat^dag y = bhat, x = Mhat^dag y (PAPER.md:128) */
 
 #define LQCD_MATPC_ASYMMETRIC 0
 #define LQCD_MATPC_SYMMETRIC  1
