@@ -290,7 +290,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   cudaDeviceProp prop;
   cudaGetDeviceProperties(&prop, device);
   c->n_sm = prop.multiProcessorCount;
-  c->partials_doubles = (size_t)c->n_sm * 8 * 16 + 4096;
+  c->partials_doubles = (size_t)c->n_sm * LQ_BLAS_CTAS_PER_SM * 16 + 4096;
   // scalars / partials for LQCD_MAX_RHS right-hand sides (batched solves; a single solve uses set 0)
   bool ok = cudaMalloc((void**)&c->S, (size_t)LQCD_MAX_RHS * S_TOTAL * sizeof(double)) == cudaSuccess &&
             cudaMalloc((void**)&c->partials, (size_t)LQCD_MAX_RHS * c->partials_doubles * sizeof(double)) == cudaSuccess &&

@@ -13,6 +13,9 @@
 namespace lq {
 
 #define LQ_BLAS_BLOCK 256
+#ifndef LQ_BLAS_CTAS_PER_SM
+#define LQ_BLAS_CTAS_PER_SM 8     /* grid of the grid-stride BLAS-1 kernels = this x number of SMs */
+#endif
 #define LQ_MAX_VEC 5
 #define LQ_GCR_KMAX 32
 

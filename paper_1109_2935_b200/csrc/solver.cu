@@ -52,7 +52,7 @@ BlasArgs mk(lqcd_ctx* c, bool blocked, char* v0 = nullptr, char* v1 = nullptr, c
 
 template <class Op>
 int blas(lqcd_ctx* c, int prec, const BlasArgs& a, cudaStream_t s) {
-  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s);
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * LQ_BLAS_CTAS_PER_SM, s);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "blas launch", e);
 }
@@ -455,10 +455,10 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
       m.k = k;
       for (int i0 = 0; i0 < k; i0 += 8) {
         m.i0 = i0; m.n = (k - i0 < 8) ? k - i0 : 8;
-        cudaError_t e = run_gcr_dots(ps, m, c->n_sm * 8, s); c->launches++;
+        cudaError_t e = run_gcr_dots(ps, m, c->n_sm * LQ_BLAS_CTAS_PER_SM, s); c->launches++;
         if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "gcr dots", e);
       }
-      { cudaError_t e = run_gcr_orth(ps, m, c->n_sm * 8, s); c->launches++;
+      { cudaError_t e = run_gcr_orth(ps, m, c->n_sm * LQ_BLAS_CTAS_PER_SM, s); c->launches++;
         if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "gcr orth", e); }
       { BlasArgs a = mk(c, false, zh[k], rh); if ((rc = blas<OpGcrScale>(c, ps, a, s))) return rc; }
       cnt.blas_flop_sites += 12.0 * (16.0 * k + 12 + 14);
@@ -511,7 +511,7 @@ BlasArgs mkr(lqcd_ctx* c, int r, char* v0 = nullptr, char* v1 = nullptr, char* v
 }
 template <class Op>
 int blasb(lqcd_ctx* c, int prec, const BlasArgs& a, int nrhs, cudaStream_t s) {
-  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s, nrhs);
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * LQ_BLAS_CTAS_PER_SM, s, nrhs);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "batched blas launch", e);
 }

@@ -180,7 +180,7 @@ BlasArgs mks(lqcd_ctx* c, char* v0 = nullptr, char* v1 = nullptr, char* v2 = nul
   return a;
 }
 template <class Op> int sblas(lqcd_ctx* c, int prec, const BlasArgs& a, cudaStream_t s) {
-  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * 8, s, 1);
+  cudaError_t e = run_blas<Op>(prec, a, c->n_sm * LQ_BLAS_CTAS_PER_SM, s, 1);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "staggered blas launch", e);
 }
