@@ -290,13 +290,24 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
 // Mhat half r12 234.4 / 228.3 / 233.0 us, Dslash fp32 r12 97.7 / 97.5 / 100.2 us.  At 6 (80 registers)
 // the clover-epilogue variants spill 60-230 bytes per thread, and with the L1 carved out for the
 // staging ring those spills miss L1 (ncu: 3 % hit rate) and travel to L2: the MR-step kernel lost
-// 30 us of 150 to them.  fp64 takes the registers it needs (1 CTA minimum).
+// 30 us of 150 to them.
+// fp64: 3 CTAs/SM (168 registers), except the recon-12 clover-epilogue variants, which spill 40-90 bytes at 3 and
+// keep 2.  Measured at 32^3x64 (2 -> 3 CTAs/SM): Dslash r18 247 -> 245, r12 211 -> 191.5, r8 283 -> 270 us;
+// Mhat r18 696 -> 691, r8 796 -> 679, r12 601 -> 614 us (hence the exception).
 #ifndef LQ_DSLASH_MINB64
-#define LQ_DSLASH_MINB64 2
+#define LQ_DSLASH_MINB64 3
+#endif
+#ifndef LQ_DSLASH_MINB64_CLOV12
+#define LQ_DSLASH_MINB64_CLOV12 2
 #endif
 #ifndef LQ_DSLASH_MINB
 #define LQ_DSLASH_MINB 5
 #endif
+
+template <class P, int RECON, bool CLOVX, bool CLOVOUT> constexpr int dslash_minb() {
+  if (sizeof(typename P::real) != 8) return LQ_DSLASH_MINB;
+  return ((CLOVX || CLOVOUT) && RECON == 12) ? LQ_DSLASH_MINB64_CLOV12 : LQ_DSLASH_MINB64;
+}
 
 // bytes of one staging buffer (one hop of every thread of the CTA): link + neighbour spinor (+ norm)
 template <class P, int RECON> struct HopStage {
@@ -313,7 +324,7 @@ template <class P, int RECON> struct HopStage {
 // DAG: -1 = dagger read from the arguments at run time (fp64, fp32); 0 / 1 = compile-time dagger (half precision:
 // the fixed-point projection fused with the decode needs the sign of every combination at compile time).
 template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST, int DAG = -1>
-__global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (sizeof(typename P::real) == 8 ? LQ_DSLASH_MINB64 : LQ_DSLASH_MINB))
+__global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (dslash_minb<P, RECON, CLOVX, CLOVOUT>()))
 dslash_kernel(const DslashArgs a) {
   static_assert(P::HALF ? (DAG == 0 || DAG == 1) : DAG == -1, "compile-time dagger for half precision only");
   typedef typename P::real R;
