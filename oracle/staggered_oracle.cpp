@@ -76,7 +76,7 @@ inline long hop(const Lat& lat, const int* c, int mu, int step, double* sign) {
 
 // out = D in  (R13)
 void stag_dslash(cplx* out, const cplx* in, const cplx* fat, const cplx* lng, const Lat& lat) {
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(lat.V >= 2048) schedule(static)
   for (long s = 0; s < lat.V; ++s) {
     int c[4];
     lat.coords(s, c);
@@ -109,7 +109,7 @@ void stag_M(cplx* out, const cplx* in, const cplx* fat, const cplx* lng, const L
   stag_dslash(out, in, fat, lng, lat);
   const double h = dagger ? 0.5 : -0.5;
   const long n = lat.V * 3;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(n >= 16384) schedule(static)
   for (long i = 0; i < n; ++i) out[i] = h * out[i] + mass * in[i];
 }
 
@@ -119,19 +119,19 @@ void stag_MdagM(cplx* out, const cplx* in, const cplx* fat, const cplx* lng, con
   std::vector<cplx> t(n);
   stag_M(t.data(), in, fat, lng, lat, mass, 0);
   stag_M(out, t.data(), fat, lng, lat, mass, 1);
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(n >= 16384) schedule(static)
   for (long i = 0; i < n; ++i) out[i] += sigma * in[i];
 }
 
 double norm2(const cplx* a, long n) {
   double s = 0;
-#pragma omp parallel for reduction(+:s) schedule(static)
+#pragma omp parallel for if(n >= 16384) reduction(+:s) schedule(static)
   for (long i = 0; i < n; ++i) s += std::norm(a[i]);
   return s;
 }
 double rdot(const cplx* a, const cplx* b, long n) {       // Re <a,b>
   double s = 0;
-#pragma omp parallel for reduction(+:s) schedule(static)
+#pragma omp parallel for if(n >= 16384) reduction(+:s) schedule(static)
   for (long i = 0; i < n; ++i) s += (std::conj(a[i]) * b[i]).real();
   return s;
 }

@@ -19,7 +19,8 @@
 //       U[mu][site][row][col],  mu = 0:x 1:y 2:z 3:t,  U_mu(x) multiplies psi(x+mu)
 //   * no checkerboard storage: parity operators are obtained by masking
 //   * no gauge compression, no spin-projection trick: full 4x4 (1 -/+ gamma_mu)
-//   * no blocking, fusion or reordering; OpenMP over the site loop only.
+//   * no blocking, fusion or reordering; OpenMP over the site loop only, and only from 2048 sites up
+//     (on the 4^4 pin lattices the thread start-up of ~25,000 tiny calls dominated the CPU test time).
 //
 // Readings of the paper (it is silent on all of these):
 //   R1  P^{+-mu} = 1 +- gamma_mu  (unnormalised; Eq. 2's -1/2 makes it a projector)
@@ -135,7 +136,7 @@ inline bool same_block(const int* blk, const int c[4], int mu, int d, const Lat&
 // dagger: (1 -/+ g_mu) exchanged.  blk: Dirichlet cut (R7) or nullptr.
 void dslash(cplx* out, const cplx* in, const cplx* U, const Lat& lat, int dagger, const int* blk) {
   const long V = lat.V;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(V >= 2048) schedule(static)
   for (long s = 0; s < V; ++s) {
     int c[4]; lat.coords(s, c);
     cplx acc[4][3];
@@ -180,7 +181,7 @@ void clover_term(cplx* T, const cplx* U, const Lat& lat, double c_sw) {
     for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b)
       isig[mu][nu][a][b] = I_ * (I_ / 2.0) * (ab[a][b] - ba[a][b]);
   }
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(V >= 2048) schedule(static)
   for (long s = 0; s < V; ++s) {
     int c[4]; lat.coords(s, c);
     cplx* Ts = T + s * 144;
@@ -248,7 +249,7 @@ void solve12(const cplx* A, const cplx* rhs, cplx* y) {
 // out = A in or A^{-1} in with A = 1 + kappa*T  (R3); mask: -1 all sites, else only that parity
 void clover_apply(cplx* out, const cplx* in, const cplx* T, const Lat& lat, double kappa, int inverse, int par) {
   const long V = lat.V;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(V >= 2048) schedule(static)
   for (long s = 0; s < V; ++s) {
     int c[4]; lat.coords(s, c);
     if (par >= 0 && lat.parity(c) != par) { for (int i = 0; i < 12; ++i) out[s*12+i] = 0; continue; }
@@ -265,7 +266,7 @@ void clover_apply(cplx* out, const cplx* in, const cplx* T, const Lat& lat, doub
 }
 
 void mask_parity(cplx* v, const Lat& lat, int keep) {
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(lat.V >= 2048) schedule(static)
   for (long s = 0; s < lat.V; ++s) {
     int c[4]; lat.coords(s, c);
     if (lat.parity(c) != keep) for (int i = 0; i < 12; ++i) v[s*12+i] = 0;
@@ -287,7 +288,7 @@ void apply_M(cplx* out, const cplx* in, const Op& op, int dagger) {
   dslash(d.data(), in, op.U, op.lat, dagger, op.blk);
   clover_apply(out, in, op.T, op.lat, op.kappa, 0, -1);
   const long n = op.n();
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(n >= 16384) schedule(static)
   for (long i = 0; i < n; ++i) out[i] -= op.kappa * d[i];
 }
 
@@ -315,7 +316,7 @@ void apply_matpc_sym(cplx* out, const cplx* in, const Op& op, int p, int dagger)
     mask_parity(t2.data(), op.lat, p);
   }
   const double k2 = op.kappa * op.kappa;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(n >= 16384) schedule(static)
   for (long i = 0; i < n; ++i) out[i] = xin[i] - k2 * t2[i];
 }
 
@@ -331,14 +332,14 @@ void apply_matpc(cplx* out, const cplx* in, const Op& op, int p, int dagger) {
   mask_parity(t1.data(), op.lat, p);
   clover_apply(out, xin.data(), op.T, op.lat, op.kappa, 0, p);
   const double k2 = op.kappa * op.kappa;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for if(n >= 16384) schedule(static)
   for (long i = 0; i < n; ++i) out[i] -= k2 * t1[i];
 }
 
 // ---- linear algebra on full-lattice arrays -------------------------------------
 cplx cdot(const cplx* a, const cplx* b, long n) {       // <a,b> = sum conj(a) b
   double re = 0, im = 0;
-#pragma omp parallel for reduction(+:re,im) schedule(static)
+#pragma omp parallel for if(n >= 16384) reduction(+:re,im) schedule(static)
   for (long i = 0; i < n; ++i) { cplx t = std::conj(a[i]) * b[i]; re += t.real(); im += t.imag(); }
   return cplx(re, im);
 }

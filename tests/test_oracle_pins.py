@@ -205,11 +205,12 @@ def test_clover_structure(small):
 
 
 # --------------------------------------------- dense linear algebra on 2^4 and 4^4 (c.5, c.7, c.9)
-def _dense(apply, shape):
+def _dense(apply, shape, cols=None):
+    """Dense matrix of a linear map, column by column (only the columns `cols` if given; the others stay 0)."""
     n = int(np.prod(shape))
-    Mat = np.empty((n, n), dtype=np.complex128)
+    Mat = np.empty((n, n), dtype=np.complex128) if cols is None else np.zeros((n, n), dtype=np.complex128)
     e = np.zeros(n, dtype=np.complex128)
-    for j in range(n):
+    for j in (range(n) if cols is None else cols):
         e[j] = 1.0
         Mat[:, j] = apply(e.reshape(shape)).ravel()
         e[j] = 0.0
@@ -363,10 +364,10 @@ def test_symmetric_even_odd_form(four):
     for p in (0, 1):
         mask = (par == p)[..., None, None]
         idx = np.flatnonzero(np.broadcast_to(mask, b.shape).ravel())
-        Mh = _dense(lambda v: oracle.matpc(v, U, Tcl, BC, kappa, p), b.shape)[np.ix_(idx, idx)]
-        Ms = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p), b.shape)[np.ix_(idx, idx)]
-        Msd = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p, dagger=True), b.shape)[np.ix_(idx, idx)]
-        A = _dense(lambda v: oracle.clover_apply(v, Tcl, kappa, parity=p), b.shape)[np.ix_(idx, idx)]
+        Mh = _dense(lambda v: oracle.matpc(v, U, Tcl, BC, kappa, p), b.shape, idx)[np.ix_(idx, idx)]
+        Ms = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p), b.shape, idx)[np.ix_(idx, idx)]
+        Msd = _dense(lambda v: oracle.matpc_sym(v, U, Tcl, BC, kappa, p, dagger=True), b.shape, idx)[np.ix_(idx, idx)]
+        A = _dense(lambda v: oracle.clover_apply(v, Tcl, kappa, parity=p), b.shape, idx)[np.ix_(idx, idx)]
         assert np.linalg.norm(A @ Ms - Mh) <= 1e-13 * np.linalg.norm(Mh)
         assert np.linalg.norm(Msd - Ms.conj().T) <= 1e-13 * np.linalg.norm(Ms)
     Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
