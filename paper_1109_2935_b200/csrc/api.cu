@@ -79,11 +79,24 @@ int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, 
   if (blocked && !c->have_blocks) return fail(c, LQCD_ESTATE, "no Schwarz blocking set");
   char*& slot = blocked ? c->bgauge[prec][ri] : c->gauge[prec][ri];
   if (!slot) {
-    int rc = dev_alloc(c, (void**)&slot, gauge_bytes(prec, recon, c->nat.ns));
+    // built into a local and published only when it holds valid links; the stream is synchronised once, so the copy
+    // is complete for every stream that uses it later
+    char* g = nullptr;
+    int rc = dev_alloc(c, (void**)&g, gauge_bytes(prec, recon, c->nat.ns));
     if (rc) return rc;
-    cudaError_t e = run_convert_gauge(prec, recon, slot, c->g64, c->bm, blocked ? 1 : 0, s);
+    unsigned bad = 0;
+    cudaError_t e = cudaMemsetAsync(c->gflag, 0, sizeof(unsigned), s);
+    if (e == cudaSuccess) e = run_convert_gauge(prec, recon, g, c->g64, c->bm, blocked ? 1 : 0, s, c->gflag);
     c->launches++;
-    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "convert_gauge", e);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, c->gflag, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cudaFree(g); return fail(c, LQCD_ECUDA, "convert_gauge", e); }
+    if (bad) {
+      cudaFree(g);
+      return fail(c, LQCD_EINVAL, (bad & 1u) ? "gauge links are not SU(3) to 1e-9: use recon 18 (recon 12 / 8 reconstruct unitary links only)"
+                                            : "recon 8 cannot represent this gauge field: a link has |a2|^2 + |a3|^2 = 0 in the stored precision (e.g. U = 1); use recon 12 or 18");
+    }
+    slot = g;
   }
   *out = slot;
   return LQCD_OK;
@@ -96,14 +109,18 @@ int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A
   if (!(c->kappa == kappa)) { drop_clover_copies(c); c->kappa = kappa; }
   char*& a = blocked ? c->bclov[prec] : c->clov[prec];
   char*& ai = blocked ? c->bclovinv[prec] : c->clovinv[prec];
-  if (!a) {
-    int rc = dev_alloc(c, (void**)&a, clover_bytes(prec, c->nat.ns));
+  if (!a || !ai) {
+    char *na = nullptr, *nai = nullptr;       // published only when both hold valid data (see get_gauge)
+    int rc = dev_alloc(c, (void**)&na, clover_bytes(prec, c->nat.ns));
     if (rc) return rc;
-    rc = dev_alloc(c, (void**)&ai, clover_bytes(prec, c->nat.ns));
-    if (rc) return rc;
-    cudaError_t e = run_clover_make(prec, a, ai, c->T72, c->bm, blocked ? 1 : 0, kappa, s);
+    rc = dev_alloc(c, (void**)&nai, clover_bytes(prec, c->nat.ns));
+    if (rc) { cudaFree(na); return rc; }
+    cudaError_t e = run_clover_make(prec, na, nai, c->T72, c->bm, blocked ? 1 : 0, kappa, s);
     c->launches++;
-    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "clover_make", e);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cudaFree(na); cudaFree(nai); return fail(c, LQCD_ECUDA, "clover_make", e); }
+    free_p(a); free_p(ai);
+    a = na; ai = nai;
   }
   *A = a; *Ainv = ai;
   return LQCD_OK;
@@ -237,10 +254,8 @@ int op_matpc_mrhs(lqcd_ctx* c, char* out, const char* in, int nrhs, int parity, 
                   cudaStream_t s) {
   const size_t need = spinor_bytes(prec, c->nat.ns) * (size_t)nrhs;
   if (c->mtmp_bytes < need) {
-    if (c->mtmp) cudaFree(c->mtmp);
-  for (void* p : {(void*)c->sfat64, (void*)c->slng64, (void*)c->sfatp[0], (void*)c->sfatp[1], (void*)c->slngp[0], (void*)c->slngp[1], (void*)c->stmp[0], (void*)c->stmp[1]}) if (p) cudaFree(p);                   // synchronises: no launch still uses the old buffer
+    if (c->mtmp) cudaFree(c->mtmp);                   // synchronises: no launch still uses the old buffer
     c->mtmp = nullptr; c->mtmp_bytes = 0;
-  c->have_stag = false; c->sfat64 = c->slng64 = nullptr; c->sfatp[0] = c->sfatp[1] = c->slngp[0] = c->slngp[1] = nullptr; c->slong_scale = 0; c->stmp[0] = c->stmp[1] = nullptr;
     int rc = dev_alloc(c, (void**)&c->mtmp, need);
     if (rc) return rc;
     c->mtmp_bytes = need;
@@ -283,6 +298,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   memset(c->tmp, 0, sizeof(c->tmp)); memset(c->btmp, 0, sizeof(c->btmp)); memset(c->tmp2, 0, sizeof(c->tmp2));
   c->S = nullptr; c->partials = nullptr; c->counters = nullptr; c->boxdots = nullptr; c->hS = nullptr;
   c->boxdots_doubles = 0;
+  c->gflag = nullptr;
   memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
   c->have_hpipe = false;
   c->mtmp = nullptr; c->mtmp_bytes = 0;
@@ -295,6 +311,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   bool ok = cudaMalloc((void**)&c->S, (size_t)LQCD_MAX_RHS * S_TOTAL * sizeof(double)) == cudaSuccess &&
             cudaMalloc((void**)&c->partials, (size_t)LQCD_MAX_RHS * c->partials_doubles * sizeof(double)) == cudaSuccess &&
             cudaMalloc((void**)&c->counters, 4096 * sizeof(unsigned)) == cudaSuccess &&
+            cudaMalloc((void**)&c->gflag, sizeof(unsigned)) == cudaSuccess &&
             cudaMallocHost((void**)&c->hS, (size_t)(S_TOTAL + 4 * LQCD_MAX_RHS) * sizeof(double)) == cudaSuccess;
   if (ok) ok = cudaMemset(c->S, 0, (size_t)LQCD_MAX_RHS * S_TOTAL * sizeof(double)) == cudaSuccess &&
                cudaMemset(c->counters, 0, 4096 * sizeof(unsigned)) == cudaSuccess;
@@ -314,6 +331,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->S) cudaFree(c->S);
   if (c->partials) cudaFree(c->partials);
   if (c->counters) cudaFree(c->counters);
+  if (c->gflag) cudaFree(c->gflag);
   if (c->boxdots) cudaFree(c->boxdots);
   if (c->hS) cudaFreeHost(c->hS);
   for (auto& b : c->pool) cudaFree(b.p);

@@ -88,11 +88,14 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_orth_kernel(const MultiArgs
   reduce_and_finalize<3>(red, a, 0, [&](const double* s) {
     double* S = a.S;
     const double gamma = sqrt(s[0]);
+    // z_k = 0 exactly (rhat = 0, or p_k in the span of the earlier directions): alpha_k = 0 and the
+    // direction drops out of the update; OpGcrScale and the host's back-substitution skip the division
+    const double ig = gamma > 0.0 ? 1.0 / gamma : 0.0;
     S[S_GCR_ZZ] = s[0];
     S[S_GCR_GAMMA] = gamma;
-    S[S_GCR_ALPHA] = s[1] / gamma; S[S_GCR_ALPHA + 1] = s[2] / gamma;
+    S[S_GCR_ALPHA] = s[1] * ig; S[S_GCR_ALPHA + 1] = s[2] * ig;
     S[S_GCR_GAMMAS + m.k] = gamma;
-    S[S_GCR_ALPHAS + 2 * m.k] = s[1] / gamma; S[S_GCR_ALPHAS + 2 * m.k + 1] = s[2] / gamma;
+    S[S_GCR_ALPHAS + 2 * m.k] = s[1] * ig; S[S_GCR_ALPHAS + 2 * m.k + 1] = s[2] * ig;
   });
 }
 

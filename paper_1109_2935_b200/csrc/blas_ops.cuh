@@ -314,7 +314,8 @@ struct OpGcrScale {        // v0 = z_k, v1 = rhat : z_k /= gamma ; rhat -= alpha
   static constexpr int NV = 1, READ = 3, WRITE = 3;
   struct Coef { double ig, ar, ai; };
   LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int) {
-    c.ig = 1.0 / a.S[S_GCR_GAMMA]; c.ar = a.S[S_GCR_ALPHA]; c.ai = a.S[S_GCR_ALPHA + 1];
+    const double g = a.S[S_GCR_GAMMA];
+    c.ig = g > 0.0 ? 1.0 / g : 0.0; c.ar = a.S[S_GCR_ALPHA]; c.ai = a.S[S_GCR_ALPHA + 1];
   }
   template <typename R> LQ_DEV static void site(const Coef& c, R* z, R* r, R*, R*, R*, double* red) {
     const R ig = (R)c.ig;

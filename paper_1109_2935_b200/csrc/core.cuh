@@ -157,13 +157,36 @@ template <class P> __host__ __device__ constexpr int site_bytes(int n, bool with
 LQ_DEV float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 LQ_DEV double fma_(double a, double b, double c) { return fma(a, b, c); }
 
+// ---------------------------------------------------------------- packed fp32 pairs (FFMA2 / FADD2 / FMUL2, sm_100)
+// A complex number (re, im) held in one aligned 64-bit register pair.  The fp32-arithmetic kernels are bound by
+// register-file bandwidth, not by the FMA lanes: a scalar FFMA reads three registers and, measured on B200 with
+// the SU(3) x half-spinor product of dslash.cuh, sustains 0.62 FFMA/clk/scheduler; the packed form
+//   (re, im) += u.re * (h.re, h.im);   (re, im) += u.im * (-h.im, h.re)
+// is two FFMA2 whose scalar factor is a broadcast operand (.F32) and whose swapped / half-negated pair is an operand
+// modifier (.LO_HI, .NP / .PN) -- ptxas folds f2_make(u, u) and f2_make(-b, a) into those -- and sustains 0.85
+// FMA-equivalents/clk (175 -> 128 clk per hop).  Each lane is an IEEE fma, so results are
+// bit-identical to the scalar sequence with the same per-component order.
+typedef unsigned long long f2;
+LQ_DEV f2 f2_make(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+LQ_DEV f2 f2_bcast(float x) { return f2_make(x, x); }
+LQ_DEV void f2_split(f2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+LQ_DEV f2 f2_fma(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+LQ_DEV f2 f2_mul(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+LQ_DEV f2 f2_add(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
 // the two 16-bit fields of w as floats holding the signed integers q
 LQ_DEV float fixed_lo(unsigned w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - LQ_MAGIC_DEC; }
 LQ_DEV float fixed_hi(unsigned w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - LQ_MAGIC_DEC; }
+// both fields of w at once: two PRMT and one FADD2
+LQ_DEV void fixed_pair(unsigned w, float& lo, float& hi) {
+  const f2 m = f2_make(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)));
+  f2_split(f2_add(m, f2_bcast(-LQ_MAGIC_DEC)), lo, hi);
+}
 // pack rint(a*sc), rint(b*sc) (|.| <= 32767) as two offset-binary 16-bit fields
 LQ_DEV unsigned fixed_pack(float a, float b, float sc) {
-  const unsigned ua = __float_as_uint(fmaf(a, sc, LQ_MAGIC_ENC)), ub = __float_as_uint(fmaf(b, sc, LQ_MAGIC_ENC));
-  return __byte_perm(ua, ub, 0x5410);
+  float ea, eb;
+  f2_split(f2_fma(f2_make(a, b), f2_bcast(sc), f2_bcast(LQ_MAGIC_ENC)), ea, eb);
+  return __byte_perm(__float_as_uint(ea), __float_as_uint(eb), 0x5410);
 }
 
 // ---------------------------------------------------------------- site vectors with a norm (spinor: 24, clover: 72)
@@ -181,7 +204,7 @@ LQ_DEV void load_site_raw(typename P::real* __restrict__ v, typename P::real& sc
     const int* np = reinterpret_cast<const int*>(f + (long long)(2 * N) * ns) + i;
     scale = __int_as_float(MODE == 2 ? ld_shared(np) : ld_nc(np)) * LQ_FIXED_INV;
 #pragma unroll
-    for (int k = 0; k < N / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
+    for (int k = 0; k < N / 2; ++k) fixed_pair(w[k], v[2 * k], v[2 * k + 1]);
   }
 }
 
@@ -254,7 +277,7 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
     alignas(16) unsigned w[RECON / 2];
     Rec<unsigned, RECON / 2>::template load<MODE>(w, g, ns, i);
 #pragma unroll
-    for (int k = 0; k < RECON / 2; ++k) { v[2 * k] = fixed_lo(w[k]); v[2 * k + 1] = fixed_hi(w[k]); }
+    for (int k = 0; k < RECON / 2; ++k) fixed_pair(w[k], v[2 * k], v[2 * k + 1]);
     if constexpr (RECON == 8) {
 #pragma unroll
       for (int k = 0; k < 6; ++k) v[k] *= LQ_FIXED_INV;
@@ -270,6 +293,25 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
   if constexpr (RECON == 18) {
 #pragma unroll
     for (int k = 0; k < 18; ++k) u[k] = v[k];
+  } else if constexpr (RECON == 12 && sizeof(R) == 4) {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) u[k] = v[k];
+    // row2 = conj(row0 x row1), packed: (re, im) of conj(a_j b_k - a_k b_j) in four FFMA2 (a = row 0, b = row 1)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int j = (c + 1) % 3, k = (c + 2) % 3;
+      const float ajr = u[2 * j], aji = u[2 * j + 1], akr = u[2 * k], aki = u[2 * k + 1];
+      const float bjr = u[6 + 2 * j], bji = u[6 + 2 * j + 1], bkr = u[6 + 2 * k], bki = u[6 + 2 * k + 1];
+      f2 t = f2_mul(f2_make(bkr, -bki), f2_bcast(ajr));
+      t = f2_fma(f2_make(-bki, -bkr), f2_bcast(aji), t);
+      t = f2_fma(f2_make(-bjr, bji), f2_bcast(akr), t);
+      t = f2_fma(f2_make(bji, bjr), f2_bcast(aki), t);
+      if constexpr (P::HALF) t = f2_mul(t, f2_bcast(LQ_FIXED_INV));
+      float re, im;
+      f2_split(t, re, im);
+      u[12 + 2 * c] = re;
+      u[12 + 2 * c + 1] = im;
+    }
   } else if constexpr (RECON == 12) {
 #pragma unroll
     for (int k = 0; k < 12; ++k) u[k] = v[k];
@@ -298,7 +340,10 @@ LQ_DEV void load_link(typename P::real* __restrict__ u, typename P::real& uscale
     const R a1m2 = fmax(R(0), R(1) - N);
     const R a1m = sqrt_(a1m2);
     const cx<R> a1 = {a1m * c1, a1m * s1};
-    const R c1m = sqrt_(fmax(R(0), R(1) - a1m2 - b1.re * b1.re - b1.im * b1.im));
+    // |c1|^2 = 1 - |a1|^2 - |b1|^2 = N - |b1|^2 (first column has unit norm).  Written with N, not with
+    // 1 - (1 - N): the latter keeps N only to an absolute 1e-16 and loses log10(1/N) digits of c1 on links
+    // close to the identity (measured on 8^4, eps = 0.01: link error 5.6e-12 -> 4.0e-16, R10).
+    const R c1m = sqrt_(fmax(R(0), (N - b1.re * b1.re) - b1.im * b1.im));
     const cx<R> cc1 = {c1m * c2, c1m * s2};
     const R iN = R(1) / N;
     const cx<R> p = cmulc(a1, b1);        // conj(a1) b1

@@ -50,6 +50,14 @@ template <int C, typename R> LQ_DEV cx<R> unit_mul(cx<R> z) {
   return {z.im, -z.re};
 }
 
+// (re, im) of unit<C>(z) as a packed pair: the swap and the signs become operand modifiers of the consuming FFMA2
+template <int C> LQ_DEV f2 unit_pair(float re, float im) {
+  if (C == 0) return f2_make(re, im);
+  if (C == 1) return f2_make(-im, re);
+  if (C == 2) return f2_make(-re, -im);
+  return f2_make(im, -re);
+}
+
 // (gamma_mu psi)_0 = c0 psi_{j0}, (gamma_mu psi)_1 = c1 psi_{j1} in the DeGrand-Rossi basis (R2)
 template <int MU> struct GammaRow;
 template <> struct GammaRow<0> { static constexpr int j0 = 3, c0 = 1, j1 = 2, c1 = 1; };   // gamma_x
@@ -70,10 +78,16 @@ LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restr
   cx<R> h[2][3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const cx<R> q0 = unit_mul<G::c0>(cx<R>{psi[6 * G::j0 + 2 * c], psi[6 * G::j0 + 2 * c + 1]});
-    const cx<R> q1 = unit_mul<G::c1>(cx<R>{psi[6 * G::j1 + 2 * c], psi[6 * G::j1 + 2 * c + 1]});
-    h[0][c] = {fma_(sigma, q0.re, psi[2 * c]), fma_(sigma, q0.im, psi[2 * c + 1])};
-    h[1][c] = {fma_(sigma, q1.re, psi[6 + 2 * c]), fma_(sigma, q1.im, psi[6 + 2 * c + 1])};
+    if constexpr (sizeof(R) == 4) {
+      const f2 sg = f2_bcast(sigma);
+      f2_split(f2_fma(sg, unit_pair<G::c0>(psi[6 * G::j0 + 2 * c], psi[6 * G::j0 + 2 * c + 1]), f2_make(psi[2 * c], psi[2 * c + 1])), h[0][c].re, h[0][c].im);
+      f2_split(f2_fma(sg, unit_pair<G::c1>(psi[6 * G::j1 + 2 * c], psi[6 * G::j1 + 2 * c + 1]), f2_make(psi[6 + 2 * c], psi[6 + 2 * c + 1])), h[1][c].re, h[1][c].im);
+    } else {
+      const cx<R> q0 = unit_mul<G::c0>(cx<R>{psi[6 * G::j0 + 2 * c], psi[6 * G::j0 + 2 * c + 1]});
+      const cx<R> q1 = unit_mul<G::c1>(cx<R>{psi[6 * G::j1 + 2 * c], psi[6 * G::j1 + 2 * c + 1]});
+      h[0][c] = {fma_(sigma, q0.re, psi[2 * c]), fma_(sigma, q0.im, psi[2 * c + 1])};
+      h[1][c] = {fma_(sigma, q1.re, psi[6 + 2 * c]), fma_(sigma, q1.im, psi[6 + 2 * c + 1])};
+    }
   }
   hop_tail<MU, FWD, R>(acc, h, u, sigma, coef);
 }
@@ -86,17 +100,24 @@ LQ_DEV void hop(R* __restrict__ acc, const R* __restrict__ psi, const R* __restr
 // instead of two decoding FADDs and one FFMA: 1.5 instead of 3 instructions per projected real.  Which
 // of the two applies to a component depends on sigma, so the dagger flag is a template parameter of the
 // half-precision kernels.  Results are bit-identical to decode-then-project.
-template <int S> LQ_DEV float fixed_sum(float ma, float mb) {
-  if (S < 0) return ma - mb;
-  return (ma - 2.0f * LQ_MAGIC_DEC) + mb;
-}
+// Packed (core.cuh, f2): both components of a projected complex number at once.  With signs (SRE, SIM):
+//   (-,-): A + (-X)                      one FADD2
+//   else : (A + K) + X',  K = -2(2^23+32768) in the '+' components and 0 in the '-' ones (adding 0 is exact),
+//          X' = X with the '-' components negated        two FADD2
 // (a + SG * unit<C>(b)) on magic floats: unit<0> = 1, <1> = i, <2> = -1, <3> = -i
 template <int C, int SG> LQ_DEV cx<float> fixed_project(float ar, float ai, float br, float bi) {
   constexpr int SRE = SG * ((C == 0 || C == 3) ? 1 : -1);
   constexpr int SIM = SG * ((C == 0 || C == 1) ? 1 : -1);
   const float xr = (C == 0 || C == 2) ? br : bi;
   const float xi = (C == 0 || C == 2) ? bi : br;
-  return {fixed_sum<SRE>(ar, xr), fixed_sum<SIM>(ai, xi)};
+  const f2 A = f2_make(ar, ai);
+  const f2 X = f2_make(SRE < 0 ? -xr : xr, SIM < 0 ? -xi : xi);
+  f2 r;
+  if (SRE < 0 && SIM < 0) r = f2_add(A, X);
+  else r = f2_add(f2_add(A, f2_make(SRE < 0 ? 0.0f : -2.0f * LQ_MAGIC_DEC, SIM < 0 ? 0.0f : -2.0f * LQ_MAGIC_DEC)), X);
+  cx<float> o;
+  f2_split(r, o.re, o.im);
+  return o;
 }
 template <int MU, bool FWD, int SG>
 LQ_DEV void hop_fixed(float* __restrict__ acc, const float* __restrict__ m, const float* __restrict__ u, float coef) {
@@ -110,9 +131,56 @@ LQ_DEV void hop_fixed(float* __restrict__ acc, const float* __restrict__ m, cons
   hop_tail<MU, FWD, float>(acc, h, u, (float)SG, coef);
 }
 
+// fp32 arithmetic: packed complex form (core.cuh, f2): 2 FFMA2 per complex multiply-add, same per-component order
+// of operations as the scalar form below (bit-identical results)
+template <int MU, bool FWD>
+LQ_DEV void hop_tail_packed(float* __restrict__ acc, const cx<float> (&h)[2][3], const float* __restrict__ u, float sigma, float coef) {
+  typedef GammaRow<MU> G;
+  f2 w[2][3];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+      f2 t;
+      if (FWD) {                         // sum_k U[r][k] * h[k]
+        t = f2_mul(f2_make(h[s][0].re, h[s][0].im), f2_bcast(u[6 * r]));
+        t = f2_fma(f2_make(-h[s][0].im, h[s][0].re), f2_bcast(u[6 * r + 1]), t);
+#pragma unroll
+        for (int k = 1; k < 3; ++k) {
+          t = f2_fma(f2_make(h[s][k].re, h[s][k].im), f2_bcast(u[6 * r + 2 * k]), t);
+          t = f2_fma(f2_make(-h[s][k].im, h[s][k].re), f2_bcast(u[6 * r + 2 * k + 1]), t);
+        }
+      } else {                           // sum_k conj(U[k][r]) * h[k]
+        t = f2_mul(f2_make(h[s][0].re, h[s][0].im), f2_bcast(u[2 * r]));
+        t = f2_fma(f2_make(h[s][0].im, -h[s][0].re), f2_bcast(u[2 * r + 1]), t);
+#pragma unroll
+        for (int k = 1; k < 3; ++k) {
+          t = f2_fma(f2_make(h[s][k].re, h[s][k].im), f2_bcast(u[6 * k + 2 * r]), t);
+          t = f2_fma(f2_make(h[s][k].im, -h[s][k].re), f2_bcast(u[6 * k + 2 * r + 1]), t);
+        }
+      }
+      w[s][r] = t;
+    }
+  }
+  const f2 cf = f2_bcast(coef), ss = f2_bcast(coef * sigma);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    float w0r, w0i, w1r, w1i;
+    f2_split(w[0][c], w0r, w0i);
+    f2_split(w[1][c], w1r, w1i);
+    f2_split(f2_fma(cf, w[0][c], f2_make(acc[2 * c], acc[2 * c + 1])), acc[2 * c], acc[2 * c + 1]);
+    f2_split(f2_fma(cf, w[1][c], f2_make(acc[6 + 2 * c], acc[6 + 2 * c + 1])), acc[6 + 2 * c], acc[6 + 2 * c + 1]);
+    f2_split(f2_fma(ss, unit_pair<(4 - G::c0) % 4>(w0r, w0i), f2_make(acc[6 * G::j0 + 2 * c], acc[6 * G::j0 + 2 * c + 1])),
+             acc[6 * G::j0 + 2 * c], acc[6 * G::j0 + 2 * c + 1]);
+    f2_split(f2_fma(ss, unit_pair<(4 - G::c1) % 4>(w1r, w1i), f2_make(acc[6 * G::j1 + 2 * c], acc[6 * G::j1 + 2 * c + 1])),
+             acc[6 * G::j1 + 2 * c], acc[6 * G::j1 + 2 * c + 1]);
+  }
+}
+
 template <int MU, bool FWD, typename R>
 LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef) {
   typedef GammaRow<MU> G;
+  if constexpr (sizeof(R) == 4) { hop_tail_packed<MU, FWD>(acc, h, u, sigma, coef); return; }
   // colour multiply: 6 FMA per real output
   cx<R> w[2][3];
 #pragma unroll
@@ -157,6 +225,26 @@ LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __res
 // lower-triangle entries (i>j) at 6 + 2*(i(i-1)/2 + j).  504 flop (PAPER.md:138 fn.1: 72 reals).
 template <typename R>
 LQ_DEV void clover_block(R* __restrict__ o, const R* __restrict__ x, const R* __restrict__ c) {
+  if constexpr (sizeof(R) == 4) {        // packed complex form (core.cuh, f2); same per-component order as below
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      f2 t = f2_mul(f2_make(x[2 * i], x[2 * i + 1]), f2_bcast(c[i]));
+#pragma unroll
+      for (int j = 0; j < 6; ++j) {
+        if (j < i) {
+          const float lr = c[6 + 2 * (i * (i - 1) / 2 + j)], li = c[6 + 2 * (i * (i - 1) / 2 + j) + 1];
+          t = f2_fma(f2_make(x[2 * j], x[2 * j + 1]), f2_bcast(lr), t);
+          t = f2_fma(f2_make(-x[2 * j + 1], x[2 * j]), f2_bcast(li), t);
+        } else if (j > i) {
+          const float lr = c[6 + 2 * (j * (j - 1) / 2 + i)], li = c[6 + 2 * (j * (j - 1) / 2 + i) + 1];
+          t = f2_fma(f2_make(x[2 * j], x[2 * j + 1]), f2_bcast(lr), t);
+          t = f2_fma(f2_make(x[2 * j + 1], -x[2 * j]), f2_bcast(li), t);
+        }
+      }
+      f2_split(t, o[2 * i], o[2 * i + 1]);
+    }
+    return;
+  }
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
     R re = c[i] * x[2 * i], im = c[i] * x[2 * i + 1];
@@ -282,6 +370,9 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
   }
 }
 
+#ifndef LQ_PROBE
+#define LQ_PROBE 0
+#endif
 #ifndef LQ_DSLASH_BLOCK
 #define LQ_DSLASH_BLOCK 128
 #endif
@@ -414,14 +505,14 @@ dslash_kernel(const DslashArgs a) {
         load_link<P, RECON, 2>(u, us, sb_, LQ_DSLASH_BLOCK, tid);                                          \
         if constexpr (P::HALF) load_site_magic<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid); \
         else load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);   \
-        if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                       \
+        if (!(LQ_PROBE & 1)) if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                  \
         cp_async_commit();                                                                                 \
         const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
         if constexpr (P::HALF) hop_fixed<MU_, FW_, (FW_ == (DAG == 1)) ? 1 : -1>(acc, psi, u, sg_ * us * ps); \
         else hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, sg_);                                     \
       }
 #pragma unroll
-      for (int h = 0; h < NST; ++h) {
+      for (int h = 0; h < ((LQ_PROBE & 1) ? 0 : NST); ++h) {
         switch (h) {                       // NST <= 4
           case 0: LQ_ISSUE(0) break;
           case 1: LQ_ISSUE(1) break;

@@ -1,6 +1,7 @@
 // dslash_inst.cuh -- host dispatch over (recon, epilogue) for one precision; included by
 // dslash_fp64.cu / dslash_fp32.cu / dslash_half.cu so the three precisions compile in parallel.
 #pragma once
+#include <mutex>
 #include "dslash.cuh"
 
 namespace lq {
@@ -22,11 +23,12 @@ static void launch_dag(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
   constexpr int NST = sizeof(typename P::real) == 8 ? ((CLOVX || CLOVOUT) ? 0 : LQ_PIPE_FP64) : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
   constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
   auto kern = dslash_kernel<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, NST, DAG>;
-  static bool configured_dev[64] = {};    // per instantiation and device (function attributes are per device)
+  // function attributes are per device: set once per instantiation and device (std::call_once, so that two
+  // contexts driven from two host threads cannot race on the flag)
+  static std::once_flag configured_dev[64];
   int dev = 0;
   cudaGetDevice(&dev);
-  bool& configured = configured_dev[dev & 63];
-  if (!configured) {
+  std::call_once(configured_dev[dev & 63], [&] {
     if (NST > 0) {
       cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
       cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -35,8 +37,7 @@ static void launch_dag(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
       // the previous kernel, and after a ring kernel the fp64 clover variants lost 5 % (696 -> 730 us)
       cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
     }
-    configured = true;
-  }
+  });
   kern<<<grid, block, SMEM, s>>>(a);
 }
 

@@ -47,7 +47,8 @@ cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStre
 
 // setup kernels (pack.cu, clover.cu)
 cudaError_t run_pack_gauge(double* g64, const double* U_canonical, const Geom& nat, cudaStream_t s);
-cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s);
+cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s,
+                              unsigned* bad = nullptr);   // bad: device word, bit 0 = not SU(3), bit 1 = recon-8 singular (pack.cu)
 cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
                             long long i0 = 0, long long i1 = -1);   // sites [i0, i1) of the parity field (default: all)
 cudaError_t run_clover_term(double* T72, const double* g64, const Geom& nat, double c_sw, cudaStream_t s);
@@ -95,6 +96,7 @@ struct lqcd_ctx {
   double* partials;       // reduction partials
   size_t partials_doubles;
   unsigned* counters;
+  unsigned* gflag;        // device word written by the gauge conversion check (pack.cu)
   double* boxdots;        // MR per-box partial dots
   size_t boxdots_doubles;
   double* hS;             // pinned host mirror of S

@@ -27,9 +27,13 @@ cudaError_t run_pack_gauge(double* g64, const double* U, const Geom& nat, cudaSt
   return cudaGetLastError();
 }
 
-// fp64 recon-18 natural -> (P, RECON), natural or block-major
+// fp64 recon-18 natural -> (P, RECON), natural or block-major.
+// Compressed forms hold SU(3) links only (PAPER.md:164 (a); R10), and recon-8 cannot hold a link whose first row is
+// (a1, 0, 0) (N = |a2|^2 + |a3|^2 = 0, e.g. U = 1: the lower 2x2 block is then not determined by the 8 stored reals).
+// `bad` (device word, may be null) collects: bit 0 = a link is not SU(3) to 1e-9 (unitarity or determinant),
+// bit 1 = a recon-8 link has N = 0 in the stored precision (the in-kernel reconstruction would divide by zero).
 template <class P, int RECON>
-__global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, const BlockMap bm, int blocked) {
+__global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, const BlockMap bm, int blocked, unsigned* bad) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= bm.nat.ns) return;
   const int pm = blockIdx.y, parity = pm >> 2;
@@ -42,25 +46,60 @@ __global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, 
   alignas(16) typename P::store_t q[RECON];
   quantize_link<P, RECON>(v, q);
   Rec<typename P::store_t, RECON>::store(q, dst + (long long)pm * RECON * sizeof(typename P::store_t) * bm.nat.ns, bm.nat.ns, i);
+  if (RECON != 18 && bad) {
+    unsigned f = 0;
+    // rows orthonormal, row2 = conj(row0 x row1)  <=>  U in SU(3)
+    double defect = 0;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int b = a; b < 2; ++b) {
+        double re = 0, im = 0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          re += u[6 * a + 2 * k] * u[6 * b + 2 * k] + u[6 * a + 2 * k + 1] * u[6 * b + 2 * k + 1];
+          im += u[6 * a + 2 * k + 1] * u[6 * b + 2 * k] - u[6 * a + 2 * k] * u[6 * b + 2 * k + 1];
+        }
+        defect = fmax(defect, fmax(fabs(re - (a == b ? 1.0 : 0.0)), fabs(im)));
+      }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int j = (c + 1) % 3, k = (c + 2) % 3;
+      const double re = u[2 * j] * u[6 + 2 * k] - u[2 * j + 1] * u[6 + 2 * k + 1] - u[2 * k] * u[6 + 2 * j] + u[2 * k + 1] * u[6 + 2 * j + 1];
+      const double im = u[2 * j] * u[6 + 2 * k + 1] + u[2 * j + 1] * u[6 + 2 * k] - u[2 * k] * u[6 + 2 * j + 1] - u[2 * k + 1] * u[6 + 2 * j];
+      defect = fmax(defect, fmax(fabs(re - u[12 + 2 * c]), fabs(-im - u[12 + 2 * c + 1])));
+    }
+    if (!(defect <= 1e-9)) f |= 1u;
+    if (RECON == 8) {
+      double n = 0;      // N as the Dslash kernels will see it (stored precision)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const double x = P::HALF ? (double)((int)(unsigned short)q[k] - 32768) : (double)q[k];
+        n += x * x;
+      }
+      if (!(n > (P::HALF ? 0.5 : (sizeof(typename P::real) == 8 ? 1e-290 : 1e-36)))) f |= 2u;
+    }
+    if (f) atomicOr(bad, f);
+  }
 }
 
 template <class P>
-static cudaError_t convert_gauge_p(int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s) {
+static cudaError_t convert_gauge_p(int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, unsigned* bad, cudaStream_t s) {
   dim3 grid((unsigned)((bm.nat.ns + 127) / 128), 8), block(128);
   switch (recon) {
-    case 18: convert_gauge_kernel<P, 18><<<grid, block, 0, s>>>(dst, g64, bm, blocked); break;
-    case 12: convert_gauge_kernel<P, 12><<<grid, block, 0, s>>>(dst, g64, bm, blocked); break;
-    case 8:  convert_gauge_kernel<P, 8><<<grid, block, 0, s>>>(dst, g64, bm, blocked); break;
+    case 18: convert_gauge_kernel<P, 18><<<grid, block, 0, s>>>(dst, g64, bm, blocked, bad); break;
+    case 12: convert_gauge_kernel<P, 12><<<grid, block, 0, s>>>(dst, g64, bm, blocked, bad); break;
+    case 8:  convert_gauge_kernel<P, 8><<<grid, block, 0, s>>>(dst, g64, bm, blocked, bad); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();
 }
 
-cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s) {
+cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s, unsigned* bad) {
   switch (prec) {
-    case 0: return convert_gauge_p<PrecD>(recon, dst, g64, bm, blocked, s);
-    case 1: return convert_gauge_p<PrecS>(recon, dst, g64, bm, blocked, s);
-    case 2: return convert_gauge_p<PrecH>(recon, dst, g64, bm, blocked, s);
+    case 0: return convert_gauge_p<PrecD>(recon, dst, g64, bm, blocked, bad, s);
+    case 1: return convert_gauge_p<PrecS>(recon, dst, g64, bm, blocked, bad, s);
+    case 2: return convert_gauge_p<PrecH>(recon, dst, g64, bm, blocked, bad, s);
   }
   return cudaErrorInvalidValue;
 }

@@ -2,8 +2,7 @@
 //   * mixed-precision BiCGstab with reliable updates  (reading R11)
 //   * additive-Schwarz preconditioner K = n_MR minimum-residual steps on the Dirichlet-cut
 //     Mhat_D, one alpha per block                      (reading R7)
-//   * CGNR with reliable updates                        ("CG on the normal equations")
-//   * CGNR with reliable updates                        (CG on the normal equations)
+//   * CGNR / CGNE with reliable updates                 ("CG on the normal equations")
 //   * GCR-DD, Algorithm 1                               (reading R8)
 // The host loop only launches kernels; all Krylov scalars live on the device (blas_ops.cuh).
 // One scalar (||r||^2) is read back per iteration for the convergence / restart decision.
@@ -21,6 +20,8 @@ typedef OpMrUpdate<true, false> OpMrFirst;
 typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;
 typedef OpMrUpdate<true, true> OpMrOnly;
+
+struct EventPair { cudaEvent_t a, b; ~EventPair() { cudaEventDestroy(a); cudaEventDestroy(b); } };
 
 struct Work {                      // workspace of one call; goes back to the context's cache when it leaves scope
   lqcd_ctx* c;
@@ -474,7 +475,8 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
       std::complex<double> tacc(c->hS[S_GCR_ALPHAS + 2 * l], c->hS[S_GCR_ALPHAS + 2 * l + 1]);
       for (int i = l + 1; i < k; ++i)
         tacc -= std::complex<double>(c->hS[S_GCR_BETA + 2 * (l * LQ_GCR_KMAX + i)], c->hS[S_GCR_BETA + 2 * (l * LQ_GCR_KMAX + i) + 1]) * chi[i];
-      chi[l] = tacc / c->hS[S_GCR_GAMMAS + l];
+      const double gl = c->hS[S_GCR_GAMMAS + l];
+      chi[l] = gl > 0.0 ? tacc / gl : std::complex<double>(0.0, 0.0);     // gamma_l = 0: z_l was exactly zero (blas.cu)
     }
     MultiArgs m; memset(&m, 0, sizeof(m));
     m.b = mk(c, false);
@@ -557,6 +559,8 @@ int solve_bicgstab_mrhs(lqcd_ctx* c, char* x, const char* b, int nrhs, const lqc
   for (char** q : lo) if ((rc = wk.get(q, fs * nrhs))) return rc;
   std::vector<double> rn(nrhs), maxr(nrhs);
   std::vector<int> done(nrhs, 0), status(nrhs, LQCD_OK), waiting(nrhs, 0);
+  // every return path (errors included) leaves the S_DONE flags of all sources clear for the next call
+  struct DoneGuard { lqcd_ctx* c; int n; cudaStream_t s; ~DoneGuard() { for (int r = 0; r < n; ++r) set_done(c, r, 0.0, s); } } done_guard{c, nrhs, s};
   for (int r = 0; r < nrhs; ++r) if ((rc = set_done(c, r, 0.0, s))) return rc;
   if ((rc = residual_mrhs(c, r_hi, b, x, nrhs, par, p.kappa, po, p.recon_outer, rn.data(), s))) return rc;
   cnt.mat_outer += nrhs;
@@ -645,7 +649,6 @@ int solve_bicgstab_mrhs(lqcd_ctx* c, char* x, const char* b, int nrhs, const lqc
   for (int r = 0; r < nrhs; ++r) {
     res[r].status = status[r];
     res[r].iterated_residual = rn[r];
-    if ((rc = set_done(c, r, 0.0, s))) return rc;           // leave the scalar sets clean for the next call
   }
   return LQCD_OK;
 }
@@ -701,7 +704,9 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   char *bp, *bq, *xp, *xq, *t1;
   for (char** q : {&bp, &bq, &xp, &xq, &t1}) if ((rc = wk.get(q, spinor_bytes(po, ns)))) return rc;
   cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  if (cudaEventCreate(&e0) != cudaSuccess) return fail(c, LQCD_ECUDA, "event");
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return fail(c, LQCD_ECUDA, "event"); }
+  EventPair ev{e0, e1};                 // destroyed on every return path
   cudaEventRecord(e0, s);
   Counts cnt;
   // pack b; ||b||
@@ -715,7 +720,6 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   if (bnorm == 0.0) {
     cudaMemsetAsync(x_can, 0, (size_t)c->V * 24 * sizeof(double), s);
     cudaStreamSynchronize(s);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     res->status = LQCD_OK;
     return LQCD_OK;
   }
@@ -740,7 +744,7 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   else if (p->solver == LQCD_SOLVER_CGNR) status = solve_cgnr(c, xp, bhat, *p, stop, res, cnt, s);
   else if (p->solver == LQCD_SOLVER_CGNE) status = solve_cgne(c, xp, bhat, *p, stop, res, cnt, s);
   else status = solve_gcr(c, xp, bhat, *p, stop, res, cnt, s);
-  if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) { cudaEventDestroy(e0); cudaEventDestroy(e1); return status; }
+  if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) return status;
   // true residual of the Schur system in the outer precision = ||b - M x|| (R6)
   double rn;
   if ((rc = residual(c, t1, bhat, xp, par, p->kappa, po, p->recon_outer, &rn, s))) return rc;
@@ -757,7 +761,6 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "invert", e);
   float ms = 0;
   cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
   res->seconds = ms * 1e-3;
   res->status = status;
   res->matpc_sloppy = (int)cnt.mat_sloppy; res->matpc_outer = (int)cnt.mat_outer; res->matpc_precond = (int)cnt.mat_precond;
@@ -785,9 +788,10 @@ int lqcd_invert_mrhs(lqcd_ctx* c, void* x_can, const void* b_can, int nrhs, cons
   char *bp, *bq, *xp, *bhat, *t1;
   for (char** q : {&bp, &bq, &xp, &bhat, &t1}) if ((rc = wk.get(q, fo * nrhs))) return rc;
   cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  if (cudaEventCreate(&e0) != cudaSuccess) return fail(c, LQCD_ECUDA, "event");
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return fail(c, LQCD_ECUDA, "event"); }
+  EventPair ev{e0, e1};
   cudaEventRecord(e0, s);
-  struct Ev { cudaEvent_t a, b; ~Ev() { cudaEventDestroy(a); cudaEventDestroy(b); } } ev{e0, e1};
   Counts cnt;
   const char *A, *Ai;
   if ((rc = get_clover(c, po, p->kappa, false, &A, &Ai, s))) return rc;

@@ -29,7 +29,7 @@ def test_extent_two_directions(dims, bc):
     psi = inputs.gaussian_spinor(dims, 5)
     for prec in (0, 1, 2):
         for recon in (18, 12, 8):
-            tol = TOL[prec] if not (prec == 0 and recon == 8) else 1e-11
+            tol = TOL[prec]        # fp64 recon-8 included (R10: measured <= 1.2e-14)
             for parity in (0, 1):
                 for dagger in (False, True):
                     want = oracle.dslash(psi * c.mask(1 - parity), c.U, c.bc, dagger=dagger) * c.mask(parity)
@@ -234,3 +234,92 @@ def test_context_lifecycle_releases_device_memory():
     assert torch.equal(o1a, o1b)
     c1.close()
     c2.close()
+
+
+def test_recon8_rejects_unit_gauge_and_compression_rejects_non_su3():
+    """recon-8 cannot hold a link with first row (a1, 0, 0) (N = |a2|^2 + |a3|^2 = 0, e.g. the cold start
+    U = 1; R10): the library must say so (LQCD_EINVAL) instead of returning NaN fields, in every
+    precision, and recon-12 / 18 must keep working on the same context.  Links that are not SU(3) are
+    refused by recon-12 and recon-8 (both reconstruct unitary links only) and accepted by recon-18."""
+    from paper_1109_2935_b200 import lqcd
+    dims = (4, 4, 4, 4)
+    psi = torch.from_numpy(inputs.gaussian_spinor(dims, 2)).cuda()
+    ctx = lqcd.Context(dims, (1, 1, 1, -1), 0)
+    ctx.load_gauge(torch.from_numpy(inputs.unit_gauge(dims)).cuda())
+    ctx.build_clover(1.0)
+    for prec in (0, 1, 2):
+        fin, fout = ctx.pack_spinor(psi, 1, prec), ctx.new_field(prec)
+        with pytest.raises(lqcd.LqcdError) as e:
+            ctx.dslash(fout, fin, 0, False, prec, 8)
+        assert e.value.code == lqcd.EINVAL and "recon 8" in str(e.value)
+        with pytest.raises(lqcd.LqcdError) as e:                   # still refused on the second call (nothing half-built is cached)
+            ctx.matpc(fout, fin, 0, False, 0.12, prec, 8)
+        assert e.value.code == lqcd.EINVAL
+        for recon in (12, 18):
+            ctx.dslash(fout, fin, 0, False, prec, recon)
+            got = torch.zeros_like(psi)
+            ctx.unpack_spinor(got, fout, 0, prec)
+            assert bool(torch.isfinite(torch.view_as_real(got)).all())
+    p = ctx.make_params(0.12, 1.0, 1e-8, prec=(0, 1, 1), recon=(18, 8, 8))
+    with pytest.raises(lqcd.LqcdError) as e:
+        ctx.invert(torch.zeros_like(psi), psi, p)
+    assert e.value.code == lqcd.EINVAL
+    # one link of an otherwise valid field scaled by 1.001: not unitary
+    U = inputs.random_gauge(dims, 0.4, 3)
+    U[2, 1, 2, 3, 0] *= 1.001
+    ctx.load_gauge(torch.from_numpy(U).cuda())
+    ctx.build_clover(1.0)
+    fin, fout = ctx.pack_spinor(psi, 1, 0), ctx.new_field(0)
+    for recon in (12, 8):
+        with pytest.raises(lqcd.LqcdError) as e:
+            ctx.dslash(fout, fin, 0, False, 0, recon)
+        assert e.value.code == lqcd.EINVAL and "SU(3)" in str(e.value)
+    ctx.dslash(fout, fin, 0, False, 0, 18)                         # recon-18 stores what it is given
+    got = torch.zeros_like(psi)
+    ctx.unpack_spinor(got, fout, 0, 0)
+    par = inputs.parity_mask(dims)
+    want = oracle.dslash(psi.cpu().numpy() * (par == 1)[..., None, None], U, (1, 1, 1, -1)) * (par == 0)[..., None, None]
+    assert _rel(got.cpu().numpy(), want) <= 1e-13
+    ctx.close()
+
+
+def test_recon8_fp64_near_unit_links():
+    """Smooth gauge fields (eps = 0.02: N ~ 1e-4 on a typical link) in fp64 / recon-8 at the north_star tolerance:
+    the reconstruction takes |c1|^2 = N - |b1|^2 (core.cuh), so its error does not grow as N -> 0."""
+    c = Case((4, 6, 4, 8), 0.02)
+    psi = inputs.gaussian_spinor(c.dims, 9)
+    for parity in (0, 1):
+        want = oracle.dslash(psi * c.mask(1 - parity), c.U, c.bc) * c.mask(parity)
+        got = c.gpu_parity_op(lambda o, i: c.ctx.dslash(o, i, parity, False, 0, 8), psi, 1 - parity, parity, 0)
+        assert _rel(got, want) <= 1e-13
+    want = oracle.matpc(psi, c.U, c.T, c.bc, 0.12, 0)
+    got = c.gpu_parity_op(lambda o, i: c.ctx.matpc(o, i, 0, False, 0.12, 0, 8), psi, 0, 0, 0)
+    assert _rel(got, want) <= 1e-13
+    c.ctx.close()
+
+
+def test_staggered_links_survive_growing_mrhs_workspace():
+    """One context serving both paths: loading staggered links, then multi-right-hand-side Mhat calls whose
+    temporary has to grow (more sources, then a wider precision), must leave the staggered links loaded."""
+    from paper_1109_2935_b200 import lqcd
+    dims, bc = (4, 4, 4, 8), (1, 1, 1, -1)
+    c = Case(dims, 0.3)
+    ctx = c.ctx
+    fat, lng = inputs.staggered_links(dims, 0.3, 4)
+    ctx.load_staggered_links(torch.from_numpy(fat).cuda(), torch.from_numpy(lng).cuda(), 0.0)
+    chi = inputs.gaussian_colour_vector(dims, 5)
+    d = torch.from_numpy(chi).cuda()
+
+    def stag():
+        out = ctx.new_staggered_field(1)
+        ctx.staggered_dslash(out, ctx.pack_staggered(d, 1, 1), 0, 1)
+        got = torch.zeros_like(d)
+        ctx.unpack_staggered(got, out, 0, 1)
+        return got
+
+    ref = stag()
+    for prec, nrhs in ((1, 2), (1, 5), (0, 5), (0, 9)):
+        fin = ctx.new_fields(prec, nrhs).zero_()
+        ctx.matpc_mrhs(ctx.new_fields(prec, nrhs), fin, nrhs, 0, False, 0.12, prec, 12)
+        assert torch.equal(stag(), ref)
+    ctx.close()

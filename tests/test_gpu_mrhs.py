@@ -26,7 +26,7 @@ def test_mrhs_matches_oracle_and_single(ragged, prec, nrhs):
     srcs = [inputs.gaussian_spinor(c.dims, 100 + r) * (1.0 + r) for r in range(nrhs)]    # different norms per source
     dev = [torch.from_numpy(s).cuda() for s in srcs]
     for recon in (18, 12, 8):
-        tol = TOL[prec] if not (prec == 0 and recon == 8) else 1e-11
+        tol = TOL[prec]        # fp64 recon-8 included (R10: measured <= 1.2e-14)
         for parity in (0, 1):
             for dagger in (False, True):
                 fin = ctx.new_fields(prec, nrhs)

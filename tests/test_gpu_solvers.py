@@ -195,6 +195,48 @@ def test_cfg4_full_size_solves_true_residual_by_oracle():
     ctx.close()
 
 
+def test_cfg5_full_size_gcr_dd_and_bicgstab_true_residual_by_oracle():
+    """BASELINE.json config 5 at full size (48^3x96 = 10.6 M sites, eps = 0.2, kappa = 0.124, c_sw = 1, Gaussian
+    source, seeds 21 / 22): GCR(16)-DD with 256 Schwarz blocks of 12^3x24 and 10 MR steps in half precision
+    (fp64 outer; sloppy fp32 and the paper's single-half-half flavour, sloppy half), against
+    mixed-precision BiCGstab on the same system (Figs. 7-8), all to 1e-10.  The true residual
+    ||b - M x|| / ||b|| is recomputed with the ORACLE's full-lattice operator (x = M^-1 b is unique, so the
+    residual pins it; the oracle's own solve at this size would take an hour), and the solvers' solutions
+    must agree with each other to 1e-8."""
+    from paper_1109_2935_b200 import lqcd
+    dims, kappa, blk = (48, 48, 48, 96), 0.124, (12, 12, 12, 24)
+    Ut = inputs.random_gauge_torch(dims, 0.2, 21, device="cuda")
+    bt = inputs.gaussian_spinor_torch(dims, 22, device="cuda")
+    ctx = lqcd.Context(dims, BC, 0)
+    ctx.load_gauge(Ut)
+    ctx.build_clover(1.0)
+    U, b = Ut.cpu().numpy(), bt.cpu().numpy()
+    del Ut
+    T = oracle.clover_term(U, 1.0)
+    bn = np.linalg.norm(b)
+    runs = [("gcr-dd fp64/fp32/half", lqcd.SOLVER_GCR_DD, (0, 1, 2), dict(gcr_kmax=16, schwarz_block=blk, mr_steps=10)),
+            ("gcr-dd fp64/half/half", lqcd.SOLVER_GCR_DD, (0, 2, 2), dict(gcr_kmax=16, schwarz_block=blk, mr_steps=10)),
+            ("bicgstab fp64/half", lqcd.SOLVER_BICGSTAB, (0, 2, 2), {}),
+            ("bicgstab fp64/fp32", lqcd.SOLVER_BICGSTAB, (0, 1, 1), {})]
+    xs = []
+    for name, solver, prec, kw in runs:
+        p = ctx.make_params(kappa, 1.0, 1e-10, solver=solver, prec=prec, recon=(18, 12, 12), **kw)
+        x = torch.zeros_like(bt)
+        info = ctx.invert(x, bt, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-10, (name, info)
+        xh = x.cpu().numpy()
+        res = np.linalg.norm((b - oracle.M(xh, U, T, BC, kappa)).ravel()) / bn
+        assert res <= 1.05e-10, (name, res)
+        assert abs(res - info["true_residual"]) <= 0.05 * res, (name, res, info["true_residual"])
+        if solver == lqcd.SOLVER_GCR_DD:
+            assert info["matpc_precond"] == 10 * info["iterations"]          # 10 MR steps per outer iteration
+        xs.append(x)
+        del xh
+    for x in xs[1:]:
+        assert float(torch.linalg.vector_norm(x - xs[0]) / torch.linalg.vector_norm(xs[0])) <= 1e-8
+    ctx.close()
+
+
 @pytest.mark.parametrize("prec", [(0, 0, 0), (0, 1, 1), (0, 2, 2)])
 def test_cgnr(mid, prec):
     """CGNR in fp64 and mixed precision: same unique solution as the oracle's solve, true
