@@ -178,9 +178,8 @@ LQ_DEV void hop_tail_packed(float* __restrict__ acc, const cx<float> (&h)[2][3],
 }
 
 template <int MU, bool FWD, typename R>
-LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef) {
+LQ_DEV void hop_tail_scalar(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef) {
   typedef GammaRow<MU> G;
-  if constexpr (sizeof(R) == 4) { hop_tail_packed<MU, FWD>(acc, h, u, sigma, coef); return; }
   // colour multiply: 6 FMA per real output
   cx<R> w[2][3];
 #pragma unroll
@@ -221,6 +220,12 @@ LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __res
   }
 }
 
+template <int MU, bool FWD, typename R>
+LQ_DEV void hop_tail(R* __restrict__ acc, const cx<R> (&h)[2][3], const R* __restrict__ u, R sigma, R coef) {
+  if constexpr (sizeof(R) == 4) hop_tail_packed<MU, FWD>(acc, h, u, sigma, coef);
+  else hop_tail_scalar<MU, FWD, R>(acc, h, u, sigma, coef);
+}
+
 // out = C in for one site: two Hermitian 6x6 blocks, 36 reals each: 6 diagonal then the 15
 // lower-triangle entries (i>j) at 6 + 2*(i(i-1)/2 + j).  504 flop (PAPER.md:138 fn.1: 72 reals).
 template <typename R>
@@ -243,8 +248,7 @@ LQ_DEV void clover_block(R* __restrict__ o, const R* __restrict__ x, const R* __
       }
       f2_split(t, o[2 * i], o[2 * i + 1]);
     }
-    return;
-  }
+  } else {
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
     R re = c[i] * x[2 * i], im = c[i] * x[2 * i + 1];
@@ -261,6 +265,7 @@ LQ_DEV void clover_block(R* __restrict__ o, const R* __restrict__ x, const R* __
       }
     }
     o[2 * i] = re; o[2 * i + 1] = im;
+  }
   }
 }
 template <typename R>
@@ -370,9 +375,6 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
   }
 }
 
-#ifndef LQ_PROBE
-#define LQ_PROBE 0
-#endif
 #ifndef LQ_DSLASH_BLOCK
 #define LQ_DSLASH_BLOCK 128
 #endif
@@ -505,14 +507,14 @@ dslash_kernel(const DslashArgs a) {
         load_link<P, RECON, 2>(u, us, sb_, LQ_DSLASH_BLOCK, tid);                                          \
         if constexpr (P::HALF) load_site_magic<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid); \
         else load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);   \
-        if (!(LQ_PROBE & 1)) if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                  \
+        if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                       \
         cp_async_commit();                                                                                 \
         const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
         if constexpr (P::HALF) hop_fixed<MU_, FW_, (FW_ == (DAG == 1)) ? 1 : -1>(acc, psi, u, sg_ * us * ps); \
         else hop<MU_, FW_, R>(acc, psi, u, FW_ ? sig_f : -sig_f, sg_);                                     \
       }
 #pragma unroll
-      for (int h = 0; h < ((LQ_PROBE & 1) ? 0 : NST); ++h) {
+      for (int h = 0; h < NST; ++h) {
         switch (h) {                       // NST <= 4
           case 0: LQ_ISSUE(0) break;
           case 1: LQ_ISSUE(1) break;
