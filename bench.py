@@ -174,6 +174,69 @@ def oracle_dslash_rate(n_apps, U, psi):
     return FLOP_DSLASH * V * n_apps / dt / 1e9, dt, oracle.num_threads(), out
 
 
+def oracle_legs(U3, psi3, dev):
+    """SURVEY 8(d) "oracle timed beside it": the oracle as it stands on the host cores for the other operators
+    and solves of BASELINE.json's configs, each a bounded sample (about a minute in total)."""
+    import numpy as np
+    import torch
+    import oracle
+    from paper_1109_2935_b200 import inputs
+    legs = []
+
+    def timed(fn, n):
+        t0 = time.time()
+        for _ in range(n):
+            r = fn()
+        return (time.time() - t0) / n, r
+    V3 = int(np.prod(psi3.shape[:4]))
+    # config 3: Mhat (3696 flop per parity site)
+    T3 = oracle.clover_term(U3, CSW)
+    dt, _ = timed(lambda: oracle.matpc(psi3, U3, T3, BC, KAPPA, 0), 2)
+    legs.append({"config": 3, "what": "Mhat (one parity) at 32^3x64", "seconds_per_application": dt,
+                 "value": FLOP_MATPC * (V3 // 2) / dt / 1e9, "unit": "GFLOP/s"})
+    del T3
+    # config 2: Dslash (both parities) and clover apply at 16^3x32
+    d2 = (16, 16, 16, 32)
+    U2 = inputs.random_gauge_torch(d2, 0.3, 1).numpy()
+    p2 = inputs.gaussian_spinor_torch(d2, 2).numpy()
+    T2 = oracle.clover_term(U2, CSW)
+    V2 = int(np.prod(d2))
+    dt, _ = timed(lambda: oracle.dslash(p2, U2, BC), 10)
+    legs.append({"config": 2, "what": "Dslash (both parities) at 16^3x32", "seconds_per_application": dt,
+                 "value": FLOP_DSLASH * V2 / dt / 1e9, "unit": "GFLOP/s"})
+    dt, _ = timed(lambda: oracle.clover_apply(p2, T2, KAPPA), 10)
+    legs.append({"config": 2, "what": "clover apply (both parities) at 16^3x32", "seconds_per_application": dt,
+                 "value": 504 * V2 / dt / 1e9, "unit": "GFLOP/s"})
+    # config 1: fp64 BiCGstab to 1e-12 at 4^4
+    d1 = (4, 4, 4, 4)
+    U1, b1 = inputs.random_gauge(d1, 0.5, 1), inputs.gaussian_spinor(d1, 2)
+    T1 = oracle.clover_term(U1, CSW)
+    dt, (x1, i1) = timed(lambda: oracle.invert(b1, U1, T1, BC, 0.12, tol=1e-12), 1)
+    legs.append({"config": 1, "what": "fp64 BiCGstab to 1e-12 at 4^4", "seconds": dt, "iterations": i1["iterations"],
+                 "true_residual": i1["true_residual"]})
+    # config 4: fp64 BiCGstab at 32^3x64 with an iteration budget (a full solve is ~90 iterations = minutes)
+    U4 = inputs.random_gauge_torch(DIMS, 0.2, 11, device=dev).cpu().numpy()
+    b4 = inputs.gaussian_spinor_torch(DIMS, 12, device=dev).cpu().numpy()
+    T4 = oracle.clover_term(U4, CSW)
+    budget = 5
+    dt, (x4, i4) = timed(lambda: oracle.invert(b4, U4, T4, BC, KAPPA, tol=1e-10, maxit=budget), 1)
+    legs.append({"config": 4, "what": "fp64 BiCGstab at 32^3x64, budget of %d iterations (the solve needs ~90)" % budget,
+                 "seconds": dt, "iterations": i4["iterations"], "residual_reached": i4["true_residual"],
+                 "seconds_per_iteration": dt / max(1, i4["iterations"]),
+                 "value": (2 * FLOP_MATPC + 1056) * (V3 // 2) * max(1, i4["iterations"]) / dt / 1e9, "unit": "GFLOP/s (effective)"})
+    del U4, b4, T4, x4
+    # config 5: operator application only (Dslash, both parities) at 48^3x96
+    d5 = (48, 48, 48, 96)
+    U5 = inputs.random_gauge_torch(d5, 0.2, 21, device=dev).cpu().numpy()
+    p5 = inputs.gaussian_spinor_torch(d5, 22, device=dev).cpu().numpy()
+    V5 = int(np.prod(d5))
+    oracle.dslash(p5, U5, BC)
+    dt, _ = timed(lambda: oracle.dslash(p5, U5, BC), 2)
+    legs.append({"config": 5, "what": "Dslash (both parities) at 48^3x96", "seconds_per_application": dt,
+                 "value": FLOP_DSLASH * V5 / dt / 1e9, "unit": "GFLOP/s"})
+    return legs
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -210,7 +273,9 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="b200")
-    ap.add_argument("--full", action="store_true", help="also run config 5 (48^3x96 GCR-DD vs BiCGstab)")
+    ap.add_argument("--full", action="store_true", help="kept for compatibility: config 5 now runs by default")
+    ap.add_argument("--no-cpu-legs", action="store_true", help="cpu_baseline: the headline Dslash only (skip Mhat / configs 1, 2, 4, 5 on the host)")
+    ap.add_argument("--no-config5", action="store_true", help="skip config 5 (48^3x96 GCR-DD vs BiCGstab, ~20 s)")
     ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
     ap.add_argument("--op", default="dslash", choices=["dslash", "staggered"],
@@ -233,7 +298,7 @@ def main():
     if world > 1:
         # replicas: every rank times the headline and the e2e leg; the sweep, the solvers and the CPU baseline
         # are rank-0-at-N=1 material and would leave the other ranks waiting in the process-group teardown
-        args.quick, args.solvers_only, args.full = True, False, False
+        args.quick, args.solvers_only, args.full, args.no_config5 = True, False, False, True
     if args.op == "staggered":
         run_staggered(args, rank, world, local)
         return
@@ -349,6 +414,10 @@ def main():
         gf, dt, cores, o_out = oracle_dslash_rate(n_apps, U.cpu().numpy(), psi.cpu().numpy())
         out["cpu_baseline"] = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
                                "sample": "%d full-lattice D applications at 32^3x64 in %.1f s (fp64, OpenMP)" % (n_apps, dt)}
+        if not args.no_cpu_legs:
+            t0 = time.time()
+            out["cpu_baseline"]["legs"] = oracle_legs(U.cpu().numpy(), psi.cpu().numpy(), dev)
+            out["cpu_baseline"]["legs_seconds"] = time.time() - t0
         # parity of the timed configuration against the oracle on the full lattice (same inputs)
         import numpy as np
         got = torch.zeros_like(psi)
@@ -360,11 +429,33 @@ def main():
     elif rank == 0:
         out["cpu_baseline"] = None
     if rank == 0:
+        if out.get("extra"):
+            out["summary"] = summarize(out["extra"])        # compact, last in the line: survives a truncated record
         print(json.dumps(out))
     ctx.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def summarize(ex):
+    """Compact restatement of `extra`: us per parity application [r18, r12, r8] and fraction of the measured HBM
+    copy bandwidth, sustained r12 figures, solver seconds."""
+    sm = {}
+    for op in ("dslash", "matpc"):
+        rows = [r for r in ex.get("sweep", []) if r["op"] == op]
+        if not rows:
+            continue
+        sm[op + "_us_r18_r12_r8"] = {p: [round(r["us"], 1) for r in rows if r["prec"] == p] for p in ("fp64", "fp32", "half")}
+        sm[op + "_frac_measured_hbm"] = {p: [round(r["frac_measured_peak"], 3) for r in rows if r["prec"] == p] for p in ("fp64", "fp32", "half")}
+        sm[op + "_sustained_r12_us_mhz"] = {r["prec"]: [round(r["sustained"]["us"], 1), r["sustained"]["sm_mhz_at_end"]]
+                                            for r in rows if r.get("sustained")}
+    sm["mrhs_us_per_rhs"] = {"%s_%s" % (r["op"], r["prec"]): round(r["us_per_rhs"], 1) for r in ex.get("mrhs", [])}
+    def srow(r):
+        return {"s": round(r["seconds"], 4), "it": r.get("iterations"), "res": r.get("true_residual", r.get("true_residual_max"))}
+    sm["cfg4"] = {"%s_%s%s" % (r["solver"], r.get("sloppy"), ("_" + str(r["precond"])) if r.get("precond") else ""): srow(r) for r in ex.get("solvers", [])}
+    sm["cfg5"] = {"%s_%s%s" % (r["solver"], r.get("sloppy"), ("_" + str(r["precond"])) if r.get("precond") else ""): srow(r) for r in ex.get("config5", [])}
+    return sm
 
 
 def run_staggered(args, rank, world, local):
@@ -521,11 +612,20 @@ def extras(ctx, psi, args, torch, lqcd, inputs, pk):
                 ms, clk = bursts[2][0] / 40.0, bursts[2][1]   # per parity application
                 best_us = bursts[0][0] / 40.0 * 1e3
                 gbs = by * Vh / (ms * 1e-3) / 1e9
+                sustained = None
+                if recon == 12:
+                    # one ~1.5 s back-to-back run: the board reaches its power cap, the SM clock drops and the
+                    # issue-bound (half) rows follow it; the HBM-bound rows do not
+                    nrep = max(50, int(1.5 / (2 * ms * 1e-3)))
+                    sms, sclk = time_region_clk(fn, nrep, psi.device.index or 0)
+                    sustained = {"us": sms / (2 * nrep) * 1e3, "seconds": sms * 1e-3, "sm_mhz_at_end": sclk}
+                    time.sleep(0.3)
                 ex["sweep"].append({"op": name, "prec": names[prec], "recon": recon, "us": ms * 1e3, "best_us": best_us,
+                                    "sustained": sustained,
                                     "gflops": flop * Vh / (ms * 1e-3) / 1e9, "gbs": gbs,
                                     "frac_measured_peak": gbs / pk["hbm_gbs"], "frac_8TBs": gbs / 8000.0,
                                     "bytes_per_site": by, "sm_mhz_during": clk,
-                                    "bound": "alu (issue slots, DESIGN.md 6.1)" if prec == 2 else "hbm"})
+                                    "bound": "hbm + fma/alu pipes (DESIGN.md 6.1)" if prec == 2 else "hbm"})
         # fused BLAS-1: axpy+norm (3 passes) and cdot (2 passes)
         for _ in range(3):
             ctx.axpy_norm(0.5, fin[0], fo[0], prec)
@@ -601,7 +701,8 @@ def extras(ctx, psi, args, torch, lqcd, inputs, pk):
     info.update({"config": "4 (lattice) with GCR-DD, 8^3x16 blocks", "best_of": 3, "solver": "gcr_dd", "sloppy": "fp32", "precond": "half",
                  "effective_gflops": info["gflop"] / info["seconds"]})
     ex["solvers"].append(info)
-    if args.full:
+    if not args.no_config5 and not args.solvers_only:
+        ctx.release_workspace()
         ex["config5"] = config5(torch, lqcd, inputs, dev)
     return ex
 
