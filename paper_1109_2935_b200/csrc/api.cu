@@ -160,8 +160,27 @@ int set_blocks(lqcd_ctx* c, const int* blk) {
 }
 
 // out = [C] ([A] y + a * D in) : one fused launch (dslash.cuh)
+// workspace of the reductions fused into the operator (dslash.cuh, DOTS >= 2): header + 3 doubles per CTA
+static int get_dotws(lqcd_ctx* c, int nsite, double** out, cudaStream_t s) {
+  const size_t need = 8 + 3 * (size_t)((nsite + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK);
+  if (c->dotws_doubles < need) {
+    if (c->dotws) cudaFree(c->dotws);             // synchronises
+    c->dotws = nullptr; c->dotws_doubles = 0;
+    int rc = dev_alloc(c, (void**)&c->dotws, need * sizeof(double));
+    if (rc) return rc;
+    c->dotws_doubles = need;
+    double hdr[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    memcpy(&hdr[0], &c->S, sizeof(double*));      // W[0] = address of the scalar array, W[1] = arrival counter = 0
+    cudaError_t e = cudaMemcpyAsync(c->dotws, hdr, sizeof(hdr), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dot workspace", e);
+  }
+  *out = c->dotws;
+  return LQCD_OK;
+}
+
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
-              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0, int cb1) {
+              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0, int cb1, int fin, const char* q) {
   DslashArgs d;
   memset(&d, 0, sizeof(d));
   d.g = blocked ? c->bm.blk : c->nat;
@@ -175,6 +194,12 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
     d.clov_y = A; d.clov_out = Ai;
   }
   if (epi == EPI_CLOVX_XPAY_DOTS) d.dots = c->boxdots;          // whole boxes (the two share storage, dslash.cuh)
+  else if (epi == EPI_CLOVX_XPAY_YDOT || epi == EPI_CLOVX_XPAY_QDOT) {
+    if (blocked || fin <= 0 || (epi == EPI_CLOVX_XPAY_QDOT && !q)) return fail(c, LQCD_EINVAL, "fused reduction arguments");
+    if ((rc = get_dotws(c, d.g.vh, &d.dots, s))) return rc;
+    d.dagger = dagger | (fin << 16);
+    if (epi == EPI_CLOVX_XPAY_QDOT) d.clov_out = q;            // the third vector travels in the unused A^-1 slot
+  }
   else { d.range.cb0 = cb0; d.range.cb1 = cb1 < 0 ? d.g.vh : cb1; }
   cudaError_t e;
   switch (prec) {
@@ -191,13 +216,15 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
 // out = Mhat in  (R6):  tmp = A^-1 D in ;  out = A in - kappa^2 D tmp.
 // sym != 0: the symmetric form Mhat_s = 1 - kappa^2 A^-1 D A^-1 D:  tmp = A^-1 D in ; out = in - kappa^2 A^-1 D tmp,
 // and Mhat_s^dag = 1 - kappa^2 D^dag A^-1 D^dag A^-1:  t0 = A^-1 in ; tmp = A^-1 D^dag t0 ; out = in - kappa^2 D^dag tmp.
+// fin != 0 (asymmetric form, natural layout only): the second launch also reduces <out,in>, ||out||^2 (q == nullptr) or
+// <q,out>, ||out||^2 over the field and its last CTA performs the scalar update `fin` (DotsFin, dslash.cuh)
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
-             bool blocked, bool dots, cudaStream_t s, int sym) {
+             bool blocked, bool dots, cudaStream_t s, int sym, int fin, const char* q) {
   char* tmp;
   int rc = get_tmp(c, prec, blocked, &tmp);
   if (rc) return rc;
   if (sym) {
-    if (blocked || dots) return fail(c, LQCD_EINVAL, "symmetric form is not available for the Schwarz operator");
+    if (blocked || dots || fin) return fail(c, LQCD_EINVAL, "symmetric form is not available for the Schwarz operator / fused reductions");
     if (!dagger) {
       rc = op_dslash(c, tmp, in, nullptr, 1 - parity, 0, prec, recon, EPI_CLOVOUT, 0.0, kappa, false, s);
       if (rc) return rc;
@@ -216,6 +243,8 @@ int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, dou
   }
   rc = op_dslash(c, tmp, in, nullptr, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, blocked, s);
   if (rc) return rc;
+  if (fin) return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, q ? EPI_CLOVX_XPAY_QDOT : EPI_CLOVX_XPAY_YDOT,
+                            -kappa * kappa, kappa, blocked, s, 0, -1, fin, q);
   return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, dots ? EPI_CLOVX_XPAY_DOTS : EPI_CLOVX_XPAY,
                    -kappa * kappa, kappa, blocked, s);
 }
@@ -299,6 +328,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   c->S = nullptr; c->partials = nullptr; c->counters = nullptr; c->boxdots = nullptr; c->hS = nullptr;
   c->boxdots_doubles = 0;
   c->gflag = nullptr;
+  c->dotws = nullptr; c->dotws_doubles = 0;
   memset(c->hws, 0, sizeof(c->hws)); memset(c->hws_bytes, 0, sizeof(c->hws_bytes));
   c->have_hpipe = false;
   c->mtmp = nullptr; c->mtmp_bytes = 0;
@@ -332,6 +362,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->partials) cudaFree(c->partials);
   if (c->counters) cudaFree(c->counters);
   if (c->gflag) cudaFree(c->gflag);
+  if (c->dotws) cudaFree(c->dotws);
   if (c->boxdots) cudaFree(c->boxdots);
   if (c->hS) cudaFreeHost(c->hS);
   for (auto& b : c->pool) cudaFree(b.p);

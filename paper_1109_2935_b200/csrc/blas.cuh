@@ -31,6 +31,9 @@ enum {
   S_TOTAL = S_GCR_ALPHAS + 2 * LQ_GCR_KMAX
 };
 
+static_assert(S_RHO == LQ_S_RHO && S_ALPHA == LQ_S_ALPHA && S_OMEGA == LQ_S_OMEGA && S_FLAG == LQ_S_FLAG && S_RTV == LQ_S_RTV &&
+              S_TS == LQ_S_TS && S_TT == LQ_S_TT, "dslash.cuh dots_finalize uses these slot numbers");
+
 struct BlasArgs {
   char* v[LQ_MAX_VEC];
   long long ns;
@@ -46,6 +49,8 @@ struct BlasArgs {
   // v[j] + r * rhs_bytes, S + r * S_TOTAL, partials + r * rhs_partials, counters + r
   long long rhs_bytes;
   long long rhs_partials;
+  // pinned host words the last CTA may publish scalars to (zero-copy; no memcpy or event between two kernels)
+  double* hmirror;
 };
 
 struct cd { double re, im; };

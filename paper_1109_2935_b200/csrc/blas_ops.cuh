@@ -167,7 +167,8 @@ struct OpBicgXR {          // v0 = x, v1 = p, v2 = s->r, v3 = t, v4 = rtilde
     site_cdot(rt, s, red[0], red[1]);
     site_norm2(s, red[2]);
   }
-  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) {
+  LQ_DEV static void finalize(const double* s, const BlasArgs& a, int) { update(s, a); publish(a); }
+  LQ_DEV static void update(const double* s, const BlasArgs& a) {
     double* S = a.S;
     const cd rho_old = {S[S_RHO], S[S_RHO + 1]};
     S[S_RHO_OLD] = rho_old.re; S[S_RHO_OLD + 1] = rho_old.im;
@@ -178,6 +179,14 @@ struct OpBicgXR {          // v0 = x, v1 = p, v2 = s->r, v3 = t, v4 = rtilde
     if (!(d1 > 0.0) || !(d2 > 0.0)) { if (s[2] > 0.0) S[S_FLAG] = 3; S[S_BETA] = 0; S[S_BETA + 1] = 0; return; }
     const cd beta = cd_mul(cd_div(cd{s[0], s[1]}, rho_old), cd_div(al, om));
     S[S_BETA] = beta.re; S[S_BETA + 1] = beta.im;
+  }
+  // publish (||r||^2, breakdown flag) of iteration i0 to the host: values first, then the iteration number the host polls
+  LQ_DEV static void publish(const BlasArgs& a) {
+    if (!a.hmirror) return;
+    volatile double* h = a.hmirror + 4 * (a.i0 & 1);
+    h[0] = a.S[S_RR]; h[1] = a.S[S_FLAG];
+    __threadfence_system();
+    h[2] = (double)a.i0;
   }
 };
 

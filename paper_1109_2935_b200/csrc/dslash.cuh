@@ -314,11 +314,37 @@ LQ_DEV void cta_reduce(double* v, double* smem /* [NV][BLOCK/32] */) {
   }
 }
 
+// The scalar updates of OpBicgOmega / OpBicgAlpha / OpCgAlpha (blas_ops.cuh) for the reductions fused into the
+// operator's epilogue; s = (re, im of the dot product, ||out||^2).  Slot numbers: blas.cuh (checked there).
+#define LQ_S_RHO 0
+#define LQ_S_ALPHA 4
+#define LQ_S_OMEGA 6
+#define LQ_S_FLAG 11
+#define LQ_S_RTV 12
+#define LQ_S_TS 14
+#define LQ_S_TT 16
+LQ_DEV void dots_finalize(double* S, const double* s, int fin) {
+  if (fin == 1) {            // omega = <t,s> / <t,t>
+    S[LQ_S_TS] = s[0]; S[LQ_S_TS + 1] = s[1]; S[LQ_S_TT] = s[2];
+    if (!(s[2] > 0.0)) { S[LQ_S_OMEGA] = 0; S[LQ_S_OMEGA + 1] = 0; S[LQ_S_FLAG] = 2; return; }
+    S[LQ_S_OMEGA] = s[0] / s[2]; S[LQ_S_OMEGA + 1] = s[1] / s[2];
+  } else if (fin == 2) {     // alpha = rho / <rtilde, v>
+    S[LQ_S_RTV] = s[0]; S[LQ_S_RTV + 1] = s[1];
+    const double d = s[0] * s[0] + s[1] * s[1];
+    if (!(d > 0.0)) { S[LQ_S_FLAG] = 1; S[LQ_S_ALPHA] = 0; S[LQ_S_ALPHA + 1] = 0; return; }
+    const double rr = S[LQ_S_RHO], ri = S[LQ_S_RHO + 1];
+    S[LQ_S_ALPHA] = (rr * s[0] + ri * s[1]) / d; S[LQ_S_ALPHA + 1] = (ri * s[0] - rr * s[1]) / d;
+  } else if (fin == 3) {     // CG on the normal equations: alpha = zz / ||w||^2
+    if (!(s[2] > 0.0)) { S[LQ_S_ALPHA] = 0; S[LQ_S_FLAG] = 1; return; }
+    S[LQ_S_ALPHA] = S[LQ_S_RHO] / s[2];
+  }
+}
+
 // Fused epilogue of one site (shared by the single- and multi-right-hand-side kernels):
 //   XPAY: acc = [A] y + coef * acc (CLOVX: A = clover block of the site);  CLOVOUT: acc = C acc;
 //   XPAY && CLOVX && CLOVOUT: acc = y + coef * C acc (symmetric even-odd form);
-//   DOTS: d0 + i d1 += <acc, y>, d2 += <acc, acc> for this site (before CLOVOUT; only used with CLOVX).
-template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+//   DOTS 1, 2: d0 + i d1 += <acc, y>, d2 += <acc, acc> for this site; DOTS 3: d0 + i d1 += <q, acc> (only with CLOVX).
+template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS>
 LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __restrict__ y, const char* __restrict__ clov_y,
                             const char* __restrict__ clov_out, double coef_d, int p, long long ns, long long idx,
                             typename P::real& d0, typename P::real& d1, typename P::real& d2) {
@@ -351,7 +377,7 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
           if constexpr (P::HALF) ay[k] *= sc;
           acc[12 * ch + k] = fma_(coef, acc[12 * ch + k], ay[k]);
         }
-        if constexpr (DOTS) {
+        if constexpr (DOTS == 1 || DOTS == 2) {
 #pragma unroll
           for (int k = 0; k < 6; ++k) {
             const R rr = acc[12 * ch + 2 * k], ri = acc[12 * ch + 2 * k + 1];
@@ -360,6 +386,19 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
             d1 = fma_(rr, yi, d1); d1 = fma_(-ri, yr, d1);
             d2 = fma_(rr, rr, d2); d2 = fma_(ri, ri, d2);
           }
+        }
+      }
+      if constexpr (DOTS == 3) {
+        // d0 + i d1 += <q, acc> with a third vector q (BiCGstab: <rtilde, v>); its pointer travels in clov_out,
+        // which this epilogue does not use
+        R q[24];
+        load_site<P, 24>(q, clov_out, ns, idx);
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+          const R rr = acc[2 * k], ri = acc[2 * k + 1];
+          d0 = fma_(q[2 * k], rr, d0); d0 = fma_(q[2 * k + 1], ri, d0);
+          d1 = fma_(q[2 * k], ri, d1); d1 = fma_(-q[2 * k + 1], rr, d1);
+          d2 = fma_(rr, rr, d2); d2 = fma_(ri, ri, d2);
         }
       }
     } else {
@@ -416,7 +455,7 @@ template <class P, int RECON> struct HopStage {
 // needed: cp.async.wait_group orders a thread's own copies.
 // DAG: -1 = dagger read from the arguments at run time (fp64, fp32); 0 / 1 = compile-time dagger (half precision:
 // the fixed-point projection fused with the decode needs the sign of every combination at compile time).
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int NST, int DAG = -1>
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS, int NST, int DAG = -1>
 __global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (dslash_minb<P, RECON, CLOVX, CLOVOUT>()))
 dslash_kernel(const DslashArgs a) {
   static_assert(P::HALF ? (DAG == 0 || DAG == 1) : DAG == -1, "compile-time dagger for half precision only");
@@ -437,7 +476,7 @@ dslash_kernel(const DslashArgs a) {
     const long long link_bytes = (long long)RECON * sizeof(typename P::store_t) * g.ns;
     const char* g_out = a.gauge + (long long)(p * 4) * link_bytes;        // links living on output-parity sites
     const char* g_in = a.gauge + (long long)((1 - p) * 4) * link_bytes;   // links living on input-parity sites
-    const R sig_f = a.dagger ? R(1) : R(-1);  // forward hop: (1 - g) for D, (1 + g) for D^dagger
+    const R sig_f = (a.dagger & 1) ? R(1) : R(-1);  // forward hop: (1 - g) for D, (1 + g) for D^dagger
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
@@ -531,7 +570,51 @@ dslash_kernel(const DslashArgs a) {
     dslash_epilogue<P, XPAY, CLOVX, CLOVOUT, DOTS>(acc, a.y, a.clov_y, a.clov_out, a.a, p, g.ns, idx, d0, d1, d2);
     store_site<P, 24>(acc, a.out, g.ns, idx);
   }
-  if constexpr (DOTS) {
+  if constexpr (DOTS >= 2) {
+    // Solver reductions fused into the operator ("BLAS1 ... extremely bandwidth
+    // intensive"): CTA sums -> per-CTA partials -> the last CTA adds them in a fixed order (bit-reproducible) and
+    // updates the Krylov scalars on the device.  a.dots = workspace W: W[0] = address of the scalar array S,
+    // W[1] = arrival counter (self-resetting), W[8 + 3 i ..] = partials of CTA i.  a.dagger >> 16 selects the update.
+    __shared__ double sm[3 * (LQ_DSLASH_BLOCK / 32)];
+    __shared__ bool last;
+    double red[3] = {(double)d0, (double)d1, (double)d2};
+    cta_reduce<3, LQ_DSLASH_BLOCK>(red, sm);
+    double* W = a.dots;
+    double* part = W + 8;
+    unsigned* counter = reinterpret_cast<unsigned*>(W + 1);
+    if (threadIdx.x == 0) {
+      part[3ll * blockIdx.x] = red[0]; part[3ll * blockIdx.x + 1] = red[1]; part[3ll * blockIdx.x + 2] = red[2];
+      __threadfence();
+      last = atomicAdd(counter, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last) {
+      __threadfence();
+      // thousands of partials for one CTA: 8 independent loads in flight per thread (one L2 round trip per 1024
+      // partials instead of per 128), added in a fixed order
+      double s[3] = {0, 0, 0};
+      for (int i0 = threadIdx.x; i0 < (int)gridDim.x; i0 += 8 * LQ_DSLASH_BLOCK) {
+        double t[8][3];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int i = i0 + u * LQ_DSLASH_BLOCK;
+          const bool ok = i < (int)gridDim.x;
+#pragma unroll
+          for (int k = 0; k < 3; ++k) t[u][k] = ok ? __ldcg(part + 3ll * i + k) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { s[0] += t[u][0]; s[1] += t[u][1]; s[2] += t[u][2]; }
+      }
+      __syncthreads();
+      cta_reduce<3, LQ_DSLASH_BLOCK>(s, sm);
+      if (threadIdx.x == 0) {
+        double* S = *reinterpret_cast<double**>(W);
+        dots_finalize(S, s, a.dagger >> 16);
+        *counter = 0;
+      }
+    }
+  }
+  if constexpr (DOTS == 1) {
     // per-warp partial sums (sites in fp64, fixed shuffle order: deterministic); no CTA barrier.
     // The MR update kernel adds the gridDim.x * (LQ_DSLASH_BLOCK/32) partials of its box.
     double red[3] = {(double)d0, (double)d1, (double)d2};
@@ -555,8 +638,13 @@ enum DslashEpi {
   EPI_XPAY = 3,       // out = y + a D in
   EPI_XPAY_CLOVOUT = 4, // out = C (y + a D in)
   EPI_CLOVX_XPAY_DOTS = 5, // EPI_CLOVX_XPAY + per-box <out,y>, <out,out>
-  EPI_XPAY_CLOVD = 6       // out = y + a C (D in)   (symmetric even-odd form)
+  EPI_XPAY_CLOVD = 6,      // out = y + a C (D in)   (symmetric even-odd form)
+  EPI_CLOVX_XPAY_YDOT = 7, // EPI_CLOVX_XPAY + global <out,y>, <out,out> and a scalar update by the last CTA
+  EPI_CLOVX_XPAY_QDOT = 8  // EPI_CLOVX_XPAY + global <q,out>, <out,out> (q in DslashArgs::clov_out) and a scalar update
 };
+
+// scalar updates the fused reductions can perform (DslashArgs::dagger >> 16)
+enum DotsFin { FIN_NONE = 0, FIN_BICG_OMEGA = 1, FIN_BICG_ALPHA = 2, FIN_CG_ALPHA = 3 };
 
 template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);
 

@@ -20,7 +20,7 @@ namespace lq {
 #define LQ_PIPE_HALF 4
 #endif
 
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS, int DAG>
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS, int DAG>
 static void launch_dag(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
   constexpr int NST = sizeof(typename P::real) == 8 ? ((CLOVX || CLOVOUT) ? 0 : LQ_PIPE_FP64) : (P::HALF ? LQ_PIPE_HALF : LQ_PIPE_FP32);
   constexpr int SMEM = NST * HopStage<P, RECON>::BYTES;
@@ -73,7 +73,7 @@ static bool tile_enabled() {
 }
 
 // half precision: the dagger flag selects one of two instantiations (dslash.cuh, hop_fixed)
-template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, bool DOTS>
+template <class P, int RECON, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS>
 static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t s) {
   // Tile form for the plain hopping term only.  Measured at 32^3x64, half r12 / r18: 71.0 -> 67.7 / 76.0 -> 71.6 us;
   // with a clover epilogue the tile form (2,770 SASS instructions, 44 KB: over the 32 KB instruction cache) is no
@@ -82,19 +82,19 @@ static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
     TileInfo ti;
     if (tile_enabled()) {
       if (tile_ok<128>(a, ti)) {
-        if (a.dagger) launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 128, 1>(a, ti, s);
+        if (a.dagger & 1) launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 128, 1>(a, ti, s);
         else launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 128, 0>(a, ti, s);
         return;
       }
       if (tile_ok<96>(a, ti)) {
-        if (a.dagger) launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 96, 1>(a, ti, s);
+        if (a.dagger & 1) launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 96, 1>(a, ti, s);
         else launch_tile<RECON, XPAY, CLOVX, CLOVOUT, 96, 0>(a, ti, s);
         return;
       }
     }
   }
   if constexpr (P::HALF) {
-    if (a.dagger) launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, 1>(a, grid, block, s);
+    if (a.dagger & 1) launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, 1>(a, grid, block, s);
     else launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, 0>(a, grid, block, s);
   } else {
     launch_dag<P, RECON, XPAY, CLOVX, CLOVOUT, DOTS, -1>(a, grid, block, s);
@@ -103,17 +103,20 @@ static void launch_one(const DslashArgs& a, dim3 grid, dim3 block, cudaStream_t 
 
 template <class P, int RECON>
 static cudaError_t launch_dslash_r(const DslashArgs& a, int epi, cudaStream_t s) {
-  const int nsite = epi == EPI_CLOVX_XPAY_DOTS ? a.g.vh : a.range.cb1 - a.range.cb0;
+  const bool whole = epi == EPI_CLOVX_XPAY_DOTS || epi == EPI_CLOVX_XPAY_YDOT || epi == EPI_CLOVX_XPAY_QDOT;   // no site range (dslash.cuh)
+  const int nsite = whole ? a.g.vh : a.range.cb1 - a.range.cb0;
   dim3 grid((nsite + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);
   dim3 block(LQ_DSLASH_BLOCK);
   switch (epi) {
-    case EPI_NONE:            launch_one<P, RECON, false, false, false, false>(a, grid, block, s); break;
-    case EPI_CLOVOUT:         launch_one<P, RECON, false, false, true, false>(a, grid, block, s); break;
-    case EPI_CLOVX_XPAY:      launch_one<P, RECON, true, true, false, false>(a, grid, block, s); break;
-    case EPI_XPAY:            launch_one<P, RECON, true, false, false, false>(a, grid, block, s); break;
-    case EPI_XPAY_CLOVOUT:    launch_one<P, RECON, true, false, true, false>(a, grid, block, s); break;
-    case EPI_CLOVX_XPAY_DOTS: launch_one<P, RECON, true, true, false, true>(a, grid, block, s); break;
-    case EPI_XPAY_CLOVD:      launch_one<P, RECON, true, true, true, false>(a, grid, block, s); break;
+    case EPI_NONE:            launch_one<P, RECON, false, false, false, 0>(a, grid, block, s); break;
+    case EPI_CLOVOUT:         launch_one<P, RECON, false, false, true, 0>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY:      launch_one<P, RECON, true, true, false, 0>(a, grid, block, s); break;
+    case EPI_XPAY:            launch_one<P, RECON, true, false, false, 0>(a, grid, block, s); break;
+    case EPI_XPAY_CLOVOUT:    launch_one<P, RECON, true, false, true, 0>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY_DOTS: launch_one<P, RECON, true, true, false, 1>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY_YDOT: launch_one<P, RECON, true, true, false, 2>(a, grid, block, s); break;
+    case EPI_CLOVX_XPAY_QDOT: launch_one<P, RECON, true, true, false, 3>(a, grid, block, s); break;
+    case EPI_XPAY_CLOVD:      launch_one<P, RECON, true, true, true, 0>(a, grid, block, s); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

@@ -97,6 +97,8 @@ struct lqcd_ctx {
   size_t partials_doubles;
   unsigned* counters;
   unsigned* gflag;        // device word written by the gauge conversion check (pack.cu)
+  double* dotws;          // workspace of the reductions fused into the operator (dslash.cuh DOTS >= 2)
+  size_t dotws_doubles;
   double* boxdots;        // MR per-box partial dots
   size_t boxdots_doubles;
   double* hS;             // pinned host mirror of S

@@ -21,7 +21,7 @@ typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;
 typedef OpMrUpdate<true, true> OpMrOnly;
 
-struct EventPair { cudaEvent_t a, b; ~EventPair() { cudaEventDestroy(a); cudaEventDestroy(b); } };
+struct EventPair { cudaEvent_t a = nullptr, b = nullptr; ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); } };
 
 struct Work {                      // workspace of one call; goes back to the context's cache when it leaves scope
   lqcd_ctx* c;
@@ -174,55 +174,100 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
     { BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc; }
     double maxr = rin;
     const double r_start = rn;                // divergence guard: BiCGstab can blow up on an indefinite operator (kappa > kappa_c)
-    int it = 0;
+    // The host decides on reliable updates and convergence from ||r_l||^2 and the breakdown flag of every iteration,
+    // but it reads them ONE ITERATION LATE: iteration k+1 is enqueued before the host waits for the scalars of
+    // iteration k, so the device never idles on the read-back (it cost 38 us of a 730 us iteration).  An update then
+    // happens one iteration after its trigger; that iteration is an ordinary BiCGstab step and is folded into x with
+    // the rest, so only the very last one of a solve is spent for nothing.
+    // The scalars travel through pinned host memory the last CTA of the iteration's final kernel writes directly
+    // (blas_ops.cuh OpBicgXR::publish): no memcpy and no event sits between two kernels of the stream.
+    volatile double* hs = c->hS + S_TOTAL;    // pinned: words 4 (k & 1) .. +2 hold (rr, flag, k) of iteration k
+    hs[2] = hs[6] = -1.0;
+    auto fold = [&]() -> int {                // x += x_l (outer precision)
+      MultiArgs m; memset(&m, 0, sizeof(m));
+      m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
+      cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
+      return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "accumulate", e);
+    };
+    auto enqueue = [&](int k) -> int {        // iteration k (1-based): kernels, then the asynchronous read-back of its scalars
+      int rc2;
+      { BlasArgs a = mk(c, false, pv, rl, v); if ((rc2 = blas<OpBicgP>(c, ps, a, s))) return rc2; }
+      if (!sym) {
+        // <rtilde, v> -> alpha and (<t,s>, <t,t>) -> omega are reduced in the second launch of Mhat (dslash.cuh DOTS 3 / 2)
+        if ((rc2 = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, 0, FIN_BICG_ALPHA, rt))) return rc2;
+      } else {
+        if ((rc2 = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc2;
+        BlasArgs a = mk(c, false, rt, v); if ((rc2 = blas<OpBicgAlpha>(c, ps, a, s))) return rc2;
+      }
+      { BlasArgs a = mk(c, false, rl, v); if ((rc2 = blas<OpBicgS>(c, ps, a, s))) return rc2; }
+      if (!sym) {
+        if ((rc2 = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, 0, FIN_BICG_OMEGA, nullptr))) return rc2;
+      } else {
+        if ((rc2 = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc2;
+        BlasArgs a = mk(c, false, t, rl); if ((rc2 = blas<OpBicgOmega>(c, ps, a, s))) return rc2;
+      }
+      { BlasArgs a = mk(c, false, xl, pv, rl, t, rt); a.i0 = k; a.hmirror = c->hS + S_TOTAL;
+        if ((rc2 = blas<OpBicgXR>(c, ps, a, s))) return rc2; }
+      cnt.mat_sloppy += 2; cnt.blas_flop_sites += 1056;
+      return LQCD_OK;
+    };
+    auto wait_for = [&](int k) -> int {       // spin until iteration k has published; a failed stream ends the wait
+      long long spins = 0;
+      while (hs[4 * (k & 1) + 2] != (double)k) {
+        if ((++spins & 0xfffff) == 0 && cudaStreamQuery(s) != cudaErrorNotReady) {
+          if (hs[4 * (k & 1) + 2] == (double)k) break;
+          return fail(c, LQCD_ECUDA, "scalar read-back", cudaGetLastError());
+        }
+      }
+      return LQCD_OK;
+    };
+    int it = 0, seen = 0;                     // iterations enqueued / examined by the host
     while (true) {
-      if (it >= p.max_iter) {
-        // iteration cap: fold what the low-precision iteration has accumulated since the last
-        // reliable update into x, so that the caller gets the best iterate and its true residual
-        MultiArgs m; memset(&m, 0, sizeof(m));
-        m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
-        cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
-        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
+      const bool can = it < p.max_iter;
+      if (can) { if ((rc = enqueue(it + 1))) return rc; ++it; }
+      const int upto = can ? it - 1 : it;     // keep one iteration in flight unless the cap is reached
+      bool trigger = false;
+      while (seen < upto && !trigger) {
+        ++seen;
+        if ((rc = wait_for(seen))) return rc;
+        const double rr = hs[4 * (seen & 1)], flag = hs[4 * (seen & 1) + 1];
+        if (!(rr == rr) || flag != 0.0) status = LQCD_EBREAKDOWN;
+        const double rln = sqrt(rr);
+        if (rln > maxr) maxr = rln;
+        trigger = status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr;
+      }
+      if (!trigger) {
+        if (can || seen < it) continue;
+        // iteration cap: fold what the low-precision iteration has accumulated since the last reliable update
+        // into x, so that the caller gets the best iterate and its true residual
+        if ((rc = fold())) return rc;
         status = LQCD_ENOCONV;
         break;
       }
-      { BlasArgs a = mk(c, false, pv, rl, v); if ((rc = blas<OpBicgP>(c, ps, a, s))) return rc; }
-      if ((rc = op_matpc(c, v, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
-      { BlasArgs a = mk(c, false, rt, v); if ((rc = blas<OpBicgAlpha>(c, ps, a, s))) return rc; }
-      { BlasArgs a = mk(c, false, rl, v); if ((rc = blas<OpBicgS>(c, ps, a, s))) return rc; }
-      if ((rc = op_matpc(c, t, rl, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
-      { BlasArgs a = mk(c, false, t, rl); if ((rc = blas<OpBicgOmega>(c, ps, a, s))) return rc; }
-      { BlasArgs a = mk(c, false, xl, pv, rl, t, rt); if ((rc = blas<OpBicgXR>(c, ps, a, s))) return rc; }
-      cnt.mat_sloppy += 2; cnt.blas_flop_sites += 1056; ++it;
-      if ((rc = read_S(c, S_RR, 2, s))) return rc;
-      const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
-      if (!(rr == rr) || flag != 0.0) { status = LQCD_EBREAKDOWN; }
-      const double rln = sqrt(rr);
-      if (rln > maxr) maxr = rln;
-      if (status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr) {
-        // reliable update: fold x_l into x, recompute the true residual in the outer precision
-        MultiArgs m; memset(&m, 0, sizeof(m));
-        m.b = mk(c, false); m.z[0] = xl; m.chi[0] = 1.0; m.n = 1;
-        cudaError_t e = run_accumulate(po, ps, x, m, s); c->launches++;
-        if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "accumulate", e);
-        { BlasArgs a = mk(c, false, xl); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
-        if ((rc = true_residual())) return rc;
-        res->restarts++;
-        if (rn <= stop) { status = LQCD_OK; break; }
-        if (rn > 1e5 * r_start) { status = LQCD_EBREAKDOWN; break; }      // the true residual has grown 1e5-fold: give up
-        if (status == LQCD_EBREAKDOWN) {
-          // restart the recurrence from the true residual
-          status = LQCD_OK;
-          if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
-          if ((rc = convert(c, ps, ps, rt, rl, 0, par, s))) return rc;
-          for (char* z : {pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
-          BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
-          if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
-        } else {
-          if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
-          BlasArgs a = mk(c, false, rt, rl); a.i0 = 1; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
-        }
-        maxr = rin;
+      // reliable update: fold x_l into x (everything enqueued so far), recompute the true residual in the outer precision
+      seen = it;
+      if ((rc = fold())) return rc;
+      { BlasArgs a = mk(c, false, xl); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+      if ((rc = true_residual())) return rc;
+      res->restarts++;
+      if (rn <= stop) { status = LQCD_OK; break; }
+      if (rn > 1e5 * r_start) { status = LQCD_EBREAKDOWN; break; }      // the true residual has grown 1e5-fold: give up
+      if (!(rn == rn)) { status = LQCD_EBREAKDOWN; break; }
+      if (status == LQCD_EBREAKDOWN) {
+        // restart the recurrence from the true residual
+        status = LQCD_OK;
+        if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+        if ((rc = convert(c, ps, ps, rt, rl, 0, par, s))) return rc;
+        for (char* z : {pv, v}) { BlasArgs a = mk(c, false, z); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
+        BlasArgs a = mk(c, false, rt, rl); a.i0 = 0; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
+      } else {
+        if ((rc = convert(c, po, ps, rl, r_hi, 0, par, s))) return rc;
+        BlasArgs a = mk(c, false, rt, rl); a.i0 = 1; if ((rc = blas<OpBicgInit>(c, ps, a, s))) return rc;
+      }
+      maxr = rin;
+      if (!can) {                              // the cap was reached and this update did not converge
+        status = LQCD_ENOCONV;
+        break;
       }
     }
     res->iterations = it;
@@ -282,8 +327,12 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
     int it = 0;
     while (true) {
       if (it >= p.max_iter) { if ((rc = fold())) return rc; status = LQCD_ENOCONV; break; }
-      if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
-      { BlasArgs a = mk(c, false, w); if ((rc = blas<OpCgAlpha>(c, ps, a, s))) return rc; }
+      if (!sym) {                               // ||w||^2 -> alpha reduced in the second launch of Mhat (dslash.cuh DOTS 2)
+        if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, 0, FIN_CG_ALPHA, nullptr))) return rc;
+      } else {
+        if ((rc = op_matpc(c, w, pv, par, 0, p.kappa, ps, p.recon_sloppy, false, false, s, sym))) return rc;
+        BlasArgs a = mk(c, false, w); if ((rc = blas<OpCgAlpha>(c, ps, a, s))) return rc;
+      }
       { BlasArgs a = mk(c, false, xl, pv, rl, w); if ((rc = blas<OpCgXR>(c, ps, a, s))) return rc; }
       cnt.mat_sloppy++; cnt.blas_flop_sites += 24.0 * (2 + 4 + 2); ++it;
       if ((rc = read_S(c, S_RR, 2, s))) return rc;
