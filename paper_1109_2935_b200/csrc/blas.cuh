@@ -123,8 +123,13 @@ LQ_DEV void reduce_and_finalize(double* red, const BlasArgs& a, int box, F fin) 
 //   NV (number of fp64 reductions), READ / WRITE bit masks over v[0..4],
 //   struct Coef; prepare(Coef&, const BlasArgs&, int box);
 //   site<R>(const Coef&, R* v0..v4, double* red);  finalize(const double* sum, const BlasArgs&, int box)
+// half precision: a site needs all 24 decoded values of every operand before it can re-quantise, and the widest passes
+// (OpBicgXR: 5 operands) would take 137 registers = one CTA of 8 warps per SM; capped at 128 for two (measured below)
+#ifndef LQ_BLAS_MINB_HALF
+#define LQ_BLAS_MINB_HALF 2
+#endif
 template <class P, class Op>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK) blas_kernel(const BlasArgs a0) {
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK, (P::HALF ? LQ_BLAS_MINB_HALF : 1)) blas_kernel(const BlasArgs a0) {
   typedef typename P::real R;
   const int box = blockIdx.y;
   BlasArgs a = a0;
