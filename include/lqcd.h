@@ -146,6 +146,10 @@ int lqcd_schwarz(lqcd_ctx* ctx, void* out, const void* in, int parity, double ka
                  const int block[4], int n_mr, double omega_mr, int prec, int recon,
                  int prec_io, void* stream);
 
+/* Blocks per launch group for later lqcd_schwarz calls on this context (lqcd_invert takes it from
+ * lqcd_invert_params::schwarz_group); 0 = all blocks per launch.  LQCD_EINVAL if negative. */
+int lqcd_set_schwarz_group(lqcd_ctx* ctx, int blocks_per_group);
+
 typedef struct {
   double kappa;
   double c_sw;            /* must equal the value given to lqcd_build_clover */
@@ -165,6 +169,15 @@ typedef struct {
   int    matpc_type;      /* LQCD_MATPC_ASYMMETRIC (default, R6) or LQCD_MATPC_SYMMETRIC: the Krylov iteration runs on
                              Mhat_s x_p = A_pp^-1 bhat; the stopping test stays ||b - M x|| <= tol ||b|| (fp64, at
                              reliable updates).  BiCGstab, CGNR and CGNE only. */
+  int    schwarz_group;   /* GCR-DD: blocks per launch group of the preconditioner; all mr_steps run on one group before
+                             the next is touched, so that a group sized to the L2 (about 5 blocks of 12^3x24 in half) keeps
+                             its links, clover blocks and vectors on chip.  0 = all blocks
+                             in one launch per step.  Results do not depend on it (blocks are independent). */
+  int    history_len;     /* capacity of residual_history in doubles (0 = none) */
+  double* residual_history; /* optional HOST buffer (caller-owned): entry k = iterated residual norm / ||b|| after
+                             iteration k+1 of the low-precision iteration (BiCGstab, CGNR, CGNE) or after outer iteration
+                             k+1 (GCR); lqcd_invert_result::history_count entries are written.  Reported, never
+                             asserted (convergence history is "parity unpinned"). */
 } lqcd_invert_params;
 
 typedef struct {
@@ -176,6 +189,7 @@ typedef struct {
   double iterated_residual;
   double seconds;         /* device time of the whole call (CUDA events) */
   double gflop;           /* nominal flops executed (operators 3696/site + BLAS-1) / 1e9 */
+  int    history_count;   /* entries written to lqcd_invert_params::residual_history */
 } lqcd_invert_result;
 
 /* Solve M x = b on the full lattice (Eq. 1): source preparation, parity solve of the Schur

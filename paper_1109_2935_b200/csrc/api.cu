@@ -180,11 +180,17 @@ static int get_dotws(lqcd_ctx* c, int nsite, double** out, cudaStream_t s) {
 }
 
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
-              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0, int cb1, int fin, const char* q) {
+              int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0, int cb1, int fin, const char* q,
+              int box0, int nbox) {
   DslashArgs d;
   memset(&d, 0, sizeof(d));
   d.g = blocked ? c->bm.blk : c->nat;
   d.out = out; d.in = in; d.y = y; d.a = a; d.parity = parity_out; d.dagger = dagger;
+  if (nbox > 0) {                                   // a group of Schwarz blocks: boxes [box0, box0 + nbox)
+    if (!blocked || box0 < 0 || box0 + nbox > d.g.nb) return fail(c, LQCD_EINVAL, "box range");
+    d.g.nb = nbox;                                  // boxes of this launch; g.ns stays the stride of the whole field
+    d.parity = parity_out | (box0 << 8);
+  }
   int rc = get_gauge(c, prec, recon, blocked, &d.gauge, s);
   if (rc) return rc;
   if (epi != EPI_NONE && epi != EPI_XPAY) {
@@ -219,7 +225,7 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
 // fin != 0 (asymmetric form, natural layout only): the second launch also reduces <out,in>, ||out||^2 (q == nullptr) or
 // <q,out>, ||out||^2 over the field and its last CTA performs the scalar update `fin` (DotsFin, dslash.cuh)
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
-             bool blocked, bool dots, cudaStream_t s, int sym, int fin, const char* q) {
+             bool blocked, bool dots, cudaStream_t s, int sym, int fin, const char* q, int box0, int nbox) {
   char* tmp;
   int rc = get_tmp(c, prec, blocked, &tmp);
   if (rc) return rc;
@@ -241,12 +247,12 @@ int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, dou
     if (rc) return rc;
     return op_dslash(c, out, tmp, in, parity, 1, prec, recon, EPI_XPAY, -kappa * kappa, kappa, false, s);
   }
-  rc = op_dslash(c, tmp, in, nullptr, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, blocked, s);
+  rc = op_dslash(c, tmp, in, nullptr, 1 - parity, dagger, prec, recon, EPI_CLOVOUT, 0.0, kappa, blocked, s, 0, -1, 0, nullptr, box0, nbox);
   if (rc) return rc;
   if (fin) return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, q ? EPI_CLOVX_XPAY_QDOT : EPI_CLOVX_XPAY_YDOT,
                             -kappa * kappa, kappa, blocked, s, 0, -1, fin, q);
   return op_dslash(c, out, tmp, in, parity, dagger, prec, recon, dots ? EPI_CLOVX_XPAY_DOTS : EPI_CLOVX_XPAY,
-                   -kappa * kappa, kappa, blocked, s);
+                   -kappa * kappa, kappa, blocked, s, 0, -1, 0, nullptr, box0, nbox);
 }
 
 // multi-right-hand-side Dslash: the same fused launch for nrhs fields sharing the links
@@ -320,6 +326,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   c->bm.nat = c->nat; c->bm.blk = c->nat; c->bm.nbd[0] = c->bm.nbd[1] = c->bm.nbd[2] = c->bm.nbd[3] = 1;
   c->launches = 0;
   c->have_gauge = c->have_blocks = c->have_clover = false;
+  c->schwarz_group = 0;
   c->g64 = nullptr; c->T72 = nullptr; c->kappa = NAN; c->c_sw = NAN;
   memset(c->gauge, 0, sizeof(c->gauge)); memset(c->bgauge, 0, sizeof(c->bgauge));
   memset(c->clov, 0, sizeof(c->clov)); memset(c->clovinv, 0, sizeof(c->clovinv));

@@ -51,6 +51,7 @@ struct BlasArgs {
   long long rhs_partials;
   // pinned host words the last CTA may publish scalars to (zero-copy; no memcpy or event between two kernels)
   double* hmirror;
+  int box0;               // first box of the launch (gridDim.y counts boxes from it): Schwarz block groups
 };
 
 struct cd { double re, im; };
@@ -131,7 +132,7 @@ LQ_DEV void reduce_and_finalize(double* red, const BlasArgs& a, int box, F fin) 
 template <class P, class Op>
 __global__ void __launch_bounds__(LQ_BLAS_BLOCK, (P::HALF ? LQ_BLAS_MINB_HALF : 1)) blas_kernel(const BlasArgs a0) {
   typedef typename P::real R;
-  const int box = blockIdx.y;
+  const int box = blockIdx.y + a0.box0;
   BlasArgs a = a0;
   if (a0.rhs_bytes) {                       // one right-hand side per blockIdx.z, each with its own scalars
     const int r = blockIdx.z;

@@ -37,7 +37,7 @@ struct DslashArgs {
     double* dots;       // DOTS: [box][chunk][warp][4] partials (re<r,y>, im<r,y>, <r,r>, unused)
     struct { int cb0, cb1; } range;  // !DOTS: sites [cb0, cb1) of every box are computed by this launch
   };
-  int parity;           // output parity
+  int parity;           // output parity (bit 0); bits 8.. = first box of the launch (the grid's y extent counts boxes from it)
   int dagger;
 };
 static_assert(sizeof(DslashArgs) == 128, "DslashArgs must stay 128 bytes (see above)");
@@ -462,13 +462,13 @@ dslash_kernel(const DslashArgs a) {
   typedef typename P::real R;
   const Geom& g = a.g;
   const int cb = (DOTS ? 0 : a.range.cb0) + blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
-  const int box = blockIdx.y;
+  const int box = blockIdx.y + (a.parity >> 8);            // first box of the launch: Schwarz block groups (solver.cu)
   const bool active = cb < (DOTS ? g.vh : a.range.cb1);
   R d0 = 0, d1 = 0, d2 = 0;                 // DOTS: this site's <r,y> (re, im) and <r,r>
   if (active) {
     const long long base = (long long)box * g.vh;
     const long long idx = base + cb;
-    const int p = a.parity;
+    const int p = a.parity & 1;
     int c[4];
     cb_to_coords(g, cb, p, c);
     const int xh = c[0] >> 1;

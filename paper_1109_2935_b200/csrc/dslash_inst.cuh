@@ -105,7 +105,7 @@ template <class P, int RECON>
 static cudaError_t launch_dslash_r(const DslashArgs& a, int epi, cudaStream_t s) {
   const bool whole = epi == EPI_CLOVX_XPAY_DOTS || epi == EPI_CLOVX_XPAY_YDOT || epi == EPI_CLOVX_XPAY_QDOT;   // no site range (dslash.cuh)
   const int nsite = whole ? a.g.vh : a.range.cb1 - a.range.cb0;
-  dim3 grid((nsite + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);
+  dim3 grid((nsite + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, a.g.nb);   // g.nb = boxes of this launch (g.ns keeps the field stride)
   dim3 block(LQ_DSLASH_BLOCK);
   switch (epi) {
     case EPI_NONE:            launch_one<P, RECON, false, false, false, 0>(a, grid, block, s); break;

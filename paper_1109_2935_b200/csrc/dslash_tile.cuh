@@ -150,7 +150,7 @@ dslash_tile_kernel(const DslashArgs a, const TileInfo ti) {
   const Geom& g = a.g;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const long long base = 0;                       // one box (tile_ok)
-  const int p = a.parity;
+  const int p = a.parity & 1;
   // the tile: rows y0 .. y0 + rows - 1 of the plane (z, t)
   const int y0 = blockIdx.x * ti.rows, z = blockIdx.y, t = ti.t0 + blockIdx.z;
   const int cb0 = ((t * g.X[2] + z) * g.X[1] + y0) * g.Xh;
@@ -236,7 +236,7 @@ template <int RECON> inline void tile_planes(const DslashArgs& a, TileInfo& ti) 
   for (int pl = 0; pl < 4; ++pl) ti.sp[pl] = a.in + (pl < 3 ? 16ll * pl : 48ll) * ns;
   for (int fb = 0; fb < 2; ++fb)
     for (int mu = 0; mu < 4; ++mu) {
-      const char* f = a.gauge + (long long)(((fb == 0 ? a.parity : 1 - a.parity) * 4) + mu) * link_bytes;
+      const char* f = a.gauge + (long long)(((fb == 0 ? (a.parity & 1) : 1 - (a.parity & 1)) * 4) + mu) * link_bytes;
       for (int pl = 0; pl < 3; ++pl) {
         const long long off = pl < RC::N16 ? 16ll * pl : (RC::N8 && pl == RC::N16) ? 16ll * RC::N16 : 16ll * RC::N16 + 8ll * RC::N8;
         ti.lk[fb][mu][pl] = f + off * ns;

@@ -67,6 +67,7 @@ struct lqcd_ctx {
   int dims[4], bc[4], device;
   long long V, Vh;
   std::string err;
+  std::vector<double> hist;   // iterated residual norms of the running solve (lqcd_invert_params::residual_history)
   lq::Geom nat;
   int n_sm;
   long long launches;
@@ -79,6 +80,7 @@ struct lqcd_ctx {
   bool have_blocks;
   lq::BlockMap bm;
   char* bgauge[3][3];
+  int schwarz_group;      // blocks per launch group of the preconditioner (0 = all; lqcd_invert_params::schwarz_group)
   // clover
   bool have_clover;
   double c_sw;

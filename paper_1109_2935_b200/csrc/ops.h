@@ -17,9 +17,10 @@ int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out);
 int set_blocks(lqcd_ctx* c, const int* blk);
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
               int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0 = 0, int cb1 = -1, int fin = 0,
-              const char* q = nullptr);
+              const char* q = nullptr, int box0 = 0, int nbox = 0);
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
-             bool blocked, bool dots, cudaStream_t s, int sym = 0, int fin = 0, const char* q = nullptr);
+             bool blocked, bool dots, cudaStream_t s, int sym = 0, int fin = 0, const char* q = nullptr,
+             int box0 = 0, int nbox = 0);
 
 // multi-right-hand-side forms (dslash_mrhs.cuh): in / out / y hold nrhs packed fields back to back
 int op_dslash_mrhs(lqcd_ctx* c, char* out, const char* in, const char* y, int nrhs, int parity_out, int dagger, int prec,

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <complex>
 #include <cstring>
+#include <nvtx3/nvToolsExt.h>
 #include "blas_ops.cuh"
 #include "ops.h"
 
@@ -20,6 +21,9 @@ typedef OpMrUpdate<true, false> OpMrFirst;
 typedef OpMrUpdate<false, false> OpMrMid;
 typedef OpMrUpdate<false, true> OpMrLast;
 typedef OpMrUpdate<true, true> OpMrOnly;
+
+// NVTX range around a solver phase (tracing); shows up in Nsight timelines, costs nothing without a tool attached
+struct Range { explicit Range(const char* name) { nvtxRangePushA(name); } ~Range() { nvtxRangePop(); } };
 
 struct EventPair { cudaEvent_t a = nullptr, b = nullptr; ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); } };
 
@@ -117,19 +121,31 @@ namespace lq {
 // workspace in precision prec (allocated by the caller).
 int schwarz_apply(lqcd_ctx* c, char* out, const char* in, int parity, double kappa, int n_mr, double omega,
                   int prec, int recon, int prec_io, char* rho, char* w, char* xk, cudaStream_t s) {
+  Range nv("lqcd: Schwarz preconditioner K");
   int rc = convert(c, prec_io, prec, rho, in, 1, parity, s);
   if (rc) return rc;
-  for (int step = 0; step < n_mr; ++step) {
-    rc = op_matpc(c, w, rho, parity, 0, kappa, prec, recon, true, true, s);
-    if (rc) return rc;
-    BlasArgs a = mk(c, true, xk, rho, w);
-    a.c[0] = omega;
-    const bool first = step == 0, last = step == n_mr - 1;
-    if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
-    else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
-    else if (last) rc = blas<OpMrLast>(c, prec, a, s);
-    else rc = blas<OpMrMid>(c, prec, a, s);
-    if (rc) return rc;
+  // Block-group schedule ("multiple levels of Schwarz-type blocking to take advantage of the multiple
+  // levels of memory locality"): the blocks are independent, so all n_mr steps can run on a group of
+  // `group` blocks -- sized so that the group's spinors, links and clover blocks stay in L2 -- before the next group
+  // is touched.  The block-major layout makes a group a contiguous box range.  group = 0: all blocks per launch.
+  const int nb = c->bm.blk.nb;
+  const int group = (c->schwarz_group > 0 && c->schwarz_group < nb) ? c->schwarz_group : nb;
+  for (int b0 = 0; b0 < nb; b0 += group) {
+    const int gn = (b0 + group <= nb) ? group : nb - b0;
+    const int box0 = group == nb ? 0 : b0, nbox = group == nb ? 0 : gn;
+    for (int step = 0; step < n_mr; ++step) {
+      rc = op_matpc(c, w, rho, parity, 0, kappa, prec, recon, true, true, s, 0, 0, nullptr, box0, nbox);
+      if (rc) return rc;
+      BlasArgs a = mk(c, true, xk, rho, w);
+      a.c[0] = omega;
+      if (nbox) { a.box0 = box0; a.nb = nbox; }
+      const bool first = step == 0, last = step == n_mr - 1;
+      if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
+      else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
+      else if (last) rc = blas<OpMrLast>(c, prec, a, s);
+      else rc = blas<OpMrMid>(c, prec, a, s);
+      if (rc) return rc;
+    }
   }
   return convert(c, prec, prec_io, out, xk, 2, parity, s);
 }
@@ -153,6 +169,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
   double rn, rin, istop = stop;       // rin, istop: norm and stopping threshold of the residual the inner iteration sees
   // true residual in the outer precision; symmetric form: hand A^-1 r to the inner iteration and scale its threshold
   auto true_residual = [&]() -> int {
+    Range nv("lqcd: true residual (outer precision)");
     int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
     if (rc2) return rc2;
     cnt.mat_outer++;
@@ -233,6 +250,7 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
         const double rr = hs[4 * (seen & 1)], flag = hs[4 * (seen & 1) + 1];
         if (!(rr == rr) || flag != 0.0) status = LQCD_EBREAKDOWN;
         const double rln = sqrt(rr);
+        c->hist.push_back(rln);
         if (rln > maxr) maxr = rln;
         trigger = status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr;
       }
@@ -245,7 +263,11 @@ int solve_bicgstab(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params
         break;
       }
       // reliable update: fold x_l into x (everything enqueued so far), recompute the true residual in the outer precision
-      seen = it;
+      while (seen < it) {                      // the iteration in flight belongs to the history as well
+        ++seen;
+        if ((rc = wait_for(seen))) return rc;
+        c->hist.push_back(sqrt(hs[4 * (seen & 1)]));
+      }
       if ((rc = fold())) return rc;
       { BlasArgs a = mk(c, false, xl); if ((rc = blas<OpZero>(c, ps, a, s))) return rc; }
       if ((rc = true_residual())) return rc;
@@ -294,6 +316,7 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
   const int sym = p.matpc_type == LQCD_MATPC_SYMMETRIC;
   double rn, rin, istop = stop;
   auto true_residual = [&]() -> int {      // as in solve_bicgstab
+    Range nv("lqcd: true residual (outer precision)");
     int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
     if (rc2) return rc2;
     cnt.mat_outer++;
@@ -339,6 +362,7 @@ int solve_cgnr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
       const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
       if (!(rr == rr) || flag != 0.0) status = LQCD_EBREAKDOWN;
       const double rln = sqrt(rr);
+      c->hist.push_back(rln);
       if (rln > maxr) maxr = rln;
       if (status == LQCD_EBREAKDOWN || rln <= istop || rln < delta * maxr) {
         if ((rc = fold())) return rc;
@@ -380,6 +404,7 @@ int solve_cgne(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
   const int sym = p.matpc_type == LQCD_MATPC_SYMMETRIC;
   double rn, rin, istop = stop;
   auto true_residual = [&]() -> int {      // as in solve_bicgstab
+    Range nv("lqcd: true residual (outer precision)");
     int rc2 = residual(c, r_hi, b, x, par, p.kappa, po, p.recon_outer, &rn, s);
     if (rc2) return rc2;
     cnt.mat_outer++;
@@ -429,6 +454,7 @@ int solve_cgne(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p,
       const double rr = c->hS[S_RR], flag = c->hS[S_FLAG];
       const bool bad = !(rr == rr) || flag != 0.0;
       const double rln = sqrt(rr);
+      c->hist.push_back(rln);
       if (rln > maxr) maxr = rln;
       bool replaced = false;
       if (bad || rln <= istop || rln < delta * maxr) {
@@ -476,6 +502,8 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
     if ((rc = wk.get(&zh[i], spinor_bytes(ps, ns)))) return rc;
   }
   if (p.precondition) {
+    if (p.schwarz_group < 0) return fail(c, LQCD_EINVAL, "schwarz_group");
+    c->schwarz_group = p.schwarz_group;
     if ((rc = set_blocks(c, p.schwarz_block))) return rc;
     for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, ns)))) return rc;
   }
@@ -515,6 +543,7 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
       ++k; ++total;
       if ((rc = read_S(c, S_RR, 1, s))) return rc;
       const double rhn = sqrt(c->hS[S_RR]);
+      c->hist.push_back(rhn);
       if (k == kmax || rhn / r0n < delta || rhn < stop || total >= p.max_iter || !(rhn == rhn)) break;
     }
     // implicit solution update: back-substitution for chi, then x += sum chi_i p_i
@@ -739,6 +768,13 @@ int lqcd_schwarz(lqcd_ctx* c, void* out, const void* in, int parity, double kapp
   return rc;
 }
 
+int lqcd_set_schwarz_group(lqcd_ctx* c, int blocks_per_group) {
+  if (!c) return LQCD_EINVAL;
+  if (blocks_per_group < 0) return fail(c, LQCD_EINVAL, "schwarz group");
+  c->schwarz_group = blocks_per_group;
+  return LQCD_OK;
+}
+
 int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_params* p, lqcd_invert_result* res, void* stream) {
   if (!c) return LQCD_EINVAL;
   if (!x_can || !b_can || !res) return fail(c, LQCD_EINVAL, "invert arguments");
@@ -747,6 +783,8 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
   memset(res, 0, sizeof(*res));
+  c->hist.clear();
+  if (p->history_len < 0 || (p->history_len > 0 && !p->residual_history)) return fail(c, LQCD_EINVAL, "residual_history");
   const int po = p->prec_outer, par = p->parity;
   const long long ns = c->nat.ns;
   Work wk(c, s);
@@ -758,6 +796,8 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   EventPair ev{e0, e1};                 // destroyed on every return path
   cudaEventRecord(e0, s);
   Counts cnt;
+  nvtxRangePushA("lqcd_invert: prepare");
+  struct PopGuard { int n = 1; ~PopGuard() { while (n-- > 0) nvtxRangePop(); } } nvtx_guard;   // balances the ranges on every return path
   // pack b; ||b||
   cudaError_t e = run_pack_spinor(po, bp, (const double*)b_can, c->nat, par, 0, s); c->launches++;
   if (e == cudaSuccess) { e = run_pack_spinor(po, bq, (const double*)b_can, c->nat, 1 - par, 0, s); c->launches++; }
@@ -789,17 +829,20 @@ int lqcd_invert(lqcd_ctx* c, void* x_can, const void* b_can, const lqcd_invert_p
   }
   const double stop = p->tol * bnorm;
   int status;
+  nvtxRangePop(); nvtxRangePushA("lqcd_invert: iterate");
   if (p->solver == LQCD_SOLVER_BICGSTAB) status = solve_bicgstab(c, xp, bhat, *p, stop, res, cnt, s);
   else if (p->solver == LQCD_SOLVER_CGNR) status = solve_cgnr(c, xp, bhat, *p, stop, res, cnt, s);
   else if (p->solver == LQCD_SOLVER_CGNE) status = solve_cgne(c, xp, bhat, *p, stop, res, cnt, s);
   else status = solve_gcr(c, xp, bhat, *p, stop, res, cnt, s);
   if (status != LQCD_OK && status != LQCD_ENOCONV && status != LQCD_EBREAKDOWN) return status;
+  nvtxRangePop(); nvtxRangePushA("lqcd_invert: true residual, reconstruct, unpack");
   // true residual of the Schur system in the outer precision = ||b - M x|| (R6)
   double rn;
   if ((rc = residual(c, t1, bhat, xp, par, p->kappa, po, p->recon_outer, &rn, s))) return rc;
   cnt.mat_outer++;
   res->true_residual = rn / bnorm;
   res->iterated_residual /= bnorm;
+  for (size_t k = 0; k < c->hist.size() && (int)k < p->history_len; ++k) { p->residual_history[k] = c->hist[k] / bnorm; res->history_count = (int)k + 1; }
   // reconstruction: x_pbar = A^-1 (b_pbar + kappa D x_p)
   if ((rc = op_dslash(c, t1, xp, bq, 1 - par, 0, po, p->recon_outer, EPI_XPAY_CLOVOUT, p->kappa, p->kappa, false, s))) return rc;
   e = run_pack_spinor(po, xp, (const double*)x_can, c->nat, par, 1, s); c->launches++;

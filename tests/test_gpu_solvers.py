@@ -341,3 +341,41 @@ def test_beyond_critical_kappa_cgnr_converges_where_bicgstab_does_not():
         res = np.linalg.norm(b - oracle.M(x.cpu().numpy(), c.U, c.T, c.bc, kappa)) / np.linalg.norm(b)
         assert abs(res - info["true_residual"]) <= 1e-6 * res       # the reported residual is the real one
     c.ctx.close()
+
+
+def test_schwarz_block_groups_and_residual_history(mid):
+    """SURVEY NEXT-1 block-group schedule: K applied group by group (all MR steps on a group of blocks before the
+    next group) is bit-identical to K applied to all blocks at once, for every group size, and still the oracle's K;
+    GCR-DD with groups reaches the same solution.  The optional residual history has one entry per iteration, ends
+    below the stopping threshold and starts near ||bhat|| / ||b||."""
+    c = mid
+    lq = c.lqcd
+    kappa, blk = 0.124, (4, 4, 4, 8)
+    r = inputs.gaussian_spinor(c.dims, 7)
+    d = torch.from_numpy(r).cuda()
+    fin = c.ctx.pack_spinor(d, 0, 2)
+    outs = []
+    for group in (0, 1, 3, 5, 1000):
+        c.ctx.set_schwarz_group(group)
+        out = c.ctx.new_field(2)
+        c.ctx.schwarz(out, fin, 0, kappa, blk, 4, 1.0, 2, 12, 2)
+        outs.append(out)
+    c.ctx.set_schwarz_group(0)
+    for o in outs[1:]:
+        assert torch.equal(o, outs[0])
+    got = torch.zeros_like(d)
+    c.ctx.unpack_spinor(got, outs[2], 0, 2)
+    want = oracle.schwarz(r, c.U, c.T, c.bc, kappa, 0, blk, n_mr=4)
+    assert _rel(got.cpu().numpy(), want) <= 2e-2
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    for solver, kw in ((lq.SOLVER_GCR_DD, dict(schwarz_block=blk, mr_steps=4, schwarz_group=3)), (lq.SOLVER_BICGSTAB, {}),
+                       (lq.SOLVER_CGNR, {})):
+        p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=solver, prec=(0, 1, 2), recon=(18, 12, 12), history_len=4000, **kw)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0 and _rel(x, xo) <= 1e-8
+        h = info["residual_history"]
+        assert len(h) == info["iterations"] and all(v == v and v >= 0 for v in h)
+        assert 0.1 < h[0] < 3.0 and min(h) <= 1.2e-10
+    with pytest.raises(lq.LqcdError):
+        c.ctx.set_schwarz_group(-1)
