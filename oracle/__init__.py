@@ -55,7 +55,7 @@ def lib():
         build()
         _lib = ctypes.CDLL(_LIB)
         _lib.orc_num_threads.restype = ctypes.c_int
-        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_cgnr_pc", "orc_invert", "orc_invert_sym"):
+        for name in ("orc_bicgstab_pc", "orc_gcr_pc", "orc_gcr_sap_pc", "orc_cgnr_pc", "orc_invert", "orc_invert_sym"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -175,6 +175,27 @@ def schwarz(r, U, Tcl, bc, kappa, parity, block, n_mr=10, omega_mr=1.0):
     lib().orc_schwarz(_p(out), _p(r), _p(U), _p(Tcl), _i4(dims_of(r)), _i4(bc), ctypes.c_double(kappa),
                       ctypes.c_int(parity), _blk(block), ctypes.c_int(n_mr), ctypes.c_double(omega_mr))
     return out
+
+
+def schwarz_sap(r, U, Tcl, bc, kappa, parity, block, n_mr=4, omega_mr=1.0, n_cycle=1):
+    """Multiplicative Schwarz (SAP) preconditioner: n_cycle cycles over the two block colours (wilson_clover_oracle.cpp)."""
+    r, U, Tcl = _c(r), _c(U), _c(Tcl)
+    out = np.empty_like(r)
+    lib().orc_schwarz_sap(_p(out), _p(r), _p(U), _p(Tcl), _i4(dims_of(r)), _i4(bc), ctypes.c_double(kappa),
+                          ctypes.c_int(parity), _blk(block), ctypes.c_int(n_mr), ctypes.c_double(omega_mr), ctypes.c_int(n_cycle))
+    return out
+
+
+def gcr_sap_pc(bhat, U, Tcl, bc, kappa, parity, stop, block, maxit=10000, kmax=16, delta=0.1, n_mr=4, omega_mr=1.0, n_cycle=1):
+    """GCR preconditioned by the multiplicative Schwarz procedure on one parity.  Returns (x, info)."""
+    bhat, U, Tcl = _c(bhat), _c(U), _c(Tcl)
+    x = np.zeros_like(bhat)
+    it, rs, rn = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_double(0)
+    st = lib().orc_gcr_sap_pc(_p(x), _p(bhat), _p(U), _p(Tcl), _i4(dims_of(bhat)), _i4(bc), ctypes.c_double(kappa),
+                              ctypes.c_int(parity), ctypes.c_double(stop), ctypes.c_int(maxit), ctypes.c_int(kmax),
+                              ctypes.c_double(delta), _blk(block), ctypes.c_int(n_mr), ctypes.c_double(omega_mr),
+                              ctypes.c_int(n_cycle), ctypes.byref(it), ctypes.byref(rs), ctypes.byref(rn))
+    return x, dict(status=st, iterations=it.value, restarts=rs.value, residual_norm=rn.value)
 
 
 def bicgstab_pc(bhat, U, Tcl, bc, kappa, parity, stop, maxit=10000, x0=None):

@@ -480,11 +480,40 @@ void schwarz_K(cplx* out, const cplx* rin, const Op& opD, int p, int n_mr, doubl
   }
 }
 
+// Multiplicative Schwarz (SAP: section 4, "Schwarz alternating procedure" of ref. [20]; multiplicative
+// variant named in PAPER.md:146 section 3.2; reading R16 in DESIGN.md).  Blocks are coloured (bx+by+bz+bt) mod 2.
+// K_sap r: x = 0; repeat n_cycle times, for colour c = 0, 1:
+//   rho = r on the blocks of colour c, 0 elsewhere;  y = (n_mr MR steps on Mhat_D from 0, one alpha per block) rho;
+//   x += y;  r -= Mhat y   (the FULL operator: the other colour sees the update).
+// One cycle with the update of r dropped between the colours would be the additive K above.
+void schwarz_sap(cplx* out, const cplx* rin, const Op& op, const Op& opD, int p, int n_mr, double omega_mr, int n_cycle) {
+  const long n = opD.n(), V = opD.lat.V;
+  const Lat& lat = opD.lat;
+  const int* blk = opD.blk;
+  std::vector<int> colour(V);
+  for (long s = 0; s < V; ++s) {
+    int c[4]; lat.coords(s, c);
+    int sum = 0;
+    for (int m = 0; m < 4; ++m) sum += blk ? c[m] / blk[m] : 0;
+    colour[s] = sum & 1;
+  }
+  std::vector<cplx> r(rin, rin + n), rho(n), y(n), t(n);
+  mask_parity(r.data(), lat, p);
+  for (long i = 0; i < n; ++i) out[i] = 0;
+  for (int cyc = 0; cyc < n_cycle; ++cyc)
+    for (int c = 0; c < 2; ++c) {
+      for (long s = 0; s < V; ++s) for (int i = 0; i < 12; ++i) rho[s*12+i] = (colour[s] == c) ? r[s*12+i] : cplx(0.0);
+      schwarz_K(y.data(), rho.data(), opD, p, n_mr, omega_mr);
+      apply_matpc(t.data(), y.data(), op, p, 0);
+      for (long i = 0; i < n; ++i) { out[i] += y[i]; r[i] -= t[i]; }
+    }
+}
+
 // c.9  GCR-DD, Algorithm 1, all in fp64 here (hats kept as names only).
 // Stops when ||r0|| <= stop.  precond: 0 = identity (plain GCR), 1 = Schwarz K.
 int gcr_dd(cplx* x, const cplx* bhat, const Op& op, const Op& opD, int p, double stop, int maxit,
            int kmax, double delta, int precond, int n_mr, double omega_mr,
-           int* iters, int* restarts, double* rnorm) {
+           int* iters, int* restarts, double* rnorm, int sap_cycles = 0) {
   const long n = op.n();
   std::vector<cplx> r0(n), rh(n), tmp(n), xh(n);
   std::vector<std::vector<cplx>> ph(kmax, std::vector<cplx>(n)), zh(kmax, std::vector<cplx>(n));
@@ -498,7 +527,8 @@ int gcr_dd(cplx* x, const cplx* bhat, const Op& op, const Op& opD, int p, double
   int k = 0, total = 0, nrest = 0, status = 0;
   while (r0n > stop) {
     if (total >= maxit) { status = 1; break; }
-    if (precond) schwarz_K(ph[k].data(), rh.data(), opD, p, n_mr, omega_mr);
+    if (precond && sap_cycles > 0) schwarz_sap(ph[k].data(), rh.data(), op, opD, p, n_mr, omega_mr, sap_cycles);
+    else if (precond) schwarz_K(ph[k].data(), rh.data(), opD, p, n_mr, omega_mr);
     else ph[k] = rh;
     apply_matpc(zh[k].data(), ph[k].data(), op, p, 0);
     for (int i = 0; i < k; ++i) {                       // orthogonalisation (modified Gram-Schmidt)
@@ -612,6 +642,23 @@ void orc_schwarz(cplx* out, const cplx* rin, const cplx* U, const cplx* T, const
                  double kappa, int parity, const int* block, int n_mr, double omega_mr) {
   Op opD(U, T, dims, bc, kappa, block);
   schwarz_K(out, rin, opD, parity, n_mr, omega_mr);
+}
+
+// K_sap r on parity p (multiplicative Schwarz, n_cycle cycles over the two block colours)
+void orc_schwarz_sap(cplx* out, const cplx* rin, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                     double kappa, int parity, const int* block, int n_mr, double omega_mr, int n_cycle) {
+  Op op(U, T, dims, bc, kappa, nullptr);
+  Op opD(U, T, dims, bc, kappa, block);
+  schwarz_sap(out, rin, op, opD, parity, n_mr, omega_mr, n_cycle);
+}
+
+// GCR preconditioned by K_sap: solve Mhat x = bhat on one parity
+int orc_gcr_sap_pc(cplx* x, const cplx* bhat, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                   double kappa, int parity, double stop, int maxit, int kmax, double delta,
+                   const int* block, int n_mr, double omega_mr, int n_cycle, int* iters, int* restarts, double* rnorm) {
+  Op op(U, T, dims, bc, kappa, nullptr);
+  Op opD(U, T, dims, bc, kappa, block);
+  return gcr_dd(x, bhat, op, opD, parity, stop, maxit, kmax, delta, 1, n_mr, omega_mr, iters, restarts, rnorm, n_cycle);
 }
 
 // Parity-system solves: Mhat x_p = bhat.  stop is an ABSOLUTE residual norm.

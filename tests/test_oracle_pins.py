@@ -448,3 +448,51 @@ def test_gcr_identities(four):
     x5, i5 = oracle.gcr_pc(bh, U, Tcl, BC, kappa, p, stop, kmax=16, delta=0.1, precond=False)
     assert _rel(x4, x3) < 1e-10
     assert i4["iterations"] < i5["iterations"]
+
+
+# --------------------------------------------- multiplicative Schwarz, SAP (R16)
+def test_schwarz_sap_pins(four):
+    """K_sap against what fixes it: (1) with accurate block solves and many cycles the alternating procedure
+    converges to the dense solution Mhat^-1 r (a wrong sign or a stale residual between the colours diverges or
+    stalls); (2) the first colour sees the original residual, so on colour-0 blocks one cycle equals the (densely
+    pinned) additive K, and the second colour equals the additive K of the residual updated with the FULL operator;
+    (3) support and parity; (4) GCR preconditioned by K_sap reproduces the dense LU solution of M x = b."""
+    dims, U, Tcl, b, kappa = four
+    blk, p = (2, 2, 2, 2), 0
+    par = inputs.parity_mask(dims)
+    T_, Z_, Y_, X_ = b.shape[:4]
+    t, z, y, x = np.meshgrid(np.arange(T_), np.arange(Z_), np.arange(Y_), np.arange(X_), indexing="ij")
+    colour = ((x // blk[0]) + (y // blk[1]) + (z // blk[2]) + (t // blk[3])) & 1
+    r = b * (par == p)[..., None, None]
+    # (1) dense Schur complement solve
+    Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
+    sp = np.repeat(par.ravel(), 12)
+    ip, iq = np.where(sp == p)[0], np.where(sp != p)[0]
+    S = Md[np.ix_(ip, ip)] - Md[np.ix_(ip, iq)] @ np.linalg.solve(Md[np.ix_(iq, iq)], Md[np.ix_(iq, ip)])
+    want = np.zeros(r.size, dtype=complex)
+    want[ip] = np.linalg.solve(S, r.ravel()[ip])
+    got = oracle.schwarz_sap(r, U, Tcl, BC, kappa, p, blk, n_mr=60, n_cycle=40).ravel()
+    assert _rel(got, want) < 1e-9
+    e1 = _rel(oracle.schwarz_sap(r, U, Tcl, BC, kappa, p, blk, n_mr=60, n_cycle=1).ravel(), want)
+    e3 = _rel(oracle.schwarz_sap(r, U, Tcl, BC, kappa, p, blk, n_mr=60, n_cycle=3).ravel(), want)
+    assert e3 < e1 < 1.0                                        # the procedure contracts the error
+    # (2) one cycle, colour by colour, against the additive K and the full operator
+    m0, m1 = (colour == 0)[..., None, None], (colour == 1)[..., None, None]
+    ks = oracle.schwarz_sap(r, U, Tcl, BC, kappa, p, blk, n_mr=5, n_cycle=1)
+    y0 = oracle.schwarz(r * m0, U, Tcl, BC, kappa, p, blk, n_mr=5)
+    assert np.max(np.abs(y0 * m1)) == 0.0
+    assert _rel((ks * m0), y0) < 1e-13
+    r1 = r - oracle.matpc(y0, U, Tcl, BC, kappa, p)
+    y1 = oracle.schwarz(r1 * m1, U, Tcl, BC, kappa, p, blk, n_mr=5)
+    assert _rel((ks * m1), y1) < 1e-13
+    assert _rel((ks * m1), oracle.schwarz(r * m1, U, Tcl, BC, kappa, p, blk, n_mr=5)) > 1e-3    # and not the additive one
+    # (3) parity
+    assert np.max(np.abs(ks[par != p])) == 0.0
+    # (4) GCR-SAP solve
+    bhat = oracle.prepare_source(b, U, Tcl, BC, kappa, p)
+    xg, ig = oracle.gcr_sap_pc(bhat, U, Tcl, BC, kappa, p, 1e-12 * np.linalg.norm(b), blk, n_mr=4, n_cycle=1)
+    xs = np.zeros(r.size, dtype=complex)
+    xs[ip] = np.linalg.solve(S, bhat.ravel()[ip])
+    assert ig["status"] == 0 and _rel(xg.ravel(), xs) < 1e-10
+    xa, ia = oracle.gcr_pc(bhat, U, Tcl, BC, kappa, p, 1e-12 * np.linalg.norm(b), block=blk, n_mr=4)
+    assert ig["iterations"] <= ia["iterations"]                   # multiplicative beats additive per outer iteration here
