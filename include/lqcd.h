@@ -72,6 +72,9 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_MATPC_ASYMMETRIC 0
 #define LQCD_MATPC_SYMMETRIC  1
 
+#define LQCD_SCHWARZ_ADDITIVE       0
+#define LQCD_SCHWARZ_MULTIPLICATIVE 1
+
 #define LQCD_FIELD_SPINOR_PARITY 0
 #define LQCD_FIELD_STAGGERED_PARITY 1   /* 3-component colour vectors of one parity (fp64 / fp32 only) */
 
@@ -146,6 +149,15 @@ int lqcd_schwarz(lqcd_ctx* ctx, void* out, const void* in, int parity, double ka
                  const int block[4], int n_mr, double omega_mr, int prec, int recon,
                  int prec_io, void* stream);
 
+/* Multiplicative Schwarz (SAP: section 4, ref. [20]; named as the alternative to the additive form in
+ * PAPER.md:146; reading R16): blocks coloured (bx+by+bz+bt) mod 2, n_cycle cycles, in each cycle for colour 0 then 1:
+ * n_mr MR steps on the blocks of that colour applied to the current residual, out += y, residual -= Mhat y with the
+ * FULL operator (precision prec_io, links recon_io).  Needs an even number of blocks in x (LQCD_EINVAL otherwise).
+ * in / out: packed fields of precision prec_io, natural layout; the block solves run in `prec` / `recon`. */
+int lqcd_schwarz_sap(lqcd_ctx* ctx, void* out, const void* in, int parity, double kappa,
+                     const int block[4], int n_mr, double omega_mr, int n_cycle, int prec, int recon,
+                     int prec_io, int recon_io, void* stream);
+
 /* Blocks per launch group for later lqcd_schwarz calls on this context (lqcd_invert takes it from
  * lqcd_invert_params::schwarz_group); 0 = all blocks per launch.  LQCD_EINVAL if negative. */
 int lqcd_set_schwarz_group(lqcd_ctx* ctx, int blocks_per_group);
@@ -173,6 +185,8 @@ typedef struct {
                              the next is touched, so that a group sized to the L2 (about 5 blocks of 12^3x24 in half) keeps
                              its links, clover blocks and vectors on chip.  0 = all blocks
                              in one launch per step.  Results do not depend on it (blocks are independent). */
+  int    schwarz_type;    /* LQCD_SCHWARZ_ADDITIVE (default) or LQCD_SCHWARZ_MULTIPLICATIVE (lqcd_schwarz_sap) */
+  int    sap_cycles;      /* multiplicative: cycles over the two colours per preconditioner application (0 -> 1) */
   int    history_len;     /* capacity of residual_history in doubles (0 = none) */
   double* residual_history; /* optional HOST buffer (caller-owned): entry k = iterated residual norm / ||b|| after
                              iteration k+1 of the low-precision iteration (BiCGstab, CGNR, CGNE) or after outer iteration

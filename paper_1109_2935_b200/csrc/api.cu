@@ -133,12 +133,15 @@ int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out) {
   return LQCD_OK;
 }
 
-int set_blocks(lqcd_ctx* c, const int* blk) {
+int set_blocks(lqcd_ctx* c, const int* blk, int cmaj) {
   if (!blk) return fail(c, LQCD_EINVAL, "null block");
   for (int m = 0; m < 4; ++m)
     if (blk[m] < 2 || (blk[m] & 1) || c->dims[m] % blk[m]) return fail(c, LQCD_EINVAL, "Schwarz block extents must be even and divide the lattice");
-  if (c->have_blocks && !memcmp(blk, c->bm.blk.X, 4 * sizeof(int))) return LQCD_OK;
+  if (cmaj && ((c->dims[0] / blk[0]) & 1)) return fail(c, LQCD_EINVAL, "multiplicative Schwarz needs an even number of blocks in x");
+  // cmaj = 0: either box order will do (the additive preconditioner does not care), so matching copies are kept
+  if (c->have_blocks && !memcmp(blk, c->bm.blk.X, 4 * sizeof(int)) && (!cmaj || c->bm.cmaj)) return LQCD_OK;
   drop_block_copies(c);
+  c->bm.cmaj = cmaj ? 1 : 0;
   int nb = 1, bcb[4];
   for (int m = 0; m < 4; ++m) {
     c->bm.nbd[m] = c->dims[m] / blk[m];
@@ -323,7 +326,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   c->V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
   c->Vh = c->V / 2;
   c->nat = make_geom(dims, boundary, 1);
-  c->bm.nat = c->nat; c->bm.blk = c->nat; c->bm.nbd[0] = c->bm.nbd[1] = c->bm.nbd[2] = c->bm.nbd[3] = 1;
+  c->bm.nat = c->nat; c->bm.blk = c->nat; c->bm.nbd[0] = c->bm.nbd[1] = c->bm.nbd[2] = c->bm.nbd[3] = 1; c->bm.cmaj = 0;
   c->launches = 0;
   c->have_gauge = c->have_blocks = c->have_clover = false;
   c->schwarz_group = 0;

@@ -129,20 +129,28 @@ cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_
 // dst (PB) = src (PA), optionally permuting between the natural layout and the block-major
 // layout of the Schwarz preconditioner (dir: 0 none, 1 natural -> blocks, 2 blocks -> natural).
 template <class PA, class PB>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK) convert_kernel(char* dst, const char* src, const BlockMap bm, int dir, int parity) {
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) convert_kernel(char* dst, const char* src, const BlockMap bm, int dir, int parity,
+                                                                int box0, int nbox) {
   const long long i = (long long)blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x;
   if (i >= bm.nat.ns) return;
   long long is = i, id = i;
+  bool zero = false;
   if (dir != 0) {
     const int box = (int)(i / bm.blk.vh), lcb = (int)(i % bm.blk.vh);
     const long long n = block_to_natural(bm, box, lcb, parity);
     if (dir == 1) { is = n; id = i; } else { is = i; id = n; }
+    zero = dir == 2 && nbox > 0 && (box < box0 || box >= box0 + nbox);     // outside the active box range (one colour)
   }
-  typename PA::real va[24];
-  load_site<PA, 24>(va, src, bm.nat.ns, is);
   typename PB::real vb[24];
+  if (zero) {
 #pragma unroll
-  for (int k = 0; k < 24; ++k) vb[k] = (typename PB::real)va[k];
+    for (int k = 0; k < 24; ++k) vb[k] = 0;
+  } else {
+    typename PA::real va[24];
+    load_site<PA, 24>(va, src, bm.nat.ns, is);
+#pragma unroll
+    for (int k = 0; k < 24; ++k) vb[k] = (typename PB::real)va[k];
+  }
   store_site<PB, 24>(vb, dst, bm.nat.ns, id);
 }
 
@@ -169,22 +177,22 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, cons
 }
 
 template <class PA>
-static cudaError_t convert_b(int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s) {
+static cudaError_t convert_b(int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s, int box0, int nbox) {
   dim3 grid((unsigned)((bm.nat.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK)), block(LQ_BLAS_BLOCK);
   switch (pb) {
-    case 0: convert_kernel<PA, PrecD><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
-    case 1: convert_kernel<PA, PrecS><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
-    case 2: convert_kernel<PA, PrecH><<<grid, block, 0, s>>>(dst, src, bm, dir, parity); break;
+    case 0: convert_kernel<PA, PrecD><<<grid, block, 0, s>>>(dst, src, bm, dir, parity, box0, nbox); break;
+    case 1: convert_kernel<PA, PrecS><<<grid, block, 0, s>>>(dst, src, bm, dir, parity, box0, nbox); break;
+    case 2: convert_kernel<PA, PrecH><<<grid, block, 0, s>>>(dst, src, bm, dir, parity, box0, nbox); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();
 }
 
-cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s) {
+cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s, int box0, int nbox) {
   switch (pa) {
-    case 0: return convert_b<PrecD>(pb, dst, src, bm, dir, parity, s);
-    case 1: return convert_b<PrecS>(pb, dst, src, bm, dir, parity, s);
-    case 2: return convert_b<PrecH>(pb, dst, src, bm, dir, parity, s);
+    case 0: return convert_b<PrecD>(pb, dst, src, bm, dir, parity, s, box0, nbox);
+    case 1: return convert_b<PrecS>(pb, dst, src, bm, dir, parity, s, box0, nbox);
+    case 2: return convert_b<PrecH>(pb, dst, src, bm, dir, parity, s, box0, nbox);
   }
   return cudaErrorInvalidValue;
 }

@@ -18,18 +18,38 @@ namespace lq {
 // (Dirichlet) boundaries; box b = bx + nbd0*(by + nbd1*(bz + nbd2*bt)) occupies the contiguous
 // index range [b*blk.vh, (b+1)*blk.vh) of every block-major field.  Block extents are even,
 // so the parity of a site inside its box equals its global parity.
+// cmaj != 0 (multiplicative Schwarz): the boxes are stored colour-major, colour = (bx+by+bz+bt) & 1 --
+// the nb/2 boxes of colour 0 first, then those of colour 1 -- so that one colour is a contiguous box range
+// (needs an even number of boxes in x: position q of colour c has bx = 2 (q % (nbd0/2)) + ((by+bz+bt+c) & 1),
+// the checkerboard trick of the site index one level up).
 struct BlockMap {
   Geom nat;     // whole lattice, nb = 1
   Geom blk;     // one box, nb = number of boxes, ns = nat.ns
   int nbd[4];
+  int cmaj;
 };
 
 LQ_DEV long long block_to_natural(const BlockMap& bm, int box, int lcb, int parity) {
   int lc[4];
   cb_to_coords(bm.blk, lcb, parity, lc);
-  int b = box, gc[4];
+  int bc[4];
+  if (bm.cmaj) {
+    const int half = bm.blk.nb >> 1, col = box >= half ? 1 : 0;
+    int q = box - col * half;
+    const int h0 = bm.nbd[0] >> 1;
+    const int bxh = q % h0; q /= h0;
+    bc[1] = q % bm.nbd[1]; q /= bm.nbd[1];
+    bc[2] = q % bm.nbd[2];
+    bc[3] = q / bm.nbd[2];
+    bc[0] = 2 * bxh + ((bc[1] + bc[2] + bc[3] + col) & 1);
+  } else {
+    int b = box;
 #pragma unroll
-  for (int m = 0; m < 4; ++m) { gc[m] = (b % bm.nbd[m]) * bm.blk.X[m] + lc[m]; b /= bm.nbd[m]; }
+    for (int m = 0; m < 4; ++m) { bc[m] = b % bm.nbd[m]; b /= bm.nbd[m]; }
+  }
+  int gc[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) gc[m] = bc[m] * bm.blk.X[m] + lc[m];
   return coords_to_cb(bm.nat, gc);
 }
 
@@ -42,7 +62,8 @@ struct MultiArgs {
 
 cudaError_t run_gcr_dots(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
 cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
-cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s);
+cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s,
+                        int box0 = 0, int nbox = 0);   // dir 2, nbox > 0: sites of boxes outside [box0, box0 + nbox) are written as zero
 cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStream_t s);
 
 // setup kernels (pack.cu, clover.cu)

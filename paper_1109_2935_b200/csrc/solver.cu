@@ -68,8 +68,8 @@ int read_S(lqcd_ctx* c, int off, int n, cudaStream_t s) {
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "scalar read-back", e);
 }
 
-int convert(lqcd_ctx* c, int pa, int pb, char* dst, const char* src, int dir, int parity, cudaStream_t s) {
-  cudaError_t e = run_convert(pa, pb, dst, src, c->bm, dir, parity, s);
+int convert(lqcd_ctx* c, int pa, int pb, char* dst, const char* src, int dir, int parity, cudaStream_t s, int box0 = 0, int nbox = 0) {
+  cudaError_t e = run_convert(pa, pb, dst, src, c->bm, dir, parity, s, box0, nbox);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "convert", e);
 }
@@ -148,6 +148,45 @@ int schwarz_apply(lqcd_ctx* c, char* out, const char* in, int parity, double kap
     }
   }
   return convert(c, prec, prec_io, out, xk, 2, parity, s);
+}
+
+// out = K_sap in: multiplicative Schwarz (SAP; PAPER.md:158 section 4, :146; reading R16).  n_cycle cycles over the two
+// block colours; the blocks of one colour are a contiguous box range of the colour-major block layout (host.h), so a
+// half-step is the additive machinery launched on that range; after it the residual is updated with the FULL operator:
+//   rho = r restricted to colour c;  y = MR^{n_mr}(Mhat_D) rho;  out += y;  r -= Mhat y.
+// in / out / r / y / t: natural layout, precision prec_io; rho, w, xk: block-major, precision prec.
+int schwarz_sap_apply(lqcd_ctx* c, char* out, const char* in, int parity, double kappa, int n_mr, double omega, int n_cycle,
+                      int prec, int recon, int prec_io, int recon_io, char* rho, char* w, char* xk, char* r, char* y, char* t,
+                      cudaStream_t s) {
+  Range nv("lqcd: multiplicative Schwarz K_sap");
+  if (!c->bm.cmaj) return fail(c, LQCD_ESTATE, "multiplicative Schwarz needs the colour-major block layout");
+  const int nb = c->bm.blk.nb, half = nb / 2;
+  int rc = convert(c, prec_io, prec_io, r, in, 0, parity, s);
+  if (rc) return rc;
+  { BlasArgs a = mk(c, false, out); if ((rc = blas<OpZero>(c, prec_io, a, s))) return rc; }
+  for (int cyc = 0; cyc < n_cycle; ++cyc)
+    for (int col = 0; col < 2; ++col) {
+      const int box0 = col * half, nbox = half;
+      // only this colour's boxes are computed below, so the other colour's part of rho need not be cleared
+      if ((rc = convert(c, prec_io, prec, rho, r, 1, parity, s))) return rc;
+      for (int step = 0; step < n_mr; ++step) {
+        if ((rc = op_matpc(c, w, rho, parity, 0, kappa, prec, recon, true, true, s, 0, 0, nullptr, box0, nbox))) return rc;
+        BlasArgs a = mk(c, true, xk, rho, w);
+        a.c[0] = omega; a.box0 = box0; a.nb = nbox;
+        const bool first = step == 0, last = step == n_mr - 1;
+        if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
+        else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
+        else if (last) rc = blas<OpMrLast>(c, prec, a, s);
+        else rc = blas<OpMrMid>(c, prec, a, s);
+        if (rc) return rc;
+      }
+      if ((rc = convert(c, prec, prec_io, y, xk, 2, parity, s, box0, nbox))) return rc;       // zero on the other colour
+      { BlasArgs a = mk(c, false, y, out); a.c[0] = 1.0; if ((rc = blas<OpAxpyNorm>(c, prec_io, a, s))) return rc; }
+      if (cyc == n_cycle - 1 && col == 1) break;                                             // the last residual is not needed
+      if ((rc = op_matpc(c, t, y, parity, 0, kappa, prec_io, recon_io, false, false, s))) return rc;
+      { BlasArgs a = mk(c, false, t, r); a.c[0] = -1.0; if ((rc = blas<OpAxpyNorm>(c, prec_io, a, s))) return rc; }
+    }
+  return LQCD_OK;
 }
 
 }  // namespace lq
@@ -501,11 +540,14 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
     if ((rc = wk.get(&ph[i], spinor_bytes(ps, ns)))) return rc;
     if ((rc = wk.get(&zh[i], spinor_bytes(ps, ns)))) return rc;
   }
+  const bool sap = p.precondition && p.schwarz_type == LQCD_SCHWARZ_MULTIPLICATIVE;
+  char *sr = nullptr, *sy = nullptr, *st = nullptr;
   if (p.precondition) {
     if (p.schwarz_group < 0) return fail(c, LQCD_EINVAL, "schwarz_group");
     c->schwarz_group = p.schwarz_group;
-    if ((rc = set_blocks(c, p.schwarz_block))) return rc;
+    if ((rc = set_blocks(c, p.schwarz_block, sap ? 1 : 0))) return rc;
     for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, ns)))) return rc;
+    if (sap) for (char** q : {&sr, &sy, &st}) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
   }
   double r0n;
   if ((rc = residual(c, r0, b, x, par, p.kappa, po, p.recon_outer, &r0n, s))) return rc;
@@ -519,7 +561,14 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
     int k = 0;
     while (true) {
       // p_k = K rhat
-      if (p.precondition) {
+      if (sap) {
+        const int ncyc = p.sap_cycles > 0 ? p.sap_cycles : 1;
+        if ((rc = schwarz_sap_apply(c, ph[k], rh, par, p.kappa, p.mr_steps, p.mr_omega, ncyc, pp, p.recon_precond, ps, p.recon_sloppy,
+                                    rho, w, xk, sr, sy, st, s))) return rc;
+        // each half-step runs the MR steps on half of the blocks: one cycle = mr_steps Mhat_D on the whole lattice
+        cnt.mat_precond += p.mr_steps * ncyc; cnt.mat_sloppy += 2 * ncyc - 1;
+        cnt.blas_flop_sites += ncyc * (p.mr_steps * (12.0 * 16 + 12.0 * 12) + 4 * 48.0);
+      } else if (p.precondition) {
         if ((rc = schwarz_apply(c, ph[k], rh, par, p.kappa, p.mr_steps, p.mr_omega, pp, p.recon_precond, ps, rho, w, xk, s))) return rc;
         cnt.mat_precond += p.mr_steps; cnt.blas_flop_sites += p.mr_steps * (12.0 * 16 + 12.0 * 12);
       } else if ((rc = convert(c, ps, ps, ph[k], rh, 0, par, s))) return rc;
@@ -741,6 +790,8 @@ int check_params(lqcd_ctx* c, const lqcd_invert_params* p) {
   if (p->solver != LQCD_SOLVER_BICGSTAB && p->solver != LQCD_SOLVER_GCR_DD && p->solver != LQCD_SOLVER_CGNR && p->solver != LQCD_SOLVER_CGNE) return fail(c, LQCD_EINVAL, "solver");
   if (!(p->tol > 0) || p->max_iter < 1) return fail(c, LQCD_EINVAL, "tol / max_iter");
   if (p->solver == LQCD_SOLVER_GCR_DD && p->precondition && p->mr_steps < 1) return fail(c, LQCD_EINVAL, "mr_steps");
+  if (p->schwarz_type != LQCD_SCHWARZ_ADDITIVE && p->schwarz_type != LQCD_SCHWARZ_MULTIPLICATIVE) return fail(c, LQCD_EINVAL, "schwarz_type");
+  if (p->sap_cycles < 0) return fail(c, LQCD_EINVAL, "sap_cycles");
   if (p->matpc_type != LQCD_MATPC_ASYMMETRIC && p->matpc_type != LQCD_MATPC_SYMMETRIC) return fail(c, LQCD_EINVAL, "matpc_type");
   if (p->matpc_type == LQCD_MATPC_SYMMETRIC && p->solver == LQCD_SOLVER_GCR_DD) return fail(c, LQCD_EINVAL, "symmetric form: BiCGstab, CGNR and CGNE only");
   return LQCD_OK;
@@ -765,6 +816,25 @@ int lqcd_schwarz(lqcd_ctx* c, void* out, const void* in, int parity, double kapp
   for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->nat.ns)))) return rc;
   rc = schwarz_apply(c, (char*)out, (const char*)in, parity, kappa, n_mr, omega_mr, prec, recon, prec_io, rho, w, xk, s);
   cudaStreamSynchronize(s);          // workspace is freed on return
+  return rc;
+}
+
+int lqcd_schwarz_sap(lqcd_ctx* c, void* out, const void* in, int parity, double kappa, const int block[4], int n_mr,
+                     double omega_mr, int n_cycle, int prec, int recon, int prec_io, int recon_io, void* stream) {
+  if (!c) return LQCD_EINVAL;
+  if (!out || !in || out == in || (parity | 1) != 1 || n_mr < 1 || n_cycle < 1 || prec < 0 || prec > 2 || prec_io < 0 || prec_io > 2)
+    return fail(c, LQCD_EINVAL, "schwarz_sap arguments");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = set_blocks(c, block, 1);
+  if (rc) return rc;
+  Work wk(c, s);
+  char *rho, *w, *xk, *r, *y, *t;
+  for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->nat.ns)))) return rc;
+  for (char** q : {&r, &y, &t}) if ((rc = wk.get(q, spinor_bytes(prec_io, c->nat.ns)))) return rc;
+  rc = schwarz_sap_apply(c, (char*)out, (const char*)in, parity, kappa, n_mr, omega_mr, n_cycle, prec, recon, prec_io, recon_io,
+                         rho, w, xk, r, y, t, s);
+  cudaStreamSynchronize(s);          // workspace is handed back on return
   return rc;
 }
 

@@ -19,13 +19,14 @@ PREC_DOUBLE, PREC_SINGLE, PREC_HALF = 0, 1, 2
 RECON_18, RECON_12, RECON_8 = 18, 12, 8
 SOLVER_BICGSTAB, SOLVER_GCR_DD, SOLVER_CGNR, SOLVER_CGNE = 0, 1, 2, 3
 MATPC_ASYMMETRIC, MATPC_SYMMETRIC = 0, 1
+SCHWARZ_ADDITIVE, SCHWARZ_MULTIPLICATIVE = 0, 1
 FIELD_SPINOR_PARITY, FIELD_STAGGERED_PARITY = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_release_workspace", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
     "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm", "lqcd_staggered_multishift",
 ]
@@ -40,7 +41,7 @@ class InvertParams(ctypes.Structure):
         ("parity", ctypes.c_int), ("gcr_kmax", ctypes.c_int), ("schwarz_block", ctypes.c_int * 4),
         ("mr_steps", ctypes.c_int), ("mr_omega", ctypes.c_double),
         ("use_initial_guess", ctypes.c_int), ("precondition", ctypes.c_int), ("matpc_type", ctypes.c_int),
-        ("schwarz_group", ctypes.c_int), ("history_len", ctypes.c_int),
+        ("schwarz_group", ctypes.c_int), ("schwarz_type", ctypes.c_int), ("sap_cycles", ctypes.c_int), ("history_len", ctypes.c_int),
         ("residual_history", ctypes.POINTER(ctypes.c_double)),
     ]
 
@@ -92,6 +93,7 @@ def load_library():
             "lqcd_matpc_mrhs": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_schwarz": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, vp]),
             "lqcd_set_schwarz_group": (i, [vp, i]),
+            "lqcd_schwarz_sap": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, i, i, vp]),
             "lqcd_invert": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_invert_mrhs": (i, [vp, vp, vp, i, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_apply_host": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
@@ -211,6 +213,11 @@ class Context:
         self._check(self.lib.lqcd_matpc_mrhs(self.h, _ptr(out), _ptr(inp), nrhs, parity, int(dagger), kappa, prec, recon, _stream()))
         return out
 
+    def schwarz_sap(self, out, inp, parity, kappa, block, n_mr, omega_mr, n_cycle, prec, recon, prec_io, recon_io):
+        self._check(self.lib.lqcd_schwarz_sap(self.h, _ptr(out), _ptr(inp), parity, kappa, _i4(block), n_mr, omega_mr, n_cycle,
+                                              prec, recon, prec_io, recon_io, _stream()))
+        return out
+
     def set_schwarz_group(self, blocks_per_group):
         self._check(self.lib.lqcd_set_schwarz_group(self.h, int(blocks_per_group)))
 
@@ -274,7 +281,7 @@ class Context:
     def make_params(kappa, c_sw, tol, solver=SOLVER_BICGSTAB, prec=(PREC_DOUBLE, PREC_SINGLE, PREC_HALF),
                     recon=(RECON_18, RECON_12, RECON_12), delta=0.1, max_iter=5000, parity=0, gcr_kmax=16,
                     schwarz_block=(0, 0, 0, 0), mr_steps=10, mr_omega=1.0, use_initial_guess=False, precondition=True,
-                    matpc_type=MATPC_ASYMMETRIC, schwarz_group=0, history_len=0):
+                    matpc_type=MATPC_ASYMMETRIC, schwarz_group=0, history_len=0, schwarz_type=0, sap_cycles=1):
         p = InvertParams()
         p.kappa, p.c_sw, p.tol, p.delta = kappa, c_sw, tol, delta
         p.max_iter, p.solver = max_iter, solver
@@ -287,6 +294,7 @@ class Context:
         p.use_initial_guess, p.precondition = int(use_initial_guess), int(precondition)
         p.matpc_type = int(matpc_type)
         p.schwarz_group = int(schwarz_group)
+        p.schwarz_type, p.sap_cycles = int(schwarz_type), int(sap_cycles)
         if history_len > 0:                       # host buffer owned by the params object
             p._history = (ctypes.c_double * int(history_len))()
             p.history_len = int(history_len)

@@ -379,3 +379,48 @@ def test_schwarz_block_groups_and_residual_history(mid):
         assert 0.1 < h[0] < 3.0 and min(h) <= 1.2e-10
     with pytest.raises(lq.LqcdError):
         c.ctx.set_schwarz_group(-1)
+
+
+def test_multiplicative_schwarz_sap(mid):
+    """Multiplicative Schwarz (SAP; R16) against the oracle: K_sap in every
+    precision (1 and 2 cycles), support on the solve parity, and GCR preconditioned by it (fp64 / mixed) against the
+    oracle's solution and, in fp64, its outer-iteration count; the additive preconditioner still works on the
+    colour-major block layout SAP leaves behind."""
+    c = mid
+    lq = c.lqcd
+    kappa, blk = 0.124, (4, 4, 4, 8)
+    r = inputs.gaussian_spinor(c.dims, 7)
+    d = torch.from_numpy(r).cuda()
+    for prec, tol in ((0, 1e-11), (1, 5e-5), (2, 2e-2)):
+        for parity in (0, 1):
+            for ncyc in (1, 2):
+                want = oracle.schwarz_sap(r, c.U, c.T, c.bc, kappa, parity, blk, n_mr=4, n_cycle=ncyc)
+                fin, out = c.ctx.pack_spinor(d, parity, prec), c.ctx.new_field(prec)
+                c.ctx.schwarz_sap(out, fin, parity, kappa, blk, 4, 1.0, ncyc, prec, 12, prec, 12)
+                got = torch.zeros_like(d)
+                c.ctx.unpack_spinor(got, out, parity, prec)
+                g = got.cpu().numpy()
+                assert np.max(np.abs(g[c.par != parity])) == 0.0
+                assert _rel(g, want) <= tol, (prec, parity, ncyc)
+    # additive K on the colour-major layout
+    want = oracle.schwarz(r, c.U, c.T, c.bc, kappa, 0, blk, n_mr=4)
+    out = c.ctx.new_field(0)
+    c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 0), 0, kappa, blk, 4, 1.0, 0, 18, 0)
+    got = torch.zeros_like(d)
+    c.ctx.unpack_spinor(got, out, 0, 0)
+    assert _rel(got.cpu().numpy(), want) <= 1e-11
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    bhat = oracle.prepare_source(b, c.U, c.T, c.bc, kappa, 0)
+    xs, isap = oracle.gcr_sap_pc(bhat, c.U, c.T, c.bc, kappa, 0, 1e-10 * np.linalg.norm(b), blk, n_mr=4, n_cycle=1)
+    for prec in ((0, 0, 0), (0, 1, 2), (0, 2, 2)):
+        p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, prec=prec, recon=(18, 12, 12), schwarz_block=blk,
+                              mr_steps=4, schwarz_type=lq.SCHWARZ_MULTIPLICATIVE, sap_cycles=1)
+        x, info = _solve(c, b, p)
+        assert info["status"] == 0 and info["true_residual"] <= 1e-10 and _rel(x, xo) <= 1e-8
+        if prec == (0, 0, 0):
+            assert abs(info["iterations"] - isap["iterations"]) <= 1
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, schwarz_block=(8, 4, 4, 8), schwarz_type=lq.SCHWARZ_MULTIPLICATIVE)
+    with pytest.raises(lq.LqcdError) as e:                        # one block in x: no two-colouring
+        _solve(c, b, p)
+    assert e.value.code == lq.EINVAL
