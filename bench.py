@@ -278,7 +278,8 @@ def main():
     ap.add_argument("--no-config5", action="store_true", help="skip config 5 (48^3x96 GCR-DD vs BiCGstab, ~20 s)")
     ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
-    ap.add_argument("--op", default="dslash", choices=["dslash", "staggered"],
+    ap.add_argument("--schwarz-group", type=int, default=0, help="--op schwarz: blocks per launch group (0 = all)")
+    ap.add_argument("--op", default="dslash", choices=["dslash", "staggered", "schwarz"],
                     help="dslash: the BASELINE metric (Wilson-clover Dslash); staggered: the improved staggered Dslash (SURVEY NEXT-3)")
     ap.add_argument("--long12", action="store_true", help="--op staggered: long links declared c3 x SU(3) and stored as 12 reals")
     ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"], help="storage precision of the timed Dslash")
@@ -301,6 +302,9 @@ def main():
         args.quick, args.solvers_only, args.full, args.no_config5 = True, False, False, True
     if args.op == "staggered":
         run_staggered(args, rank, world, local)
+        return
+    if args.op == "schwarz":
+        run_schwarz(args, rank, world, local)
         return
 
     import torch
@@ -361,7 +365,9 @@ def main():
     ms = max_over_ranks(ms, dev)
 
     # ---- e2e: host buffers through lqcd_apply_host -----------------------------------------------
-    h_in = psi.cpu().pin_memory()
+    # canonical host arrays: complex64 for fp32 / half compute (lqcd_apply_host_c64; the path is PCIe-bound and the
+    # storage holds no more digits), complex128 for fp64
+    h_in = (psi.cpu() if prec == lqcd.PREC_DOUBLE else psi.to(torch.complex64).cpu()).pin_memory()
     h_out = torch.empty_like(h_in).pin_memory()
     e2e_steps = max(3, min(args.steps, 5))
     ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon)
@@ -369,7 +375,7 @@ def main():
     e2e_ms = time_region(lambda: ctx.apply_host(h_out, h_in, 0, 0, False, KAPPA, prec, recon), e2e_steps)
     e2e_ms = max_over_ranks(e2e_ms, dev)
     clocks = sampler.stop() if rank == 0 else None
-    cbytes = V * 12 * 16
+    cbytes = V * 12 * (16 if prec == lqcd.PREC_DOUBLE else 8)
 
     ms_step = ms / args.steps
     value = whole_job_gflops(FLOP_DSLASH * V * nrhs, world, ms_step)
@@ -391,7 +397,8 @@ def main():
                      "frac_of_8TBs_nominal": achieved / 8000.0,
                      "traffic_source": "profiles/r1_dslash_%s_r%d.md" % (args.prec, recon) if (args.prec, recon) in NCU_TRAFFIC else None},
         "e2e": {"value": whole_job_gflops(FLOP_DSLASH * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
-                "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps},
+                "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps,
+                "host_dtype": "complex128" if prec == lqcd.PREC_DOUBLE else "complex64"},
         "gpu_launches": launches,
         "clocks": clocks,
     }
@@ -456,6 +463,45 @@ def summarize(ex):
     sm["cfg4"] = {"%s_%s%s" % (r["solver"], r.get("sloppy"), ("_" + str(r["precond"])) if r.get("precond") else ""): srow(r) for r in ex.get("solvers", [])}
     sm["cfg5"] = {"%s_%s%s" % (r["solver"], r.get("sloppy"), ("_" + str(r["precond"])) if r.get("precond") else ""): srow(r) for r in ex.get("config5", [])}
     return sm
+
+
+def run_schwarz(args, rank, world, local):
+    """The Schwarz preconditioner K alone at config 5 (48^3x96, 256 blocks of 12^3x24, 10 MR steps, half precision;
+    PAPER.md:250, :310): a step = one application of K.  Not the BASELINE metric; used for the block-group
+    measurements of SURVEY NEXT-1 (--schwarz-group) and their ncu captures."""
+    import torch
+    from paper_1109_2935_b200 import inputs, lqcd
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dims, blk, n_mr = (48, 48, 48, 96), (12, 12, 12, 24), 10
+    U = inputs.random_gauge_torch(dims, 0.2, 21 + rank, device=dev)
+    b = inputs.gaussian_spinor_torch(dims, 22 + rank, device=dev)
+    ctx = lqcd.Context(dims, BC, local)
+    ctx.load_gauge(U)
+    del U
+    ctx.build_clover(CSW)
+    ctx.set_schwarz_group(args.schwarz_group)
+    fin, out = ctx.pack_spinor(b, 0, 2), ctx.new_field(2)
+    step = lambda: ctx.schwarz(out, fin, 0, KAPPA, blk, n_mr, 1.0, 2, 12, 2)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    l0 = ctx.launch_count()
+    ms = time_region(step, args.steps) / args.steps
+    launches = (ctx.launch_count() - l0) // args.steps
+    Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
+    by = n_mr * (matpc_bytes(2, 12) + 7 * SPINOR_B[2])            # per site per K: 10 x (Mhat_D + ~7 vector passes)
+    pk, pk_kind = peaks()
+    if rank == 0:
+        print(json.dumps({"metric": "schwarz_preconditioner_ms", "value": ms, "unit": "ms", "n_gpus": 1, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "i16+f32", "data": "synthetic",
+                          "config": {"workload": "config 5 preconditioner: 48^3x96, 256 Schwarz blocks of 12^3x24, 10 MR steps, half", "schwarz_group": args.schwarz_group},
+                          "gpu_launches": launches,
+                          "roofline": {"bound": "hbm", "achieved": by * Vh / (ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                       "frac": by * Vh / (ms * 1e-3) / 1e9 / pk["hbm_gbs"], "traffic": None, "peak_kind": pk_kind,
+                                       "kernel": "10 x (dslash_kernel<half,12> x 2 + OpMrUpdate)", "algorithmic_bytes_per_launch": by * Vh},
+                          "e2e": None, "cpu_baseline": None}))
+    ctx.close()
 
 
 def run_staggered(args, rank, world, local):

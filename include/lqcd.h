@@ -272,6 +272,10 @@ int lqcd_staggered_multishift(lqcd_ctx* ctx, void* x_canonical, const void* b_ca
  * LQCD_ENOMEM, LQCD_ECUDA. */
 int lqcd_apply_host(lqcd_ctx* ctx, void* out_host, const void* in_host, int op, int parity, int dagger,
                     double kappa, int prec, int recon, void* stream);
+/* The same call with complex64 canonical HOST arrays (half the PCIe bytes; the path is PCIe-bound): for fp32 and
+ * half-precision compute only (prec == LQCD_PREC_DOUBLE -> LQCD_EINVAL), whose storage holds no more digits. */
+int lqcd_apply_host_c64(lqcd_ctx* ctx, void* out_host, const void* in_host, int op, int parity, int dagger,
+                        double kappa, int prec, int recon, void* stream);
 int lqcd_invert_host(lqcd_ctx* ctx, void* x_host, const void* b_host,
                      const lqcd_invert_params* params, lqcd_invert_result* result, void* stream);
 

@@ -71,7 +71,8 @@ cudaError_t run_pack_gauge(double* g64, const double* U_canonical, const Geom& n
 cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, cudaStream_t s,
                               unsigned* bad = nullptr);   // bad: device word, bit 0 = not SU(3), bit 1 = recon-8 singular (pack.cu)
 cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
-                            long long i0 = 0, long long i1 = -1);   // sites [i0, i1) of the parity field (default: all)
+                            long long i0 = 0, long long i1 = -1,    // sites [i0, i1) of the parity field (default: all)
+                            int canonical_single = 0);              // canonical array is complex64 (lqcd_apply_host_c64)
 cudaError_t run_clover_term(double* T72, const double* g64, const Geom& nat, double c_sw, cudaStream_t s);
 cudaError_t run_clover_make(int prec, char* A, char* Ainv, const double* T72, const BlockMap& bm, int blocked, double kappa, cudaStream_t s);
 cudaError_t run_clover_apply(int prec, char* out, const char* in, const char* clov, const Geom& g, int parity, cudaStream_t s);

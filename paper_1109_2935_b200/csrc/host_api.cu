@@ -42,17 +42,17 @@ int hpipe(lqcd_ctx* c) {
 }
 }  // namespace
 
-extern "C" {
-
-int lqcd_apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, int parity, int dagger, double kappa,
-                    int prec, int recon, void* stream) {
+// creal = bytes of one real of the canonical host arrays: 8 (complex128) or 4 (complex64)
+static int apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, int parity, int dagger, double kappa,
+                      int prec, int recon, void* stream, int creal) {
   if (!c) return LQCD_EINVAL;
   if (!out_host || !in_host || (op != 0 && op != 1) || (parity | 1) != 1 || prec < 0 || prec > 2 || recon_index(recon) < 0)
     return fail(c, LQCD_EINVAL, "apply_host arguments");
   if (!c->have_gauge || (op == 1 && !c->have_clover)) return fail(c, LQCD_ESTATE, "apply_host before load_gauge / build_clover");
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
-  const size_t cbytes = (size_t)c->V * 24 * sizeof(double), pbytes = spinor_bytes(prec, c->nat.ns);
+  const size_t cbytes = (size_t)c->V * 24 * creal, pbytes = spinor_bytes(prec, c->nat.ns);
+  const int c32 = creal == 4;
   int rc;
   if ((rc = hpipe(c))) return rc;
   void *can_in, *can_out, *pk[4];
@@ -84,7 +84,7 @@ int lqcd_apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, in
     const long long i0 = k * sl_sites, i1 = i0 + sl_sites;
     for (int p = 0; p < 2; ++p) {
       if (op == 1 && p != parity) continue;
-      e = run_pack_spinor(prec, op == 1 ? pout[0] : pout[p], (const double*)can_out, c->nat, p, 1, s, i0, i1); c->launches++;
+      e = run_pack_spinor(prec, op == 1 ? pout[0] : pout[p], (const double*)can_out, c->nat, p, 1, s, i0, i1, c32); c->launches++;
       if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "unpack", e);
     }
     if ((e = cudaEventRecord(c->hev_out[k], s)) != cudaSuccess || (e = cudaStreamWaitEvent(c->hs_out, c->hev_out[k], 0)) != cudaSuccess ||
@@ -97,7 +97,7 @@ int lqcd_apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, in
     const long long i0 = j * sl_sites, i1 = i0 + sl_sites;
     for (int p = 0; p < 2; ++p) {
       if (op == 1 && p != parity) continue;
-      e = run_pack_spinor(prec, op == 1 ? pin[0] : pin[p], (const double*)can_in, c->nat, p, 0, s, i0, i1); c->launches++;
+      e = run_pack_spinor(prec, op == 1 ? pin[0] : pin[p], (const double*)can_in, c->nat, p, 0, s, i0, i1, c32); c->launches++;
       if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "pack", e);
     }
     packed[j] = true;
@@ -128,6 +128,19 @@ int lqcd_apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, in
   LQ_CK(cudaStreamSynchronize(s), "apply_host");
 #undef LQ_CK
   return LQCD_OK;
+}
+
+extern "C" {
+
+int lqcd_apply_host(lqcd_ctx* c, void* out_host, const void* in_host, int op, int parity, int dagger, double kappa,
+                    int prec, int recon, void* stream) {
+  return apply_host(c, out_host, in_host, op, parity, dagger, kappa, prec, recon, stream, 8);
+}
+
+int lqcd_apply_host_c64(lqcd_ctx* c, void* out_host, const void* in_host, int op, int parity, int dagger, double kappa,
+                        int prec, int recon, void* stream) {
+  if (c && prec == 0) return fail(c, LQCD_EINVAL, "apply_host_c64: single-precision host arrays serve fp32 / half compute only");
+  return apply_host(c, out_host, in_host, op, parity, dagger, kappa, prec, recon, stream, 4);
 }
 
 int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const lqcd_invert_params* p, lqcd_invert_result* res, void* stream) {

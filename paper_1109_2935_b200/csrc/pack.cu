@@ -104,15 +104,16 @@ cudaError_t run_convert_gauge(int prec, int recon, char* dst, const double* g64,
   return cudaErrorInvalidValue;
 }
 
-// canonical psi[t][z][y][x][4][3] (complex128) <-> packed parity field of precision P
-template <class P>
-__global__ void pack_spinor_kernel(char* packed, double* canonical, const Geom g, int parity, int unpack, long long i0, long long i1) {
+// canonical psi[t][z][y][x][4][3] (complex128, or complex64 for the single-precision host entry point) <-> packed
+// parity field of precision P
+template <class P, typename C>
+__global__ void pack_spinor_kernel(char* packed, C* canonical, const Geom g, int parity, int unpack, long long i0, long long i1) {
   const long long i = i0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= i1) return;
   int c[4];
   cb_to_coords(g, (int)i, parity, c);
   const long long site = c[0] + (long long)g.X[0] * (c[1] + (long long)g.X[1] * (c[2] + (long long)g.X[2] * c[3]));
-  double* p = canonical + site * 24;
+  C* p = canonical + site * 24;
   typename P::real v[24];
   if (!unpack) {
 #pragma unroll
@@ -121,22 +122,27 @@ __global__ void pack_spinor_kernel(char* packed, double* canonical, const Geom g
   } else {
     load_site<P, 24>(v, packed, g.ns, i);
 #pragma unroll
-    for (int k = 0; k < 24; ++k) p[k] = (double)v[k];
+    for (int k = 0; k < 24; ++k) p[k] = (C)v[k];
   }
 }
 
-cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
-                            long long i0, long long i1) {
-  if (i1 < 0) i1 = nat.ns;
+template <typename C>
+static cudaError_t pack_spinor_c(int prec, char* packed, C* c, const Geom& nat, int parity, int unpack, cudaStream_t s, long long i0, long long i1) {
   dim3 grid((unsigned)((i1 - i0 + 127) / 128)), block(128);
-  double* c = const_cast<double*>(canonical);
   switch (prec) {
-    case 0: pack_spinor_kernel<PrecD><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
-    case 1: pack_spinor_kernel<PrecS><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
-    case 2: pack_spinor_kernel<PrecH><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
+    case 0: pack_spinor_kernel<PrecD, C><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
+    case 1: pack_spinor_kernel<PrecS, C><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
+    case 2: pack_spinor_kernel<PrecH, C><<<grid, block, 0, s>>>(packed, c, nat, parity, unpack, i0, i1); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();
+}
+
+cudaError_t run_pack_spinor(int prec, char* packed, const double* canonical, const Geom& nat, int parity, int unpack, cudaStream_t s,
+                            long long i0, long long i1, int canonical_single) {
+  if (i1 < 0) i1 = nat.ns;
+  if (canonical_single) return pack_spinor_c<float>(prec, packed, reinterpret_cast<float*>(const_cast<double*>(canonical)), nat, parity, unpack, s, i0, i1);
+  return pack_spinor_c<double>(prec, packed, const_cast<double*>(canonical), nat, parity, unpack, s, i0, i1);
 }
 
 }  // namespace lq

@@ -26,7 +26,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_release_workspace", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_apply_host_c64", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
     "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm", "lqcd_staggered_multishift",
 ]
@@ -97,6 +97,7 @@ def load_library():
             "lqcd_invert": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_invert_mrhs": (i, [vp, vp, vp, i, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_apply_host": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
+            "lqcd_apply_host_c64": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_invert_host": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_axpy_norm": (i, [vp, d, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_cdot": (i, [vp, vp, vp, i, ctypes.POINTER(d), vp]),
@@ -322,10 +323,11 @@ class Context:
         return [r[k].as_dict() for k in range(nrhs)]
 
     def apply_host(self, out_host, in_host, op, parity, dagger, kappa, prec, recon):
-        """out_host, in_host: canonical complex128 HOST tensors (pinned for full-speed copies)."""
-        assert not out_host.is_cuda and not in_host.is_cuda
-        self._check(self.lib.lqcd_apply_host(self.h, _ptr(out_host), _ptr(in_host), op, parity, int(dagger), kappa,
-                                             prec, recon, _stream()))
+        """out_host, in_host: canonical complex128 (or, for fp32 / half compute, complex64) HOST tensors (pinned for
+        full-speed copies); the dtype selects lqcd_apply_host / lqcd_apply_host_c64."""
+        assert not out_host.is_cuda and not in_host.is_cuda and out_host.dtype == in_host.dtype
+        fn = self.lib.lqcd_apply_host_c64 if in_host.dtype == torch.complex64 else self.lib.lqcd_apply_host
+        self._check(fn(self.h, _ptr(out_host), _ptr(in_host), op, parity, int(dagger), kappa, prec, recon, _stream()))
         return out_host
 
     def invert_host(self, x_host, b_host, params, allow_fail=False):

@@ -424,3 +424,33 @@ def test_multiplicative_schwarz_sap(mid):
     with pytest.raises(lq.LqcdError) as e:                        # one block in x: no two-colouring
         _solve(c, b, p)
     assert e.value.code == lq.EINVAL
+
+
+def test_apply_host_complex64_equals_device_path():
+    """lqcd_apply_host_c64: complex64 host arrays (half the PCIe bytes) for fp32 / half compute give bit for bit
+    what the device path gives on the same single-precision values; fp64 compute is refused."""
+    from paper_1109_2935_b200 import lqcd
+    c = Case((8, 4, 6, 8), 0.3)
+    kappa = 0.12
+    psi = inputs.gaussian_spinor(c.dims, 5)
+    h32 = torch.from_numpy(psi).to(torch.complex64).pin_memory()
+    d = h32.to(torch.complex128).cuda()
+    out32 = torch.empty_like(h32).pin_memory()
+    for prec in (1, 2):
+        for op, parity, dagger in ((0, 0, False), (0, 0, True), (1, 0, False), (1, 1, True)):
+            c.ctx.apply_host(out32, h32, op, parity, dagger, kappa, prec, 12)
+            ref = torch.zeros_like(d)
+            if op == 0:
+                for p in (0, 1):
+                    fo = c.ctx.new_field(prec)
+                    c.ctx.dslash(fo, c.ctx.pack_spinor(d, 1 - p, prec), p, dagger, prec, 12)
+                    c.ctx.unpack_spinor(ref, fo, p, prec)
+            else:
+                fo = c.ctx.new_field(prec)
+                c.ctx.matpc(fo, c.ctx.pack_spinor(d, parity, prec), parity, dagger, kappa, prec, 12)
+                c.ctx.unpack_spinor(ref, fo, parity, prec)
+            assert torch.equal(out32, ref.to(torch.complex64).cpu()), (prec, op, parity, dagger)
+    with pytest.raises(lqcd.LqcdError) as e:
+        c.ctx.apply_host(out32, h32, 0, 0, False, kappa, 0, 18)
+    assert e.value.code == lqcd.EINVAL
+    c.ctx.close()
