@@ -43,10 +43,11 @@ def matpc_bytes(prec, recon):
     return 5 * SPINOR_B[prec] + 16 * recon * LINK_B[prec] + 2 * CLOVER_B[prec]
 
 
-# ncu --set full captures of one launch at 32^3x64 (profiles/r1_dslash_*.md): DRAM bytes read + written,
-# and executed warp instructions (the half-precision kernels are issue-bound)
-NCU_TRAFFIC = {("fp32", 12): 593.75e6, ("half", 12): 301.72e6, ("staggered", "fp32"): 1238.6e6}
-NCU_WARP_INST = {("half", 12): 69.50e6}
+# ncu --set full captures of one launch at 32^3x64 (profiles/r2_dslash_*.md, commit named there): DRAM bytes read + written,
+# and executed warp instructions of the half-precision kernel (its math pipes are the second limiter)
+NCU_TRAFFIC = {("fp32", 12): 595.84e6, ("half", 12): 300.01e6, ("staggered", "fp32"): 1238.6e6}
+NCU_TRAFFIC_SRC = {("fp32", 12): "profiles/r2_dslash_fp32_r12.md", ("half", 12): "profiles/r2_dslash_half_r12_tile.md"}
+NCU_WARP_INST = {("half", 12): 47.62e6}
 N_SCHEDULERS = 148 * 4      # one warp instruction per scheduler per clock (B200: 148 SMs x 4 SMSPs)
 
 
@@ -395,7 +396,7 @@ def main():
                      "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC.get((args.prec, recon)) if nrhs == 1 else None, "peak_kind": pk_kind,
                      "kernel": ("dslash_kernel<%s,%d> (EPI_NONE)" if nrhs == 1 else "dslash_mrhs_kernel<%s,%d> (EPI_NONE)") % (args.prec, recon), "algorithmic_bytes_per_launch": algo_bytes,
                      "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "traffic_source": "profiles/r1_dslash_%s_r%d.md" % (args.prec, recon) if (args.prec, recon) in NCU_TRAFFIC else None},
+                     "traffic_source": NCU_TRAFFIC_SRC.get((args.prec, recon))},
         "e2e": {"value": whole_job_gflops(FLOP_DSLASH * V, world, e2e_ms / e2e_steps), "unit": "GFLOP/s",
                 "h2d_bytes_per_step": cbytes, "d2h_bytes_per_step": cbytes, "steps": e2e_steps,
                 "host_dtype": "complex128" if prec == lqcd.PREC_DOUBLE else "complex64"},
@@ -403,15 +404,16 @@ def main():
         "clocks": clocks,
     }
 
+    if nrhs == 1 and args.prec == "half" and recon != 8:
+        out["roofline"]["kernel"] = "dslash_tile_kernel<%d> (EPI_NONE; dslash_kernel<half,%d> where the tile form does not apply)" % (recon, recon)
     if (args.prec, recon) in NCU_WARP_INST and nrhs == 1:
-        # issue-bound kernel: executed warp instructions per launch (ncu) / time vs 1 per scheduler per clock
+        # second limiter of the half-precision kernel: the math pipes (executed warp instructions per launch from ncu over
+        # time, against 1 per scheduler per clock; FFMA2 and PRMT occupy their pipe for 2 cycles each)
         ips = NCU_WARP_INST[(args.prec, recon)] / (kern_ms * 1e-3) / 1e9
         ipeak = N_SCHEDULERS * pk["sm_max_mhz"] * 1e-3
-        out["roofline_hbm"] = out["roofline"]
-        out["roofline"] = {"bound": "alu", "achieved": ips, "peak": ipeak, "unit": "G warp-inst/s", "frac": ips / ipeak,
-                           "traffic": NCU_TRAFFIC.get((args.prec, recon)), "kernel": out["roofline_hbm"]["kernel"],
-                           "peak_kind": "148 SMs x 4 schedulers x 1 warp instruction/clk x sm_max_mhz (DESIGN.md 6.1)",
-                           "warp_instructions_per_launch": NCU_WARP_INST[(args.prec, recon)]}
+        out["roofline_issue"] = {"bound": "alu", "achieved": ips, "peak": ipeak, "unit": "G warp-inst/s", "frac": ips / ipeak,
+                                 "peak_kind": "148 SMs x 4 schedulers x 1 warp instruction/clk x sm_max_mhz (DESIGN.md 6.1)",
+                                 "warp_instructions_per_launch": NCU_WARP_INST[(args.prec, recon)]}
     if rank == 0 and args.solvers_only:
         out["extra"] = extras(ctx, psi, args, torch, lqcd, inputs, pk)
         out["cpu_baseline"] = None
