@@ -9,13 +9,17 @@
 //
 //   XPAY    : r = y + a*r           (CLOVX: y := A_x y first)       -> Mhat second half, source prep
 //   CLOVOUT : r = C_x r             (C = A^-1 of the output parity)  -> Mhat first half, reconstruction
-//   DOTS    : per-box partial sums of <r,y> and <r,r>               -> fused MR reductions
+//   DOTS 1  : per-box partial sums of <r,y> and <r,r>               -> fused MR reductions
+//   DOTS 2/3: global <r,y> / <q,r> and <r,r>, scalar update by the last CTA -> BiCGstab omega / alpha, CGNR alpha
+//             (BLAS-1 is "extremely bandwidth intensive", so the reduction-only passes are not paid twice)
 //
 // One thread per output site (PAPER.md:164, :200-202 K1): 8 neighbour spinors + 8 links are
 // loaded with 128-bit coalesced loads; the 8-fold reuse of each input spinor is served by L2
 // (126 MB on B200).  CUDA-core FMA only: 3x3 complex matvecs
 // are not a dense contraction.  Spin projection uses the rank-2 structure of (1 +- g_mu) in
-// the chiral basis: 12 reals per hop go through the SU(3) multiply instead of 24.
+// the chiral basis: 12 reals per hop go through the SU(3) multiply instead of 24.  fp32 arithmetic is written in
+// packed complex form (FFMA2 with broadcast / swap-negate operand modifiers, core.cuh f2): the kernels are bound by
+// register-file bandwidth before the FMA lanes.  dslash_tile.cuh holds the CTA-tile form with bulk-async staging.
 #pragma once
 #include "core.cuh"
 

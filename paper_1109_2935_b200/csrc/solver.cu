@@ -4,8 +4,10 @@
 //     Mhat_D, one alpha per block                      (reading R7)
 //   * CGNR / CGNE with reliable updates                 ("CG on the normal equations")
 //   * GCR-DD, Algorithm 1                               (reading R8)
-// The host loop only launches kernels; all Krylov scalars live on the device (blas_ops.cuh).
-// One scalar (||r||^2) is read back per iteration for the convergence / restart decision.
+//   * multiplicative Schwarz (SAP) as the alternative preconditioner (reading R16)
+// The host loop only launches kernels; all Krylov scalars live on the device (blas_ops.cuh), two of BiCGstab's
+// reductions ride in the operator's epilogue (dslash.cuh DOTS 2 / 3), and ||r||^2 reaches the host through zero-copy
+// pinned words one iteration behind the device (solve_bicgstab); CGNR / CGNE / GCR read it back per iteration.
 #include <cmath>
 #include <complex>
 #include <cstring>
