@@ -543,9 +543,12 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
     if ((rc = wk.get(&zh[i], spinor_bytes(ps, ns)))) return rc;
   }
   const bool sap = p.precondition && p.schwarz_type == LQCD_SCHWARZ_MULTIPLICATIVE;
+  // the solve's group size must not outlive it (lqcd_set_schwarz_group is the context-level setting)
+  struct GroupGuard { lqcd_ctx* c; int saved; bool armed; ~GroupGuard() { if (armed) c->schwarz_group = saved; } } group_guard{c, c->schwarz_group, false};
   char *sr = nullptr, *sy = nullptr, *st = nullptr;
   if (p.precondition) {
     if (p.schwarz_group < 0) return fail(c, LQCD_EINVAL, "schwarz_group");
+    group_guard.armed = true;
     c->schwarz_group = p.schwarz_group;
     if ((rc = set_blocks(c, p.schwarz_block, sap ? 1 : 0))) return rc;
     for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, ns)))) return rc;
