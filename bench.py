@@ -772,12 +772,13 @@ def config5(torch, lqcd, inputs, dev):
     # the paper's configuration (additive Schwarz, 10 MR steps) first, then the variants of SURVEY NEXT-1:
     # fewer MR steps, the L2-sized block-group schedule, multiplicative Schwarz (SAP)
     runs = [("bicgstab", lqcd.SOLVER_BICGSTAB, (0, 1, 1), None, {}), ("bicgstab", lqcd.SOLVER_BICGSTAB, (0, 2, 2), None, {}),
+            ("bicgstab_delta0.01", lqcd.SOLVER_BICGSTAB, (0, 2, 2), None, dict(delta=0.01)),
             ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 1, 2), B5, dict(mr_steps=10)), ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10)),
             ("gcr_dd_mr4", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=4)),
             ("gcr_dd_group5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10, schwarz_group=5)),
             ("gcr_sap_mr5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=5, schwarz_type=lqcd.SCHWARZ_MULTIPLICATIVE, sap_cycles=1))]
     for name, solver, prec, blk, extra_kw in runs:
-        kw = dict(gcr_kmax=16, schwarz_block=blk, **extra_kw) if blk else {}
+        kw = dict(gcr_kmax=16, schwarz_block=blk, **extra_kw) if blk else dict(extra_kw)
         p = ctx.make_params(KAPPA, CSW, 1e-10, solver=solver, prec=prec, recon=(18, 12, 12), **kw)
         ctx.invert(x, b, p, allow_fail=True)        # warm-up (allocations, gauge / clover copies)
         best = None
