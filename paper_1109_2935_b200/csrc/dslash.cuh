@@ -20,6 +20,8 @@
 // the chiral basis: 12 reals per hop go through the SU(3) multiply instead of 24.  fp32 arithmetic is written in
 // packed complex form (FFMA2 with broadcast / swap-negate operand modifiers, core.cuh f2): the kernels are bound by
 // register-file bandwidth before the FMA lanes.  dslash_tile.cuh holds the CTA-tile form with bulk-async staging.
+// Half / recon 12: the clover block and the xpay vector of the epilogue are cp.async'ed into the thread's own
+// bytes of the ring slots that hops 4..6 have drained (EpiSlot), so the epilogue starts from shared memory.
 #pragma once
 #include "core.cuh"
 
@@ -344,14 +346,75 @@ LQ_DEV void dots_finalize(double* S, const double* s, int fin) {
   }
 }
 
+// ---- epilogue operands staged through freed ring slots (half precision, recon-12, 4-stage ring) ----------------
+// The clover block (148 B) and the xpay vector (52 B) of a site are needed only after the 8 hops, and loading them
+// then exposes their latency (ncu: long_scoreboard 2.1 per issue in the second launch of Mhat).  From hop 4 on the
+// ring slot a thread has just read is not refilled (there is no hop 8), so its private pieces of that slot -- one
+// 16-byte and one 8-byte link piece, three 16-byte spinor pieces and the 4-byte norm -- take the epilogue's operands
+// instead, by cp.async like everything else: after hop 4 clover chunks 0-3, the first half of chunk 8 and the norm
+// (slot 0), after hop 5 chunks 4-7 and the second half of chunk 8 (slot 1), after hop 6 the xpay vector (slot 2).
+// Every piece is private to its thread, so no barrier is needed; results are bit-identical to the direct loads.
+#ifndef LQ_DSLASH_BLOCK
+#define LQ_DSLASH_BLOCK 128
+#endif
+#define LQ_DSLASH_BLOCK_V LQ_DSLASH_BLOCK
+template <int B> struct EpiSlot {
+  static constexpr int SLOT = B * 76;
+  LQ_DEV static char* p16(char* ring, int s, int j, int tid) {     // j = 0: link piece; 1..3: spinor pieces
+    return ring + s * SLOT + (j == 0 ? 0 : 24 * B + 16 * (j - 1) * B) + 16 * tid;
+  }
+  LQ_DEV static char* p8(char* ring, int s, int tid) { return ring + s * SLOT + 16 * B + 8 * tid; }
+  LQ_DEV static char* p4(char* ring, int s, int tid) { return ring + s * SLOT + 72 * B + 4 * tid; }
+};
+template <int PART, int B>
+LQ_DEV void epi_stage_clover(char* ring, int tid, const char* __restrict__ clov, long long ns, long long idx) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    cp_async<16>(EpiSlot<B>::p16(ring, PART, j, tid), clov + 16ll * (4 * PART + j) * ns + 16ll * idx);
+  cp_async<8>(EpiSlot<B>::p8(ring, PART, tid), clov + 16ll * 8 * ns + 16ll * idx + 8 * PART);
+  if (PART == 0) cp_async<4>(EpiSlot<B>::p4(ring, 0, tid), clov + 144ll * ns + 4ll * idx);
+}
+template <int B>
+LQ_DEV void epi_stage_y(char* ring, int tid, const char* __restrict__ y, long long ns, long long idx) {
+#pragma unroll
+  for (int j = 0; j < 3; ++j) cp_async<16>(EpiSlot<B>::p16(ring, 2, j + 1, tid), y + 16ll * j * ns + 16ll * idx);
+  cp_async<4>(EpiSlot<B>::p4(ring, 2, tid), y + 48ll * ns + 4ll * idx);
+}
+// the staged clover block as load_site_raw<PrecH, 72> returns it (integers as floats, scale apart)
+template <int B> LQ_DEV void epi_load_clover(float* __restrict__ cl, float& sc, char* ring, int tid) {
+  alignas(16) unsigned w[36];
+#pragma unroll
+  for (int k = 0; k < 8; ++k)
+    *reinterpret_cast<int4*>(w + 4 * k) = ld_shared(reinterpret_cast<const int4*>(EpiSlot<B>::p16(ring, k >> 2, k & 3, tid)));
+  *reinterpret_cast<int2*>(w + 32) = ld_shared(reinterpret_cast<const int2*>(EpiSlot<B>::p8(ring, 0, tid)));
+  *reinterpret_cast<int2*>(w + 34) = ld_shared(reinterpret_cast<const int2*>(EpiSlot<B>::p8(ring, 1, tid)));
+  sc = __int_as_float(ld_shared(reinterpret_cast<const int*>(EpiSlot<B>::p4(ring, 0, tid)))) * LQ_FIXED_INV;
+#pragma unroll
+  for (int k = 0; k < 36; ++k) fixed_pair(w[k], cl[2 * k], cl[2 * k + 1]);
+}
+// the staged xpay vector as load_site<PrecH, 24> returns it
+template <int B> LQ_DEV void epi_load_y(float* __restrict__ yv, char* ring, int tid) {
+  alignas(16) unsigned w[12];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    *reinterpret_cast<int4*>(w + 4 * k) = ld_shared(reinterpret_cast<const int4*>(EpiSlot<B>::p16(ring, 2, k + 1, tid)));
+  const float sc = __int_as_float(ld_shared(reinterpret_cast<const int*>(EpiSlot<B>::p4(ring, 2, tid)))) * LQ_FIXED_INV;
+#pragma unroll
+  for (int k = 0; k < 12; ++k) fixed_pair(w[k], yv[2 * k], yv[2 * k + 1]);
+#pragma unroll
+  for (int k = 0; k < 24; ++k) yv[k] *= sc;
+}
+
 // Fused epilogue of one site (shared by the single- and multi-right-hand-side kernels):
 //   XPAY: acc = [A] y + coef * acc (CLOVX: A = clover block of the site);  CLOVOUT: acc = C acc;
 //   XPAY && CLOVX && CLOVOUT: acc = y + coef * C acc (symmetric even-odd form);
 //   DOTS 1, 2: d0 + i d1 += <acc, y>, d2 += <acc, acc> for this site; DOTS 3: d0 + i d1 += <q, acc> (only with CLOVX).
-template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS>
+// STG_C / STG_Y: the clover block / the xpay vector were staged in the ring (EpiSlot above) instead of being loaded here.
+template <class P, bool XPAY, bool CLOVX, bool CLOVOUT, int DOTS, bool STG_C = false, bool STG_Y = false>
 LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __restrict__ y, const char* __restrict__ clov_y,
                             const char* __restrict__ clov_out, double coef_d, int p, long long ns, long long idx,
-                            typename P::real& d0, typename P::real& d1, typename P::real& d2) {
+                            typename P::real& d0, typename P::real& d1, typename P::real& d2,
+                            char* ring = nullptr, int tid = 0) {
   typedef typename P::real R;
   if constexpr (XPAY && CLOVX && CLOVOUT) {
     // symmetric even-odd form, second half: acc = y + coef * C acc
@@ -365,13 +428,15 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
   }
   if constexpr (XPAY) {
     R yv[24];
-    load_site<P, 24>(yv, y, ns, idx);
+    if constexpr (STG_Y) epi_load_y<LQ_DSLASH_BLOCK_V>(yv, ring, tid);
+    else load_site<P, 24>(yv, y, ns, idx);
     const R coef = (R)coef_d;
     if constexpr (CLOVX) {
       // r = A y + coef * acc, one chiral block at a time so that y, A y and the clover block
       // die early (the DOTS variant needs y for the partial sums as well)
       R cl[72], sc;
-      load_site_raw<P, 72>(cl, sc, clov_y + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+      if constexpr (STG_C) epi_load_clover<LQ_DSLASH_BLOCK_V>(cl, sc, ring, tid);
+      else load_site_raw<P, 72>(cl, sc, clov_y + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
 #pragma unroll
       for (int ch = 0; ch < 2; ++ch) {
         R ay[12];
@@ -412,7 +477,15 @@ LQ_DEV void dslash_epilogue(typename P::real* __restrict__ acc, const char* __re
   }
   if constexpr (CLOVOUT) {
     R t[24];
-    clover_site<P>(t, acc, clov_out + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+    if constexpr (STG_C) {
+      R cl[72], sc;
+      epi_load_clover<LQ_DSLASH_BLOCK_V>(cl, sc, ring, tid);
+      clover_mul<R>(t, acc, cl);
+#pragma unroll
+      for (int k = 0; k < 24; ++k) t[k] *= sc;
+    } else {
+      clover_site<P>(t, acc, clov_out + (long long)p * site_bytes<P>(72, true) * ns, ns, idx);
+    }
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = t[k];
   }
@@ -464,6 +537,13 @@ __global__ void __launch_bounds__(LQ_DSLASH_BLOCK, (dslash_minb<P, RECON, CLOVX,
 dslash_kernel(const DslashArgs a) {
   static_assert(P::HALF ? (DAG == 0 || DAG == 1) : DAG == -1, "compile-time dagger for half precision only");
   typedef typename P::real R;
+  // epilogue operands through the ring (EpiSlot): half precision, recon-12 (16 + 8 byte link pieces), 4-stage ring
+#ifdef LQ_NO_EPI_STAGE
+  constexpr bool STG_OK = false;
+#else
+  constexpr bool STG_OK = P::HALF && RECON == 12 && NST == 4 && !(XPAY && CLOVX && CLOVOUT);
+#endif
+  constexpr bool STG_C = STG_OK && (CLOVX != CLOVOUT), STG_Y = STG_OK && XPAY;
   const Geom& g = a.g;
   const int cb = (DOTS ? 0 : a.range.cb0) + blockIdx.x * LQ_DSLASH_BLOCK + threadIdx.x;
   const int box = blockIdx.y + (a.parity >> 8);            // first box of the launch: Schwarz block groups (solver.cu)
@@ -527,6 +607,8 @@ dslash_kernel(const DslashArgs a) {
       extern __shared__ __align__(16) char lq_stage[];
       typedef HopStage<P, RECON> HS;
       const int tid = threadIdx.x;
+      const char* epi_clov = (CLOVX ? a.clov_y : a.clov_out) + (long long)p * site_bytes<P>(72, true) * g.ns;
+      (void)epi_clov;
       // hop h: mu = h/2, forward for even h.  Issue = start the async copies of its link and spinor.
 #define LQ_ISSUE(H)                                                                                        \
       {                                                                                                    \
@@ -551,6 +633,12 @@ dslash_kernel(const DslashArgs a) {
         if constexpr (P::HALF) load_site_magic<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid); \
         else load_site_raw<P, 24, 2>(psi, ps, sb_ + LQ_DSLASH_BLOCK * HS::LINK_B, LQ_DSLASH_BLOCK, tid);   \
         if ((H) + NST < 8) LQ_ISSUE(((H) + NST) % 8)                                                       \
+        /* slots that are not refilled take the epilogue's operands (EpiSlot) */                           \
+        if constexpr (STG_C) {                                                                             \
+          if ((H) == 4) epi_stage_clover<0, LQ_DSLASH_BLOCK>(lq_stage, tid, epi_clov, g.ns, idx);           \
+          if ((H) == 5) epi_stage_clover<1, LQ_DSLASH_BLOCK>(lq_stage, tid, epi_clov, g.ns, idx);           \
+        }                                                                                                  \
+        if constexpr (STG_Y) { if ((H) == 6) epi_stage_y<LQ_DSLASH_BLOCK>(lq_stage, tid, a.y, g.ns, idx); } \
         cp_async_commit();                                                                                 \
         const R sg_ = FW_ ? ((c[MU_] + 1 == g.X[MU_]) ? (R)g.bc[MU_] : R(1)) : ((c[MU_] == 0) ? (R)g.bc[MU_] : R(1)); \
         if constexpr (P::HALF) hop_fixed<MU_, FW_, (FW_ == (DAG == 1)) ? 1 : -1>(acc, psi, u, sg_ * us * ps); \
@@ -571,7 +659,14 @@ dslash_kernel(const DslashArgs a) {
 #undef LQ_ISSUE
     }
 
-    dslash_epilogue<P, XPAY, CLOVX, CLOVOUT, DOTS>(acc, a.y, a.clov_y, a.clov_out, a.a, p, g.ns, idx, d0, d1, d2);
+    if constexpr (STG_C || STG_Y) {
+      extern __shared__ __align__(16) char lq_stage[];
+      cp_async_wait<0>();
+      dslash_epilogue<P, XPAY, CLOVX, CLOVOUT, DOTS, STG_C, STG_Y>(acc, a.y, a.clov_y, a.clov_out, a.a, p, g.ns, idx, d0, d1, d2,
+                                                                     lq_stage, threadIdx.x);
+    } else {
+      dslash_epilogue<P, XPAY, CLOVX, CLOVOUT, DOTS>(acc, a.y, a.clov_y, a.clov_out, a.a, p, g.ns, idx, d0, d1, d2);
+    }
     store_site<P, 24>(acc, a.out, g.ns, idx);
   }
   if constexpr (DOTS >= 2) {
