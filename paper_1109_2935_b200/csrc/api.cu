@@ -173,7 +173,7 @@ static int get_dotws(lqcd_ctx* c, int nsite, double** out, cudaStream_t s) {
     if (rc) return rc;
     c->dotws_doubles = need;
     double hdr[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    memcpy(&hdr[0], &c->S, sizeof(double*));      // W[0] = address of the scalar array, W[1] = arrival counter = 0
+    memcpy(&hdr[0], &c->S, sizeof(double*));      // W[0] = address of the scalar array
     cudaError_t e = cudaMemcpyAsync(c->dotws, hdr, sizeof(hdr), cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dot workspace", e);
@@ -206,7 +206,6 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
   else if (epi == EPI_CLOVX_XPAY_YDOT || epi == EPI_CLOVX_XPAY_QDOT) {
     if (blocked || fin <= 0 || (epi == EPI_CLOVX_XPAY_QDOT && !q)) return fail(c, LQCD_EINVAL, "fused reduction arguments");
     if ((rc = get_dotws(c, d.g.vh, &d.dots, s))) return rc;
-    d.dagger = dagger | (fin << 16);
     if (epi == EPI_CLOVX_XPAY_QDOT) d.clov_out = q;            // the third vector travels in the unused A^-1 slot
   }
   else { d.range.cb0 = cb0; d.range.cb1 = cb1 < 0 ? d.g.vh : cb1; }
@@ -219,6 +218,11 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
   }
   c->launches++;
   if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dslash launch", e);
+  if (epi == EPI_CLOVX_XPAY_YDOT || epi == EPI_CLOVX_XPAY_QDOT) {
+    e = run_dots_finalize(d.dots, (d.g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK, fin, s);
+    c->launches++;
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "dots finalize launch", e);
+  }
   return LQCD_OK;
 }
 
@@ -226,7 +230,7 @@ int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_
 // sym != 0: the symmetric form Mhat_s = 1 - kappa^2 A^-1 D A^-1 D:  tmp = A^-1 D in ; out = in - kappa^2 A^-1 D tmp,
 // and Mhat_s^dag = 1 - kappa^2 D^dag A^-1 D^dag A^-1:  t0 = A^-1 in ; tmp = A^-1 D^dag t0 ; out = in - kappa^2 D^dag tmp.
 // fin != 0 (asymmetric form, natural layout only): the second launch also reduces <out,in>, ||out||^2 (q == nullptr) or
-// <q,out>, ||out||^2 over the field and its last CTA performs the scalar update `fin` (DotsFin, dslash.cuh)
+// <q,out>, ||out||^2 over the field and dots_finalize_kernel (blas.cu), launched behind it, performs the scalar update `fin` (DotsFin, dslash.cuh)
 int op_matpc(lqcd_ctx* c, char* out, const char* in, int parity, int dagger, double kappa, int prec, int recon,
              bool blocked, bool dots, cudaStream_t s, int sym, int fin, const char* q, int box0, int nbox) {
   char* tmp;

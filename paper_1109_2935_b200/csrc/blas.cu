@@ -218,4 +218,31 @@ cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStre
   return cudaErrorInvalidValue;
 }
 
+// Final sum of the per-CTA partials of a reduction fused into the operator (dslash.cuh, DOTS >= 2) and the scalar
+// update `fin`: one CTA, partials added in a fixed order (bit-reproducible).  W: workspace of get_dotws (api.cu).
+__global__ void __launch_bounds__(1024) dots_finalize_kernel(double* W, int n, int fin) {
+  __shared__ double sm[3 * 32];
+  const double* part = W + 8;
+  double s[3] = {0, 0, 0};
+  for (int i0 = threadIdx.x; i0 < n; i0 += 8 * 1024) {
+    double t[8][3];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int i = i0 + u * 1024;
+      const bool ok = i < n;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) t[u][k] = ok ? __ldcg(part + 3ll * i + k) : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { s[0] += t[u][0]; s[1] += t[u][1]; s[2] += t[u][2]; }
+  }
+  cta_reduce<3, 1024>(s, sm);
+  if (threadIdx.x == 0) dots_finalize(*reinterpret_cast<double**>(W), s, fin);
+}
+
+cudaError_t run_dots_finalize(double* W, int n, int fin, cudaStream_t s) {
+  dots_finalize_kernel<<<1, 1024, 0, s>>>(W, n, fin);
+  return cudaGetLastError();
+}
+
 }  // namespace lq

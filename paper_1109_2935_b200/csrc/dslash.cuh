@@ -10,7 +10,7 @@
 //   XPAY    : r = y + a*r           (CLOVX: y := A_x y first)       -> Mhat second half, source prep
 //   CLOVOUT : r = C_x r             (C = A^-1 of the output parity)  -> Mhat first half, reconstruction
 //   DOTS 1  : per-box partial sums of <r,y> and <r,r>               -> fused MR reductions
-//   DOTS 2/3: global <r,y> / <q,r> and <r,r>, scalar update by the last CTA -> BiCGstab omega / alpha, CGNR alpha
+//   DOTS 2/3: global <r,y> / <q,r> and <r,r>, scalar update by dots_finalize_kernel behind it -> BiCGstab omega / alpha, CGNR alpha
 //             (BLAS-1 is "extremely bandwidth intensive", so the reduction-only passes are not paid twice)
 //
 // One thread per output site (PAPER.md:164, :200-202 K1): 8 neighbour spinors + 8 links are
@@ -671,46 +671,17 @@ dslash_kernel(const DslashArgs a) {
   }
   if constexpr (DOTS >= 2) {
     // Solver reductions fused into the operator ("BLAS1 ... extremely bandwidth
-    // intensive"): CTA sums -> per-CTA partials -> the last CTA adds them in a fixed order (bit-reproducible) and
-    // updates the Krylov scalars on the device.  a.dots = workspace W: W[0] = address of the scalar array S,
-    // W[1] = arrival counter (self-resetting), W[8 + 3 i ..] = partials of CTA i.  a.dagger >> 16 selects the update.
+    // intensive"): CTA sums -> per-CTA partials; dots_finalize_kernel (blas.cu), launched behind this kernel, adds them
+    // in a fixed order (bit-reproducible) and updates the Krylov scalars on the device.  a.dots = workspace W:
+    // W[0] = address of the scalar array S, W[8 + 3 i ..] = partials of CTA i.  The CTA writes and leaves: a fence +
+    // arrival counter + last-CTA sum here (round 2's first form) kept every CTA resident ~1.5 us longer, which cost
+    // the fp32 solver 5 % (measured).
     __shared__ double sm[3 * (LQ_DSLASH_BLOCK / 32)];
-    __shared__ bool last;
     double red[3] = {(double)d0, (double)d1, (double)d2};
     cta_reduce<3, LQ_DSLASH_BLOCK>(red, sm);
-    double* W = a.dots;
-    double* part = W + 8;
-    unsigned* counter = reinterpret_cast<unsigned*>(W + 1);
     if (threadIdx.x == 0) {
-      part[3ll * blockIdx.x] = red[0]; part[3ll * blockIdx.x + 1] = red[1]; part[3ll * blockIdx.x + 2] = red[2];
-      __threadfence();
-      last = atomicAdd(counter, 1u) == gridDim.x - 1;
-    }
-    __syncthreads();
-    if (last) {
-      __threadfence();
-      // thousands of partials for one CTA: 8 independent loads in flight per thread (one L2 round trip per 1024
-      // partials instead of per 128), added in a fixed order
-      double s[3] = {0, 0, 0};
-      for (int i0 = threadIdx.x; i0 < (int)gridDim.x; i0 += 8 * LQ_DSLASH_BLOCK) {
-        double t[8][3];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int i = i0 + u * LQ_DSLASH_BLOCK;
-          const bool ok = i < (int)gridDim.x;
-#pragma unroll
-          for (int k = 0; k < 3; ++k) t[u][k] = ok ? __ldcg(part + 3ll * i + k) : 0.0;
-        }
-#pragma unroll
-        for (int u = 0; u < 8; ++u) { s[0] += t[u][0]; s[1] += t[u][1]; s[2] += t[u][2]; }
-      }
-      __syncthreads();
-      cta_reduce<3, LQ_DSLASH_BLOCK>(s, sm);
-      if (threadIdx.x == 0) {
-        double* S = *reinterpret_cast<double**>(W);
-        dots_finalize(S, s, a.dagger >> 16);
-        *counter = 0;
-      }
+      double* part = a.dots + 8 + 3ll * blockIdx.x;
+      part[0] = red[0]; part[1] = red[1]; part[2] = red[2];
     }
   }
   if constexpr (DOTS == 1) {
@@ -738,11 +709,11 @@ enum DslashEpi {
   EPI_XPAY_CLOVOUT = 4, // out = C (y + a D in)
   EPI_CLOVX_XPAY_DOTS = 5, // EPI_CLOVX_XPAY + per-box <out,y>, <out,out>
   EPI_XPAY_CLOVD = 6,      // out = y + a C (D in)   (symmetric even-odd form)
-  EPI_CLOVX_XPAY_YDOT = 7, // EPI_CLOVX_XPAY + global <out,y>, <out,out> and a scalar update by the last CTA
+  EPI_CLOVX_XPAY_YDOT = 7, // EPI_CLOVX_XPAY + global <out,y>, <out,out> and a scalar update (dots_finalize_kernel)
   EPI_CLOVX_XPAY_QDOT = 8  // EPI_CLOVX_XPAY + global <q,out>, <out,out> (q in DslashArgs::clov_out) and a scalar update
 };
 
-// scalar updates the fused reductions can perform (DslashArgs::dagger >> 16)
+// scalar updates the fused reductions can perform (argument of dots_finalize_kernel, blas.cu)
 enum DotsFin { FIN_NONE = 0, FIN_BICG_OMEGA = 1, FIN_BICG_ALPHA = 2, FIN_CG_ALPHA = 3 };
 
 template <class P> cudaError_t launch_dslash(const DslashArgs& a, int recon, int epi, cudaStream_t s);

@@ -65,6 +65,7 @@ cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_
 cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s,
                         int box0 = 0, int nbox = 0);   // dir 2, nbox > 0: sites of boxes outside [box0, box0 + nbox) are written as zero
 cudaError_t run_accumulate(int ph, int pl, char* y, const MultiArgs& m, cudaStream_t s);
+cudaError_t run_dots_finalize(double* W, int n, int fin, cudaStream_t s);
 
 // setup kernels (pack.cu, clover.cu)
 cudaError_t run_pack_gauge(double* g64, const double* U_canonical, const Geom& nat, cudaStream_t s);
