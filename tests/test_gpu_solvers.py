@@ -454,3 +454,24 @@ def test_apply_host_complex64_equals_device_path():
         c.ctx.apply_host(out32, h32, 0, 0, False, kappa, 0, 18)
     assert e.value.code == lqcd.EINVAL
     c.ctx.close()
+
+
+@pytest.mark.parametrize("solver", ["bicgstab", "cgnr"])
+def test_fused_reductions_are_bit_reproducible(mid, solver):
+    """SURVEY 8(a) a8 "deterministic reductions": the sums fused into M-hat's second launch (per-CTA partials, added
+    in a fixed order by dots_finalize_kernel) and the BLAS-1 sums give the same bits on every run — two identical
+    solves return bitwise identical x, iteration counts and residual histories, in every inner precision."""
+    c = mid
+    lq = c.lqcd
+    b = inputs.gaussian_spinor(c.dims, 5)
+    for sloppy in (0, 1, 2):
+        runs = []
+        for _ in range(2):
+            p = c.ctx.make_params(0.124, 1.0, 1e-10, solver=lq.SOLVER_BICGSTAB if solver == "bicgstab" else lq.SOLVER_CGNR,
+                                  prec=(0, sloppy, sloppy), recon=(18, 12, 12), history_len=4000)
+            x, info = _solve(c, b, p)
+            assert info["status"] == 0
+            runs.append((x, info["iterations"], list(info["residual_history"])))
+        assert runs[0][1] == runs[1][1]
+        assert runs[0][2] == runs[1][2]
+        assert np.array_equal(runs[0][0], runs[1][0])
