@@ -285,6 +285,18 @@ int lqcd_axpy_norm(lqcd_ctx* ctx, double a, const void* x, void* y, int prec, do
 /* <x,y> = sum conj(x) y -> dot_host[0..1] (re, im). */
 int lqcd_cdot(lqcd_ctx* ctx, const void* x, const void* y, int prec, double* dot_host, void* stream);
 
+/* <x,y> and ||y||^2 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (stream capture into a CUDA
+ * graph, serving loops, harnesses that forbid it).  Same sums as lqcd_cdot (the reductions of the
+ * Krylov solvers).  x, y: packed parity fields of precision prec (DEVICE).  out_device: 3 doubles in DEVICE memory
+ * owned by the caller, written on `stream`: re <x,y>, im <x,y>, ||y||^2; no copy to the host and no stream sync.
+ * The per-CTA partial sums live in a 768 KiB file-scope __device__ array of the library (held by every GPU that
+ * loads it until the process exits), which bounds the field: at most 2^23 = 8,388,608 sites per parity field, else
+ * LQCD_EINVAL with the limit in lqcd_last_error.  The call issues two kernel launches and no cudaMalloc / cudaFree /
+ * memcpy / event; the first call on a device also looks up the array's address (cudaGetSymbolAddress; make that call
+ * outside stream capture).  All calls on a device share the array: calls ordered on one stream are safe, calls that
+ * overlap on the GPU (two streams, two threads) race.  Sums are added in a fixed order (bit-reproducible). */
+int lqcd_cdot_static(lqcd_ctx* ctx, const void* x, const void* y, int prec, double* out_device, void* stream);
+
 /* number of kernel launches issued by this context since creation (bench: gpu_launches) */
 long long lqcd_launch_count(const lqcd_ctx* ctx);
 

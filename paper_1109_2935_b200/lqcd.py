@@ -27,7 +27,7 @@ EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_release_workspace", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
     "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_apply_host_c64", "lqcd_invert_host",
-    "lqcd_axpy_norm", "lqcd_cdot", "lqcd_launch_count",
+    "lqcd_axpy_norm", "lqcd_cdot", "lqcd_cdot_static", "lqcd_launch_count",
     "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm", "lqcd_staggered_multishift",
 ]
 
@@ -101,6 +101,7 @@ def load_library():
             "lqcd_invert_host": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_axpy_norm": (i, [vp, d, vp, vp, i, ctypes.POINTER(d), vp]),
             "lqcd_cdot": (i, [vp, vp, vp, i, ctypes.POINTER(d), vp]),
+            "lqcd_cdot_static": (i, [vp, vp, vp, i, vp, vp]),
             "lqcd_launch_count": (ctypes.c_longlong, [vp]),
             "lqcd_load_staggered_links": (i, [vp, vp, vp, d, vp]),
             "lqcd_pack_staggered": (i, [vp, vp, vp, i, i, vp]),
@@ -276,6 +277,12 @@ class Context:
         d = (ctypes.c_double * 2)()
         self._check(self.lib.lqcd_cdot(self.h, _ptr(x), _ptr(y), prec, d, _stream()))
         return complex(d[0], d[1])
+
+    def cdot_static(self, x, y, prec, out):
+        """lqcd_cdot_static: (re <x,y>, im <x,y>, ||y||^2) into the caller's CUDA float64 tensor `out` (3 elements);
+        nothing is allocated, copied or synchronised."""
+        assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 3 and out.is_contiguous()
+        self._check(self.lib.lqcd_cdot_static(self.h, _ptr(x), _ptr(y), prec, _ptr(out), _stream()))
 
     # -- solvers --------------------------------------------------------------------------------
     @staticmethod
