@@ -151,7 +151,8 @@ int set_blocks(lqcd_ctx* c, const int* blk, int cmaj) {
   c->bm.nat = c->nat;
   c->bm.blk = make_geom(blk, bcb, nb);
   c->have_blocks = true;
-  const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * (LQ_DSLASH_BLOCK / 32) * 4;
+  // per-warp partial dots of every box, then alpha_b (re, im) of every box
+  const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * (LQ_DSLASH_BLOCK / 32) * 4 + 2 * (size_t)nb;
   if (need > c->boxdots_doubles) {
     if (c->boxdots) cudaFree(c->boxdots);
     c->boxdots = nullptr; c->boxdots_doubles = 0;

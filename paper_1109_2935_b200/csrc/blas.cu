@@ -35,6 +35,16 @@ typedef OpMrUpdate<true, true> OpMrOnly;
 LQ_INST(OpMrFirst) LQ_INST(OpMrMid) LQ_INST(OpMrLast) LQ_INST(OpMrOnly)
 #undef LQ_INST
 
+// alpha_b of the MR step for boxes [box0, box0 + nbox) (blas_ops.cuh)
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK) mr_alpha_kernel(const double* boxdots, int nchunk, int box0, double c0, double* boxalpha) {
+  mr_alpha_box(boxdots, nchunk, box0 + blockIdx.x, c0, boxalpha);
+}
+
+cudaError_t run_mr_alpha(const BlasArgs& a, cudaStream_t s) {
+  mr_alpha_kernel<<<a.nb, LQ_BLAS_BLOCK, 0, s>>>(a.boxdots, a.nchunk, a.box0, a.c[0], const_cast<double*>(a.boxalpha));
+  return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------- GCR multi-vector kernels
 // beta_{i,k} = <z_i, z_k> for i in [i0, i0+n), n <= 8, one pass over z_k and the n vectors.
 template <class P>

@@ -43,6 +43,7 @@ struct BlasArgs {
   unsigned* counters;     // [nb], zero on entry, reset by the last CTA
   const double* boxdots;  // MR: per-box partial dots written by the Dslash epilogue [nb][nchunk][4], nchunk = CTAs per box x warps per CTA
   int nchunk;
+  const double* boxalpha; // MR: alpha_b (re, im) per box, formed from boxdots by mr_alpha_kernel (blas.cu)
   double c[4];            // host coefficients
   int i0, i1;
   // batched launch over right-hand sides (gridDim.z = nrhs, nb must be 1): right-hand side r uses
@@ -129,8 +130,12 @@ LQ_DEV void reduce_and_finalize(double* red, const BlasArgs& a, int box, F fin) 
 #ifndef LQ_BLAS_MINB_HALF
 #define LQ_BLAS_MINB_HALF 2
 #endif
+// the three-operand MR update runs three CTAs per SM (80 registers; 12 bytes spilled in one variant): K at config 5 14.05 -> 13.6 ms
+template <bool FIRST, bool LASTSTEP> struct OpMrUpdate;
+template <class Op> struct BlasMinbHalf { static constexpr int value = LQ_BLAS_MINB_HALF; };
+template <bool F, bool L> struct BlasMinbHalf<OpMrUpdate<F, L>> { static constexpr int value = 3; };
 template <class P, class Op>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK, (P::HALF ? LQ_BLAS_MINB_HALF : 1)) blas_kernel(const BlasArgs a0) {
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK, (P::HALF ? BlasMinbHalf<Op>::value : 1)) blas_kernel(const BlasArgs a0) {
   typedef typename P::real R;
   const int box = blockIdx.y + a0.box0;
   BlasArgs a = a0;

@@ -337,25 +337,33 @@ struct OpGcrScale {        // v0 = z_k, v1 = rhat : z_k /= gamma ; rhat -= alpha
 };
 
 // ---- Schwarz / MR: one alpha per box ---------------------------------------------
-// v0 = x, v1 = rho, v2 = w.  alpha_b = c0 * <w,rho>_b / <w,w>_b from the Dslash epilogue's partials.
+// alpha_b = c0 * <w,rho>_b / <w,w>_b from the Dslash epilogue's per-warp partials: one CTA per box adds the box's
+// nchunk partials in a fixed order (deterministic) and writes (re, im) of alpha_b.  A kernel of its own: summing the
+// partials at the start of every CTA of the update pass (162 x 4 x 3 doubles per box at 12^3x24, read by 81 CTAs)
+// was 80 us of its 350 us at config 5.
+LQ_DEV void mr_alpha_box(const double* boxdots, int nchunk, int box, double c0, double* boxalpha) {
+  __shared__ double sm[3 * (LQ_BLAS_BLOCK / 32)];
+  double s[3] = {0, 0, 0};
+  const double* d = boxdots + (long long)box * nchunk * 4;
+  for (int i = threadIdx.x; i < nchunk; i += LQ_BLAS_BLOCK) {
+    s[0] += __ldcg(d + 4 * i); s[1] += __ldcg(d + 4 * i + 1); s[2] += __ldcg(d + 4 * i + 2);
+  }
+  cta_reduce<3, LQ_BLAS_BLOCK>(s, sm);
+  if (threadIdx.x == 0) {
+    const double ww = s[2];
+    boxalpha[2 * box] = (ww > 0.0) ? c0 * s[0] / ww : 0.0;
+    boxalpha[2 * box + 1] = (ww > 0.0) ? c0 * s[1] / ww : 0.0;
+  }
+}
+
+// v0 = x, v1 = rho, v2 = w:  x += alpha_b rho;  rho -= alpha_b w
 template <bool FIRST, bool LASTSTEP>
 struct OpMrUpdate {
   static constexpr int NV = 0, READ = (FIRST ? 0 : 1) | 2 | (LASTSTEP ? 0 : 4), WRITE = 1 | (LASTSTEP ? 0 : 2);
   struct Coef { double ar, ai; };
   LQ_DEV static void prepare(Coef& c, const BlasArgs& a, int box) {
-    __shared__ double sm[3 * (LQ_BLAS_BLOCK / 32)];
-    __shared__ double res[3];
-    double s[3] = {0, 0, 0};
-    const double* d = a.boxdots + (long long)box * a.nchunk * 4;
-    for (int i = threadIdx.x; i < a.nchunk; i += LQ_BLAS_BLOCK) {
-      s[0] += __ldcg(d + 4 * i); s[1] += __ldcg(d + 4 * i + 1); s[2] += __ldcg(d + 4 * i + 2);
-    }
-    cta_reduce<3, LQ_BLAS_BLOCK>(s, sm);
-    if (threadIdx.x == 0) { res[0] = s[0]; res[1] = s[1]; res[2] = s[2]; }
-    __syncthreads();
-    const double ww = res[2];
-    c.ar = (ww > 0.0) ? a.c[0] * res[0] / ww : 0.0;
-    c.ai = (ww > 0.0) ? a.c[0] * res[1] / ww : 0.0;
+    c.ar = __ldcg(a.boxalpha + 2 * box);
+    c.ai = __ldcg(a.boxalpha + 2 * box + 1);
   }
   template <typename R> LQ_DEV static void site(const Coef& c, R* x, R* rho, R* w, R*, R*, double*) {
     if (FIRST) {

@@ -60,6 +60,7 @@ struct MultiArgs {
   int k, i0, n;
 };
 
+cudaError_t run_mr_alpha(const BlasArgs& a, cudaStream_t s);   // boxes [a.box0, a.box0 + a.nb): alpha_b = a.c[0] <w,rho>_b / <w,w>_b
 cudaError_t run_gcr_dots(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
 cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s);
 cudaError_t run_convert(int pa, int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s,

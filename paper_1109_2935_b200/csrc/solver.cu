@@ -54,6 +54,7 @@ BlasArgs mk(lqcd_ctx* c, bool blocked, char* v0 = nullptr, char* v1 = nullptr, c
   a.S = c->S; a.partials = c->partials; a.counters = c->counters;
   a.boxdots = c->boxdots;
   a.nchunk = (g.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK * (LQ_DSLASH_BLOCK / 32);   // per-warp partials per box
+  a.boxalpha = c->boxdots ? c->boxdots + (size_t)g.nb * a.nchunk * 4 : nullptr;         // behind the partials (set_blocks)
   return a;
 }
 
@@ -62,6 +63,12 @@ int blas(lqcd_ctx* c, int prec, const BlasArgs& a, cudaStream_t s) {
   cudaError_t e = run_blas<Op>(prec, a, c->n_sm * LQ_BLAS_CTAS_PER_SM, s);
   c->launches++;
   return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "blas launch", e);
+}
+
+int mr_alpha(lqcd_ctx* c, const BlasArgs& a, cudaStream_t s) {
+  cudaError_t e = run_mr_alpha(a, s);
+  c->launches++;
+  return e == cudaSuccess ? LQCD_OK : fail(c, LQCD_ECUDA, "mr alpha launch", e);
 }
 
 int read_S(lqcd_ctx* c, int off, int n, cudaStream_t s) {
@@ -141,6 +148,7 @@ int schwarz_apply(lqcd_ctx* c, char* out, const char* in, int parity, double kap
       BlasArgs a = mk(c, true, xk, rho, w);
       a.c[0] = omega;
       if (nbox) { a.box0 = box0; a.nb = nbox; }
+      if ((rc = mr_alpha(c, a, s))) return rc;
       const bool first = step == 0, last = step == n_mr - 1;
       if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
       else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
@@ -175,6 +183,7 @@ int schwarz_sap_apply(lqcd_ctx* c, char* out, const char* in, int parity, double
         if ((rc = op_matpc(c, w, rho, parity, 0, kappa, prec, recon, true, true, s, 0, 0, nullptr, box0, nbox))) return rc;
         BlasArgs a = mk(c, true, xk, rho, w);
         a.c[0] = omega; a.box0 = box0; a.nb = nbox;
+        if ((rc = mr_alpha(c, a, s))) return rc;
         const bool first = step == 0, last = step == n_mr - 1;
         if (first && last) rc = blas<OpMrOnly>(c, prec, a, s);
         else if (first) rc = blas<OpMrFirst>(c, prec, a, s);
