@@ -47,27 +47,26 @@ cudaError_t run_mr_alpha(const BlasArgs& a, cudaStream_t s) {
 
 // ---------------------------------------------------------------- GCR multi-vector kernels
 // beta_{i,k} = <z_i, z_k> for i in [i0, i0+n), n <= 8, one pass over z_k and the n vectors.
-template <class P>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_dots_kernel(const MultiArgs m) {
+// N = number of vectors of this pass at compile time: the loads of all N + 1 operands of a site are issued before the
+// first is used (with a run-time count the loop was load -> use -> load and ran at 3.3 TB/s)
+template <class P, int N>
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK, 2) gcr_dots_kernel(const MultiArgs m) {
   typedef typename P::real R;
   const BlasArgs& a = m.b;
   double red[16];
 #pragma unroll
   for (int k = 0; k < 16; ++k) red[k] = 0;
   for (int cb = blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x; cb < a.vh; cb += gridDim.x * LQ_BLAS_BLOCK) {
-    R zk[24];
+    R zk[24], zi[N][24];
     load_site<P, 24>(zk, m.z[m.k], a.ns, cb);
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (j < m.n) {
-        R zi[24];
-        load_site<P, 24>(zi, m.z[m.i0 + j], a.ns, cb);
-        site_cdot(zi, zk, red[2 * j], red[2 * j + 1]);
-      }
-    }
+    for (int j = 0; j < N; ++j) load_site<P, 24>(zi[j], m.z[m.i0 + j], a.ns, cb);
+#pragma unroll
+    for (int j = 0; j < N; ++j) site_cdot(zi[j], zk, red[2 * j], red[2 * j + 1]);
   }
   reduce_and_finalize<16>(red, a, 0, [&](const double* s) {
-    for (int j = 0; j < m.n; ++j) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
       double* b = a.S + S_GCR_BETA + 2 * ((m.i0 + j) * LQ_GCR_KMAX + m.k);
       b[0] = s[2 * j]; b[1] = s[2 * j + 1];
     }
@@ -109,17 +108,32 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_orth_kernel(const MultiArgs
   });
 }
 
+template <class P>
+static cudaError_t gcr_dots_n(const MultiArgs& m, dim3 grid, dim3 block, cudaStream_t s) {
+  switch (m.n) {
+    case 1: gcr_dots_kernel<P, 1><<<grid, block, 0, s>>>(m); break;
+    case 2: gcr_dots_kernel<P, 2><<<grid, block, 0, s>>>(m); break;
+    case 3: gcr_dots_kernel<P, 3><<<grid, block, 0, s>>>(m); break;
+    case 4: gcr_dots_kernel<P, 4><<<grid, block, 0, s>>>(m); break;
+    case 5: gcr_dots_kernel<P, 5><<<grid, block, 0, s>>>(m); break;
+    case 6: gcr_dots_kernel<P, 6><<<grid, block, 0, s>>>(m); break;
+    case 7: gcr_dots_kernel<P, 7><<<grid, block, 0, s>>>(m); break;
+    case 8: gcr_dots_kernel<P, 8><<<grid, block, 0, s>>>(m); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
 cudaError_t run_gcr_dots(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s) {
   int gx = (m.b.vh + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK;
   if (gx > max_ctas) gx = max_ctas;
   dim3 grid(gx), block(LQ_BLAS_BLOCK);
   switch (prec) {
-    case 0: gcr_dots_kernel<PrecD><<<grid, block, 0, s>>>(m); break;
-    case 1: gcr_dots_kernel<PrecS><<<grid, block, 0, s>>>(m); break;
-    case 2: gcr_dots_kernel<PrecH><<<grid, block, 0, s>>>(m); break;
-    default: return cudaErrorInvalidValue;
+    case 0: return gcr_dots_n<PrecD>(m, grid, block, s);
+    case 1: return gcr_dots_n<PrecS>(m, grid, block, s);
+    case 2: return gcr_dots_n<PrecH>(m, grid, block, s);
   }
-  return cudaGetLastError();
+  return cudaErrorInvalidValue;
 }
 
 cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_t s) {
