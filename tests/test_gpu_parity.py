@@ -248,8 +248,8 @@ def test_cfg3_full_size_all_precisions():
 def test_cfg5_full_size_operator_and_schwarz():
     """BASELINE.json config 5 at full size, 48^3x96 (10.6 M sites, eps = 0.2, kappa = 0.124, c_sw = 1):
     Dslash (fp32 and half, recon-12), Mhat (half) and the Schwarz preconditioner K with 256 blocks
-    of 12^3x24 and 10 MR steps in half precision, element by element against the oracle on the same
-    arrays.  K's tolerance is the one of DESIGN.md R7 / SURVEY 8(c).8 (error compounds over steps)."""
+    of 12^3x24 and 10 MR steps in half precision, and the multiplicative variant (SAP) on the same blocks, element by
+    element against the oracle on the same arrays.  K's tolerance is the one of DESIGN.md R7 / SURVEY 8(c).8 (error compounds over steps)."""
     from paper_1109_2935_b200 import lqcd
     dims, kappa, blk = (48, 48, 48, 96), 0.124, (12, 12, 12, 24)
     Ut = inputs.random_gauge_torch(dims, 0.2, 21, device="cuda")
@@ -290,6 +290,16 @@ def test_cfg5_full_size_operator_and_schwarz():
         assert float(torch.count_nonzero(got * ~even)) == 0
         err = float(torch.linalg.vector_norm(got - want_k) / torch.linalg.vector_norm(want_k))
         assert err <= tol, ("schwarz", n_mr, err)
+    # multiplicative Schwarz (SAP, R16) on the same 256 blocks in the colour-major block order: one cycle,
+    # 2 MR steps per half-step, half precision inside, fp32 outside
+    want_k = torch.from_numpy(oracle.schwarz_sap(psi, U, T, BC, kappa, 0, blk, n_mr=2, n_cycle=1)).cuda()
+    fk = ctx.new_field(1)
+    ctx.schwarz_sap(fk, ctx.pack_spinor(pt, 0, 1), 0, kappa, blk, 2, 1.0, 1, 2, 12, 1, 12)
+    got = torch.zeros_like(pt)
+    ctx.unpack_spinor(got, fk, 0, 1)
+    assert float(torch.count_nonzero(got * ~even)) == 0
+    err = float(torch.linalg.vector_norm(got - want_k) / torch.linalg.vector_norm(want_k))
+    assert err <= 1e-2, ("schwarz_sap", err)
     ctx.close()
 
 
