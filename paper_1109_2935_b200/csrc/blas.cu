@@ -76,18 +76,34 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK, 2) gcr_dots_kernel(const MultiA
 // z_k -= sum_{i<k} beta_{i,k} z_i ; then zz = ||z_k||^2, zr = <z_k, rhat> ;
 // last CTA: gamma_k = sqrt(zz), alpha_k = zr / gamma_k  (Algorithm 1)
 template <class P>
-__global__ void __launch_bounds__(LQ_BLAS_BLOCK) gcr_orth_kernel(const MultiArgs m) {
+__global__ void __launch_bounds__(LQ_BLAS_BLOCK, (sizeof(typename P::real) == 8 ? 1 : 2)) gcr_orth_kernel(const MultiArgs m) {
   typedef typename P::real R;
   const BlasArgs& a = m.b;
   double red[3] = {0, 0, 0};
+  // -beta_{i,k} in the arithmetic type, once per CTA (read from the device scalars inside the site loop they cost two
+  // dependent global loads and two conversions per vector and site)
+  __shared__ R nb[2 * LQ_GCR_KMAX];
+  if (threadIdx.x < m.k) {
+    const double* b = a.S + S_GCR_BETA + 2 * (threadIdx.x * LQ_GCR_KMAX + m.k);
+    nb[2 * threadIdx.x] = (R)(-b[0]); nb[2 * threadIdx.x + 1] = (R)(-b[1]);
+  }
+  __syncthreads();
+  constexpr int U = sizeof(R) == 8 ? 1 : 3;      // earlier directions whose loads are in flight together
   for (int cb = blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x; cb < a.vh; cb += gridDim.x * LQ_BLAS_BLOCK) {
     R zk[24], r[24];
     load_site<P, 24>(zk, m.z[m.k], a.ns, cb);
-    for (int i = 0; i < m.k; ++i) {
+    int i0 = 0;
+    for (; i0 + U <= m.k; i0 += U) {             // whole rounds: no predicates, so the U loads are issued back to back
+      R zi[U][24];
+#pragma unroll
+      for (int u = 0; u < U; ++u) load_site<P, 24>(zi[u], m.z[i0 + u], a.ns, cb);
+#pragma unroll
+      for (int u = 0; u < U; ++u) site_caxpy<R>(nb[2 * (i0 + u)], nb[2 * (i0 + u) + 1], zi[u], zk);
+    }
+    for (; i0 < m.k; ++i0) {
       R zi[24];
-      load_site<P, 24>(zi, m.z[i], a.ns, cb);
-      const double* b = a.S + S_GCR_BETA + 2 * (i * LQ_GCR_KMAX + m.k);
-      site_caxpy<R>((R)(-b[0]), (R)(-b[1]), zi, zk);
+      load_site<P, 24>(zi, m.z[i0], a.ns, cb);
+      site_caxpy<R>(nb[2 * i0], nb[2 * i0 + 1], zi, zk);
     }
     if (m.k > 0) store_site<P, 24>(zk, (char*)m.z[m.k], a.ns, cb);
     load_site<P, 24>(r, a.v[0], a.ns, cb);
