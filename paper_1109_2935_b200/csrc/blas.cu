@@ -202,9 +202,7 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, cons
   if (i >= m.b.ns) return;
   typename PH_::real acc[24];
   load_site<PH_, 24>(acc, y, m.b.ns, i);
-  for (int j = 0; j < m.n; ++j) {
-    typename PL_::real x[24];
-    load_site<PL_, 24>(x, m.z[j], m.b.ns, i);
+  auto add = [&](const typename PL_::real* x, int j) {
     const typename PH_::real cr = (typename PH_::real)m.chi[2 * j], ci = (typename PH_::real)m.chi[2 * j + 1];
 #pragma unroll
     for (int k = 0; k < 12; ++k) {
@@ -212,6 +210,21 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, cons
       acc[2 * k] += cr * xr - ci * xi;
       acc[2 * k + 1] += cr * xi + ci * xr;
     }
+  };
+  // whole rounds of U vectors without predicates, so that their loads are in flight together (same order of the sums)
+  constexpr int U = sizeof(typename PL_::real) == 8 ? 1 : 3;
+  int j = 0;
+  for (; j + U <= m.n; j += U) {
+    typename PL_::real x[U][24];
+#pragma unroll
+    for (int u = 0; u < U; ++u) load_site<PL_, 24>(x[u], m.z[j + u], m.b.ns, i);
+#pragma unroll
+    for (int u = 0; u < U; ++u) add(x[u], j + u);
+  }
+  for (; j < m.n; ++j) {
+    typename PL_::real x[24];
+    load_site<PL_, 24>(x, m.z[j], m.b.ns, i);
+    add(x, j);
   }
   store_site<PH_, 24>(acc, y, m.b.ns, i);
 }
