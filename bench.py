@@ -279,6 +279,7 @@ def main():
     ap.add_argument("--no-config5", action="store_true", help="skip config 5 (48^3x96 GCR-DD vs BiCGstab, ~20 s)")
     ap.add_argument("--quick", action="store_true", help="headline only: no sweep, no solvers, no cpu baseline")
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
+    ap.add_argument("--config5-only", action="store_true", help="headline + the config-5 solves only (for ncu launch lists of GCR-DD)")
     ap.add_argument("--schwarz-group", type=int, default=0, help="--op schwarz: blocks per launch group (0 = all)")
     ap.add_argument("--op", default="dslash", choices=["dslash", "staggered", "schwarz"],
                     help="dslash: the BASELINE metric (Wilson-clover Dslash); staggered: the improved staggered Dslash (SURVEY NEXT-3)")
@@ -300,7 +301,7 @@ def main():
     if world > 1:
         # replicas: every rank times the headline and the e2e leg; the sweep, the solvers and the CPU baseline
         # are rank-0-at-N=1 material and would leave the other ranks waiting in the process-group teardown
-        args.quick, args.solvers_only, args.full, args.no_config5 = True, False, False, True
+        args.quick, args.solvers_only, args.full, args.no_config5, args.config5_only = True, False, False, True, False
     if args.op == "staggered":
         run_staggered(args, rank, world, local)
         return
@@ -414,7 +415,7 @@ def main():
         out["roofline_issue"] = {"bound": "alu", "achieved": ips, "peak": ipeak, "unit": "G warp-inst/s", "frac": ips / ipeak,
                                  "peak_kind": "148 SMs x 4 schedulers x 1 warp instruction/clk x sm_max_mhz (DESIGN.md 6.1)",
                                  "warp_instructions_per_launch": NCU_WARP_INST[(args.prec, recon)]}
-    if rank == 0 and args.solvers_only:
+    if rank == 0 and (args.solvers_only or args.config5_only):
         out["extra"] = extras(ctx, psi, args, torch, lqcd, inputs, pk)
         out["cpu_baseline"] = None
     elif rank == 0 and not args.quick:
@@ -634,6 +635,10 @@ def extras(ctx, psi, args, torch, lqcd, inputs, pk):
     Vh = V // 2
     ex = {"sweep": [], "blas": [], "solvers": []}
     names = {0: "fp64", 1: "fp32", 2: "half"}
+    if args.config5_only:
+        ctx.release_workspace()
+        ex["config5"] = config5(torch, lqcd, inputs, psi.device)
+        return ex
     for prec in (() if args.solvers_only else (0, 1, 2)):
         fin = [ctx.pack_spinor(psi, p, prec) for p in (0, 1)]
         fo = [ctx.new_field(prec) for _ in (0, 1)]
@@ -776,7 +781,8 @@ def config5(torch, lqcd, inputs, dev):
             ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 1, 2), B5, dict(mr_steps=10)), ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10)),
             ("gcr_dd_mr4", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=4)),
             ("gcr_dd_group5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10, schwarz_group=5)),
-            ("gcr_sap_mr5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=5, schwarz_type=lqcd.SCHWARZ_MULTIPLICATIVE, sap_cycles=1))]
+            ("gcr_sap_mr5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=5, schwarz_type=lqcd.SCHWARZ_MULTIPLICATIVE, sap_cycles=1)),
+            ("gcr_noprecond", lqcd.SOLVER_GCR_DD, (0, 2, 2), None, dict(gcr_kmax=16, precondition=False))]
     for name, solver, prec, blk, extra_kw in runs:
         kw = dict(gcr_kmax=16, schwarz_block=blk, **extra_kw) if blk else dict(extra_kw)
         p = ctx.make_params(KAPPA, CSW, 1e-10, solver=solver, prec=prec, recon=(18, 12, 12), **kw)
