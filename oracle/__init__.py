@@ -177,6 +177,19 @@ def schwarz(r, U, Tcl, bc, kappa, parity, block, n_mr=10, omega_mr=1.0):
     return out
 
 
+def schwarz_ras(r, U, Tcl, bc, kappa, parity, block, overlap, n_mr=10, omega_mr=1.0, only_block=-1):
+    """Overlapping (restricted) additive Schwarz: every block's domain grown by `overlap` sites, block by block
+    (wilson_clover_oracle.cpp schwarz_ras).  only_block >= 0: the contribution of that block alone."""
+    r, U, Tcl = _c(r), _c(U), _c(Tcl)
+    out = np.empty_like(r)
+    rc = lib().orc_schwarz_ras(_p(out), _p(r), _p(U), _p(Tcl), _i4(dims_of(r)), _i4(bc), ctypes.c_double(kappa),
+                               ctypes.c_int(parity), _blk(block), ctypes.c_int(overlap), ctypes.c_int(n_mr),
+                               ctypes.c_double(omega_mr), ctypes.c_int(only_block))
+    if rc:
+        raise ValueError("schwarz_ras: a domain would reach around the lattice")
+    return out
+
+
 def schwarz_sap(r, U, Tcl, bc, kappa, parity, block, n_mr=4, omega_mr=1.0, n_cycle=1):
     """Multiplicative Schwarz (SAP) preconditioner: n_cycle cycles over the two block colours (wilson_clover_oracle.cpp)."""
     r, U, Tcl = _c(r), _c(U), _c(Tcl)

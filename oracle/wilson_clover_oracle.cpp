@@ -7,7 +7,8 @@
 // even-odd (Schur complement) preconditioned form (Sec. 3.1),
 // BiCGstab, the non-overlapping additive-Schwarz preconditioner
 // with a fixed number of MR steps (PAPER.md:146, Sec. 3.2; :250, Sec. 8.1) and
-// the GCR-DD solver (Algorithm 1).
+// the GCR-DD solver (Algorithm 1); plus the multiplicative (SAP) and the overlapping (restricted
+// additive) Schwarz variants the paper names.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 // --impl reference legs may load this file.  It shares no code, header, table
@@ -134,7 +135,10 @@ inline bool same_block(const int* blk, const int c[4], int mu, int d, const Lat&
 // ---- c.1  Dslash: the hopping part of Eq. 2 ---------------
 // (D psi)(x) = sum_mu [ s+ (1 - g_mu) U_mu(x) psi(x+mu) + s- (1 + g_mu) U_mu(x-mu)^dag psi(x-mu) ]
 // dagger: (1 -/+ g_mu) exchanged.  blk: Dirichlet cut (R7) or nullptr.
-void dslash(cplx* out, const cplx* in, const cplx* U, const Lat& lat, int dagger, const int* blk) {
+// dom: optional site mask (overlapping Schwarz domains, schwarz_ras below): a hop is kept only if both its ends are
+// in the domain.
+void dslash(cplx* out, const cplx* in, const cplx* U, const Lat& lat, int dagger, const int* blk,
+            const unsigned char* dom = nullptr) {
   const long V = lat.V;
 #pragma omp parallel for if(V >= 2048) schedule(static)
   for (long s = 0; s < V; ++s) {
@@ -145,6 +149,7 @@ void dslash(cplx* out, const cplx* in, const cplx* U, const Lat& lat, int dagger
       for (int dir = +1; dir >= -1; dir -= 2) {
         if (!same_block(blk, c, mu, dir, lat)) continue;
         const long n = lat.shifted(c, mu, dir);
+        if (dom && !(dom[s] && dom[n])) continue;
         const bool wraps = (dir > 0) ? (c[mu] == lat.L[mu] - 1) : (c[mu] == 0);
         const double sgn = (wraps && lat.bc[mu] < 0) ? -1.0 : 1.0;
         // colour part: U_mu(x) psi(x+mu)  or  U_mu(x-mu)^dagger psi(x-mu)
@@ -277,6 +282,7 @@ struct Op {                         // everything an operator application needs
   const cplx* U; const cplx* T; Lat lat; double kappa;
   const int* blk;                   // Schwarz block extents or nullptr
   int sym;                          // 0: asymmetric Schur complement (default), 1: symmetric form (c.5 "Optional")
+  const unsigned char* dom = nullptr;   // site mask of one overlapping Schwarz domain (schwarz_ras) or nullptr
   Op(const cplx* U_, const cplx* T_, const int* dims, const int* bc, double k, const int* blk_, int sym_ = 0)
     : U(U_), T(T_), lat(dims, bc), kappa(k), blk(blk_), sym(sym_) {}
   long n() const { return lat.V * 12; }
@@ -285,7 +291,7 @@ struct Op {                         // everything an operator application needs
 // c.3  M = A - kappa D   (2*kappa times Eq. 2; reading R3)
 void apply_M(cplx* out, const cplx* in, const Op& op, int dagger) {
   std::vector<cplx> d(op.n());
-  dslash(d.data(), in, op.U, op.lat, dagger, op.blk);
+  dslash(d.data(), in, op.U, op.lat, dagger, op.blk, op.dom);
   clover_apply(out, in, op.T, op.lat, op.kappa, 0, -1);
   const long n = op.n();
 #pragma omp parallel for if(n >= 16384) schedule(static)
@@ -325,10 +331,10 @@ void apply_matpc(cplx* out, const cplx* in, const Op& op, int p, int dagger) {
   const long n = op.n();
   std::vector<cplx> xin(in, in + n), t1(n), t2(n);
   mask_parity(xin.data(), op.lat, p);
-  dslash(t1.data(), xin.data(), op.U, op.lat, dagger, op.blk);     // lives on pbar
+  dslash(t1.data(), xin.data(), op.U, op.lat, dagger, op.blk, op.dom);     // lives on pbar
   mask_parity(t1.data(), op.lat, 1 - p);
   clover_apply(t2.data(), t1.data(), op.T, op.lat, op.kappa, 1, 1 - p);
-  dslash(t1.data(), t2.data(), op.U, op.lat, dagger, op.blk);      // back on p
+  dslash(t1.data(), t2.data(), op.U, op.lat, dagger, op.blk, op.dom);      // back on p
   mask_parity(t1.data(), op.lat, p);
   clover_apply(out, xin.data(), op.T, op.lat, op.kappa, 0, p);
   const double k2 = op.kappa * op.kappa;
@@ -509,6 +515,55 @@ void schwarz_sap(cplx* out, const cplx* rin, const Op& op, const Op& opD, int p,
     }
 }
 
+// Overlapping additive Schwarz in its restricted form (PAPER.md:146 "blocks which may or may not overlap", :338
+// "overlapping domains"; the restricted variant is the one of the paper's ref. [21]; reading R18 in
+// DESIGN.md).  The domain of block b is its box grown by `ovl` sites on both sides of every partitioned direction
+// (through the periodic wrap of the lattice; it must stay shorter than the lattice).  For every block, one at a time:
+//   rho = r on the domain, 0 elsewhere;  x_b = n_mr MR steps from 0 on Mhat with every hop that leaves the domain
+//   dropped, one alpha per domain;  out += x_b on the block's OWN box only (each site is written by exactly one block).
+// ovl = 0 is the non-overlapping K above.  only_block >= 0: that block alone (sampling at large sizes).
+// Returns 0, or 1 if a domain would reach around the lattice.
+int schwarz_ras(cplx* out, const cplx* rin, const Op& op, const int* blk, int ovl, int p, int n_mr, double omega_mr, int only_block) {
+  const long n = op.n(), V = op.lat.V;
+  const Lat& lat = op.lat;
+  int nb[4], NB = 1;
+  for (int m = 0; m < 4; ++m) {
+    nb[m] = lat.L[m] / blk[m]; NB *= nb[m];
+    if (nb[m] > 1 && ovl > 0 && blk[m] + 2 * ovl >= lat.L[m]) return 1;
+  }
+  for (long i = 0; i < n; ++i) out[i] = 0;
+  std::vector<unsigned char> dom(V), own(V);
+  std::vector<cplx> rho(n), w(n), xb(n);
+  for (int b = 0; b < NB; ++b) {
+    if (only_block >= 0 && b != only_block) continue;
+    int bc[4], q = b;
+    for (int m = 0; m < 4; ++m) { bc[m] = q % nb[m]; q /= nb[m]; }
+    for (long s = 0; s < V; ++s) {
+      int c[4]; lat.coords(s, c);
+      bool in = true, mine = true;
+      for (int m = 0; m < 4; ++m) {
+        if (nb[m] == 1) continue;                               // unpartitioned direction: the whole extent
+        const int d = ((c[m] - bc[m] * blk[m]) % lat.L[m] + lat.L[m]) % lat.L[m];   // distance from the box's first site
+        mine = mine && d < blk[m];
+        in = in && (d < blk[m] + ovl || d >= lat.L[m] - ovl);
+      }
+      dom[s] = in; own[s] = mine;
+    }
+    Op od = op; od.blk = nullptr; od.dom = dom.data();
+    for (long s = 0; s < V; ++s) for (int i = 0; i < 12; ++i) { rho[s*12+i] = dom[s] ? rin[s*12+i] : cplx(0.0); xb[s*12+i] = 0; }
+    mask_parity(rho.data(), lat, p);
+    for (int step = 0; step < n_mr; ++step) {
+      apply_matpc(w.data(), rho.data(), od, p, 0);
+      cplx wr = 0; double ww = 0;
+      for (long i = 0; i < n; ++i) { wr += std::conj(w[i]) * rho[i]; ww += std::norm(w[i]); }
+      const cplx a = (ww > 0.0) ? omega_mr * wr / ww : cplx(0.0);
+      for (long i = 0; i < n; ++i) { xb[i] += a * rho[i]; rho[i] -= a * w[i]; }
+    }
+    for (long s = 0; s < V; ++s) if (own[s]) for (int i = 0; i < 12; ++i) out[s*12+i] += xb[s*12+i];
+  }
+  return 0;
+}
+
 // c.9  GCR-DD, Algorithm 1, all in fp64 here (hats kept as names only).
 // Stops when ||r0|| <= stop.  precond: 0 = identity (plain GCR), 1 = Schwarz K.
 int gcr_dd(cplx* x, const cplx* bhat, const Op& op, const Op& opD, int p, double stop, int maxit,
@@ -645,6 +700,12 @@ void orc_schwarz(cplx* out, const cplx* rin, const cplx* U, const cplx* T, const
 }
 
 // K_sap r on parity p (multiplicative Schwarz, n_cycle cycles over the two block colours)
+int orc_schwarz_ras(cplx* out, const cplx* rin, const cplx* U, const cplx* T, const int* dims, const int* bc,
+                    double kappa, int parity, const int* block, int overlap, int n_mr, double omega_mr, int only_block) {
+  Op op(U, T, dims, bc, kappa, nullptr);
+  return schwarz_ras(out, rin, op, block, overlap, parity, n_mr, omega_mr, only_block);
+}
+
 void orc_schwarz_sap(cplx* out, const cplx* rin, const cplx* U, const cplx* T, const int* dims, const int* bc,
                      double kappa, int parity, const int* block, int n_mr, double omega_mr, int n_cycle) {
   Op op(U, T, dims, bc, kappa, nullptr);

@@ -496,3 +496,61 @@ def test_schwarz_sap_pins(four):
     assert ig["status"] == 0 and _rel(xg.ravel(), xs) < 1e-10
     xa, ia = oracle.gcr_pc(bhat, U, Tcl, BC, kappa, p, 1e-12 * np.linalg.norm(b), block=blk, n_mr=4)
     assert ig["iterations"] <= ia["iterations"]                   # multiplicative beats additive per outer iteration here
+
+
+def test_schwarz_ras_pins():
+    """Overlapping restricted additive Schwarz (reading R18) against what fixes it, on 6x2x2x8 with blocks 2x2x2x4
+    (partitioned in x and t, antiperiodic t, domains that reach through the lattice's wrap): (1) no overlap = the
+    densely pinned K; (2) block by block, a dense restatement: the domain built from coordinates here, M cut to the
+    domain entry by entry, its Schur complement on parity p, MR with one alpha, restriction to the block's own box;
+    (3) the blocks add up; (4) support and parity; (5) a domain that would reach around the lattice is refused."""
+    dims, kappa, p = (6, 2, 2, 8), 0.12, 0
+    blk, ovl = (2, 2, 2, 4), 1
+    U = inputs.random_gauge(dims, 0.5, 3)
+    Tcl = oracle.clover_term(U, 1.0)
+    b = inputs.gaussian_spinor(dims, 4)
+    par = inputs.parity_mask(dims)
+    r = b * (par == p)[..., None, None]
+    # (1)
+    assert _rel(oracle.schwarz_ras(r, U, Tcl, BC, kappa, p, blk, 0, n_mr=4), oracle.schwarz(r, U, Tcl, BC, kappa, p, blk, n_mr=4)) < 1e-14
+    # (2)
+    Md = _dense(lambda v: oracle.M(v, U, Tcl, BC, kappa), b.shape)
+    T_, Z_, Y_, X_ = b.shape[:4]
+    t, z, y, x = np.meshgrid(np.arange(T_), np.arange(Z_), np.arange(Y_), np.arange(X_), indexing="ij")
+    sp = np.repeat(par.ravel(), 12)
+    total = np.zeros(r.size, dtype=complex)
+    nbx, nbt = dims[0] // blk[0], dims[3] // blk[3]
+    for bt in range(nbt):
+        for bx in range(nbx):
+            box = bx + nbx * bt                                   # y, z are not partitioned
+            dx, dt = (x - bx * blk[0]) % dims[0], (t - bt * blk[3]) % dims[3]
+            own = (dx < blk[0]) & (dt < blk[3])
+            dom = ((dx < blk[0] + ovl) | (dx >= dims[0] - ovl)) & ((dt < blk[3] + ovl) | (dt >= dims[3] - ovl))
+            assert dom.sum() == (blk[0] + 2) * 2 * 2 * (blk[3] + 2) and (own & ~dom).sum() == 0
+            sd = np.repeat(dom.ravel(), 12)
+            ip, iq = np.where(sd & (sp == p))[0], np.where(sd & (sp != p))[0]
+            S = Md[np.ix_(ip, ip)] - Md[np.ix_(ip, iq)] @ np.linalg.solve(Md[np.ix_(iq, iq)], Md[np.ix_(iq, ip)])
+            rho = r.ravel()[ip].copy()
+            xb = np.zeros_like(rho)
+            for _ in range(3):
+                w = S @ rho
+                a = np.vdot(w, rho) / np.vdot(w, w).real
+                xb += a * rho
+                rho -= a * w
+            want = np.zeros(r.size, dtype=complex)
+            want[ip] = xb
+            want *= np.repeat(own.ravel(), 12)
+            got = oracle.schwarz_ras(r, U, Tcl, BC, kappa, p, blk, ovl, n_mr=3, only_block=box).ravel()
+            assert _rel(got, want) < 1e-12, box
+            total += want
+    # (3), (4)
+    full = oracle.schwarz_ras(r, U, Tcl, BC, kappa, p, blk, ovl, n_mr=3)
+    assert _rel(full.ravel(), total) < 1e-12
+    assert np.max(np.abs(full[par != p])) == 0.0
+    # the overlap changes the result (it is not silently ignored) and still approximates Mhat^-1
+    assert _rel(full, oracle.schwarz(r, U, Tcl, BC, kappa, p, blk, n_mr=3)) > 1e-3
+    res = r - oracle.matpc(oracle.schwarz_ras(r, U, Tcl, BC, kappa, p, blk, ovl, n_mr=10), U, Tcl, BC, kappa, p)
+    assert np.linalg.norm(res) < 0.5 * np.linalg.norm(r)
+    # (5)
+    with pytest.raises(ValueError):
+        oracle.schwarz_ras(r, U, Tcl, BC, kappa, p, blk, 2)       # x: 2 + 4 = 6 = L
