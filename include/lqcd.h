@@ -162,6 +162,16 @@ int lqcd_schwarz_sap(lqcd_ctx* ctx, void* out, const void* in, int parity, doubl
  * lqcd_invert_params::schwarz_group); 0 = all blocks per launch.  LQCD_EINVAL if negative. */
 int lqcd_set_schwarz_group(lqcd_ctx* ctx, int blocks_per_group);
 
+/* Overlapping Schwarz domains for later lqcd_schwarz calls on this context (lqcd_invert takes the value from
+ * lqcd_invert_params::schwarz_overlap).  PAPER.md:146 ("blocks which may or may not overlap ... a tunable parameter"),
+ * :338; reading R18: restricted additive Schwarz -- the domain of a block is its box grown by `overlap` sites
+ * on both sides of every partitioned direction (through the lattice's periodic wrap), the MR steps run on the domain
+ * with Dirichlet boundaries, and the result is kept on the block's own box.  0 = non-overlapping (default, the paper's
+ * runs).  LQCD_EINVAL at the next Schwarz call if a grown domain would reach around the lattice (block + 2 overlap >=
+ * extent) or if overlap x number of partitioned directions is odd; the multiplicative variant takes no overlap.  The
+ * block-major copies of links, clover blocks and work vectors grow by the volume ratio of grown domain to block. */
+int lqcd_set_schwarz_overlap(lqcd_ctx* ctx, int overlap);
+
 typedef struct {
   double kappa;
   double c_sw;            /* must equal the value given to lqcd_build_clover */
@@ -192,6 +202,8 @@ typedef struct {
                              iteration k+1 of the low-precision iteration (BiCGstab, CGNR, CGNE) or after outer iteration
                              k+1 (GCR); lqcd_invert_result::history_count entries are written.  Reported, never
                              asserted (convergence history is "parity unpinned"). */
+  int    schwarz_overlap; /* GCR-DD, additive: sites by which every Schwarz domain is grown on both sides of each partitioned
+                             direction (lqcd_set_schwarz_overlap; 0 = the paper's non-overlapping blocks) */
 } lqcd_invert_params;
 
 typedef struct {

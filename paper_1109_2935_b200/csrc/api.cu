@@ -82,7 +82,7 @@ int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, 
     // built into a local and published only when it holds valid links; the stream is synchronised once, so the copy
     // is complete for every stream that uses it later
     char* g = nullptr;
-    int rc = dev_alloc(c, (void**)&g, gauge_bytes(prec, recon, c->nat.ns));
+    int rc = dev_alloc(c, (void**)&g, gauge_bytes(prec, recon, blocked ? c->bm.blk.ns : c->nat.ns));
     if (rc) return rc;
     unsigned bad = 0;
     cudaError_t e = cudaMemsetAsync(c->gflag, 0, sizeof(unsigned), s);
@@ -111,9 +111,10 @@ int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A
   char*& ai = blocked ? c->bclovinv[prec] : c->clovinv[prec];
   if (!a || !ai) {
     char *na = nullptr, *nai = nullptr;       // published only when both hold valid data (see get_gauge)
-    int rc = dev_alloc(c, (void**)&na, clover_bytes(prec, c->nat.ns));
+    const long long ns = blocked ? c->bm.blk.ns : c->nat.ns;
+    int rc = dev_alloc(c, (void**)&na, clover_bytes(prec, ns));
     if (rc) return rc;
-    rc = dev_alloc(c, (void**)&nai, clover_bytes(prec, c->nat.ns));
+    rc = dev_alloc(c, (void**)&nai, clover_bytes(prec, ns));
     if (rc) { cudaFree(na); return rc; }
     cudaError_t e = run_clover_make(prec, na, nai, c->T72, c->bm, blocked ? 1 : 0, kappa, s);
     c->launches++;
@@ -128,28 +129,39 @@ int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A
 
 int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out) {
   char*& t = blocked ? c->btmp[prec] : c->tmp[prec];
-  if (!t) { int rc = dev_alloc(c, (void**)&t, spinor_bytes(prec, c->nat.ns)); if (rc) return rc; }
+  if (!t) { int rc = dev_alloc(c, (void**)&t, spinor_bytes(prec, blocked ? c->bm.blk.ns : c->nat.ns)); if (rc) return rc; }
   *out = t;
   return LQCD_OK;
 }
 
-int set_blocks(lqcd_ctx* c, const int* blk, int cmaj) {
+int set_blocks(lqcd_ctx* c, const int* blk, int cmaj, int overlap) {
   if (!blk) return fail(c, LQCD_EINVAL, "null block");
   for (int m = 0; m < 4; ++m)
     if (blk[m] < 2 || (blk[m] & 1) || c->dims[m] % blk[m]) return fail(c, LQCD_EINVAL, "Schwarz block extents must be even and divide the lattice");
   if (cmaj && ((c->dims[0] / blk[0]) & 1)) return fail(c, LQCD_EINVAL, "multiplicative Schwarz needs an even number of blocks in x");
+  // overlapping domains (reading R18): every partitioned direction grows by `overlap` sites on both sides
+  int ovl[4], osum = 0;
+  for (int m = 0; m < 4; ++m) {
+    ovl[m] = (overlap > 0 && c->dims[m] / blk[m] > 1) ? overlap : 0;
+    osum += ovl[m];
+    if (ovl[m] && blk[m] + 2 * ovl[m] >= c->dims[m]) return fail(c, LQCD_EINVAL, "Schwarz overlap: a domain would reach around the lattice");
+  }
+  if (overlap < 0 || (osum & 1)) return fail(c, LQCD_EINVAL, "Schwarz overlap: overlap x number of partitioned directions must be even");
+  if (osum && cmaj) return fail(c, LQCD_EINVAL, "multiplicative Schwarz is built for non-overlapping blocks");
   // cmaj = 0: either box order will do (the additive preconditioner does not care), so matching copies are kept
-  if (c->have_blocks && !memcmp(blk, c->bm.blk.X, 4 * sizeof(int)) && (!cmaj || c->bm.cmaj)) return LQCD_OK;
+  if (c->have_blocks && !memcmp(blk, c->bm.core, 4 * sizeof(int)) && !memcmp(ovl, c->bm.ovl, 4 * sizeof(int)) && (!cmaj || c->bm.cmaj)) return LQCD_OK;
   drop_block_copies(c);
   c->bm.cmaj = cmaj ? 1 : 0;
-  int nb = 1, bcb[4];
+  int nb = 1, bcb[4], ext[4];
   for (int m = 0; m < 4; ++m) {
     c->bm.nbd[m] = c->dims[m] / blk[m];
     nb *= c->bm.nbd[m];
     bcb[m] = (c->bm.nbd[m] == 1) ? c->bc[m] : 0;    // unpartitioned direction keeps its wrap (R7)
+    c->bm.core[m] = blk[m]; c->bm.ovl[m] = ovl[m];
+    ext[m] = blk[m] + 2 * ovl[m];
   }
   c->bm.nat = c->nat;
-  c->bm.blk = make_geom(blk, bcb, nb);
+  c->bm.blk = make_geom(ext, bcb, nb);
   c->have_blocks = true;
   // per-warp partial dots of every box, then alpha_b (re, im) of every box
   const size_t need = (size_t)nb * ((c->bm.blk.vh + LQ_DSLASH_BLOCK - 1) / LQ_DSLASH_BLOCK) * (LQ_DSLASH_BLOCK / 32) * 4 + 2 * (size_t)nb;
@@ -332,9 +344,11 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
   c->Vh = c->V / 2;
   c->nat = make_geom(dims, boundary, 1);
   c->bm.nat = c->nat; c->bm.blk = c->nat; c->bm.nbd[0] = c->bm.nbd[1] = c->bm.nbd[2] = c->bm.nbd[3] = 1; c->bm.cmaj = 0;
+  for (int m = 0; m < 4; ++m) { c->bm.core[m] = c->dims[m]; c->bm.ovl[m] = 0; }
   c->launches = 0;
   c->have_gauge = c->have_blocks = c->have_clover = false;
   c->schwarz_group = 0;
+  c->schwarz_overlap = 0;
   c->g64 = nullptr; c->T72 = nullptr; c->kappa = NAN; c->c_sw = NAN;
   memset(c->gauge, 0, sizeof(c->gauge)); memset(c->bgauge, 0, sizeof(c->bgauge));
   memset(c->clov, 0, sizeof(c->clov)); memset(c->clovinv, 0, sizeof(c->clovinv));

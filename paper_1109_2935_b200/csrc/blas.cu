@@ -171,15 +171,20 @@ cudaError_t run_gcr_orth(int prec, const MultiArgs& m, int max_ctas, cudaStream_
 template <class PA, class PB>
 __global__ void __launch_bounds__(LQ_BLAS_BLOCK) convert_kernel(char* dst, const char* src, const BlockMap bm, int dir, int parity,
                                                                 int box0, int nbox) {
+  // one thread per site of the block-major field (= per lattice site without overlap).  With overlapping domains
+  // (host.h) a gather (dir 1) copies a lattice site into every box that holds it, with the box's sign; a scatter
+  // (dir 2) writes the own sites of every box only, so each lattice site is written once.
   const long long i = (long long)blockIdx.x * LQ_BLAS_BLOCK + threadIdx.x;
-  if (i >= bm.nat.ns) return;
-  long long is = i, id = i;
-  bool zero = false;
+  if (i >= (dir == 0 ? bm.nat.ns : bm.blk.ns)) return;
+  long long is = i, id = i, ns_s = bm.nat.ns, ns_d = bm.nat.ns;
+  bool zero = false, own = true;
+  int sign = 1;
   if (dir != 0) {
     const int box = (int)(i / bm.blk.vh), lcb = (int)(i % bm.blk.vh);
-    const long long n = block_to_natural(bm, box, lcb, parity);
-    if (dir == 1) { is = n; id = i; } else { is = i; id = n; }
+    const long long n = block_to_natural(bm, box, lcb, parity, &own, &sign);
+    if (dir == 1) { is = n; id = i; ns_d = bm.blk.ns; } else { is = i; id = n; ns_s = bm.blk.ns; }
     zero = dir == 2 && nbox > 0 && (box < box0 || box >= box0 + nbox);     // outside the active box range (one colour)
+    if (dir == 2 && !own) return;
   }
   typename PB::real vb[24];
   if (zero) {
@@ -187,11 +192,12 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) convert_kernel(char* dst, const
     for (int k = 0; k < 24; ++k) vb[k] = 0;
   } else {
     typename PA::real va[24];
-    load_site<PA, 24>(va, src, bm.nat.ns, is);
+    load_site<PA, 24>(va, src, ns_s, is);
+    const typename PB::real sg = (typename PB::real)((dir == 1) ? sign : 1);
 #pragma unroll
-    for (int k = 0; k < 24; ++k) vb[k] = (typename PB::real)va[k];
+    for (int k = 0; k < 24; ++k) vb[k] = sg * (typename PB::real)va[k];
   }
-  store_site<PB, 24>(vb, dst, bm.nat.ns, id);
+  store_site<PB, 24>(vb, dst, ns_d, id);
 }
 
 // y (PH) += sum_{i<n} chi_i * x_i (PL)   (implicit solution update; and
@@ -231,7 +237,8 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, cons
 
 template <class PA>
 static cudaError_t convert_b(int pb, char* dst, const char* src, const BlockMap& bm, int dir, int parity, cudaStream_t s, int box0, int nbox) {
-  dim3 grid((unsigned)((bm.nat.ns + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK)), block(LQ_BLAS_BLOCK);
+  const long long nsite = dir == 0 ? bm.nat.ns : bm.blk.ns;
+  dim3 grid((unsigned)((nsite + LQ_BLAS_BLOCK - 1) / LQ_BLAS_BLOCK)), block(LQ_BLAS_BLOCK);
   switch (pb) {
     case 0: convert_kernel<PA, PrecD><<<grid, block, 0, s>>>(dst, src, bm, dir, parity, box0, nbox); break;
     case 1: convert_kernel<PA, PrecS><<<grid, block, 0, s>>>(dst, src, bm, dir, parity, box0, nbox); break;

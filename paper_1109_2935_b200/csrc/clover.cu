@@ -159,7 +159,8 @@ cudaError_t run_clover_term(double* T72, const double* g64, const Geom& nat, dou
 template <class P>
 __global__ void __launch_bounds__(64) clover_make_kernel(char* A, char* Ainv, const double* __restrict__ T72, const BlockMap bm, int blocked, double kappa) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= bm.nat.ns) return;
+  const long long ns_d = blocked ? bm.blk.ns : bm.nat.ns;      // block-major copies have their own size with overlapping domains (host.h)
+  if (i >= ns_d) return;
   const int parity = blockIdx.y;
   long long is = i;
   if (blocked) is = block_to_natural(bm, (int)(i / bm.blk.vh), (int)(i % bm.blk.vh), parity);
@@ -203,17 +204,17 @@ __global__ void __launch_bounds__(64) clover_make_kernel(char* A, char* Ainv, co
     }
   }
   typename P::real v[72];
-  const long long pb = (long long)parity * site_bytes<P>(72, true) * bm.nat.ns;
+  const long long pb = (long long)parity * site_bytes<P>(72, true) * ns_d;
 #pragma unroll
   for (int k = 0; k < 72; ++k) v[k] = (typename P::real)t[k];
-  store_site<P, 72>(v, A + pb, bm.nat.ns, i);
+  store_site<P, 72>(v, A + pb, ns_d, i);
 #pragma unroll
   for (int k = 0; k < 72; ++k) v[k] = (typename P::real)inv[k];
-  store_site<P, 72>(v, Ainv + pb, bm.nat.ns, i);
+  store_site<P, 72>(v, Ainv + pb, ns_d, i);
 }
 
 cudaError_t run_clover_make(int prec, char* A, char* Ainv, const double* T72, const BlockMap& bm, int blocked, double kappa, cudaStream_t s) {
-  dim3 grid((unsigned)((bm.nat.ns + 63) / 64), 2), block(64);
+  dim3 grid((unsigned)(((blocked ? bm.blk.ns : bm.nat.ns) + 63) / 64), 2), block(64);
   switch (prec) {
     case 0: clover_make_kernel<PrecD><<<grid, block, 0, s>>>(A, Ainv, T72, bm, blocked, kappa); break;
     case 1: clover_make_kernel<PrecS><<<grid, block, 0, s>>>(A, Ainv, T72, bm, blocked, kappa); break;

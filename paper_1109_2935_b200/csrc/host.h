@@ -22,14 +22,26 @@ namespace lq {
 // the nb/2 boxes of colour 0 first, then those of colour 1 -- so that one colour is a contiguous box range
 // (needs an even number of boxes in x: position q of colour c has bx = 2 (q % (nbd0/2)) + ((by+bz+bt+c) & 1),
 // the checkerboard trick of the site index one level up).
+// Overlapping domains (reading R18): ovl[m] > 0 grows every box by ovl[m] sites on both sides of the
+// partitioned direction m, through the lattice's periodic wrap.  blk then holds the GROWN extents (blk.X = core + 2 ovl,
+// blk.ns = nb * blk.vh > nat.ns: a block-major field has its own size), a site of the lattice appears in several boxes,
+// and a box site knows whether it belongs to the box's own core.  The sum of the ovl[m] is even (set_blocks), so the
+// parity of a site inside its grown box is still its global parity.  A grown box may contain an antiperiodic boundary
+// of the lattice in its interior; the box operator carries no sign there (Dirichlet coefficients only at box edges):
+// inside a box the sign plane is removed by psi -> -psi on the far side, applied when a field is gathered into the
+// boxes (`sign` below) -- the own sites, the only ones scattered back, all have sign +1.
 struct BlockMap {
   Geom nat;     // whole lattice, nb = 1
-  Geom blk;     // one box, nb = number of boxes, ns = nat.ns
+  Geom blk;     // one box (grown extents), nb = number of boxes, ns = nb * vh (= nat.ns without overlap)
   int nbd[4];
   int cmaj;
+  int core[4];  // extents of the box itself
+  int ovl[4];   // overlap per direction (0: none / direction not partitioned)
 };
 
-LQ_DEV long long block_to_natural(const BlockMap& bm, int box, int lcb, int parity) {
+// natural checkerboard index of site lcb of box `box`; own: the site is in the box's core; sign: -1 if the site lies beyond
+// an antiperiodic lattice boundary as seen from the box's core
+LQ_DEV long long block_to_natural(const BlockMap& bm, int box, int lcb, int parity, bool* own = nullptr, int* sign = nullptr) {
   int lc[4];
   cb_to_coords(bm.blk, lcb, parity, lc);
   int bc[4];
@@ -47,9 +59,18 @@ LQ_DEV long long block_to_natural(const BlockMap& bm, int box, int lcb, int pari
 #pragma unroll
     for (int m = 0; m < 4; ++m) { bc[m] = b % bm.nbd[m]; b /= bm.nbd[m]; }
   }
-  int gc[4];
+  int gc[4], sg = 1;
+  bool mine = true;
 #pragma unroll
-  for (int m = 0; m < 4; ++m) gc[m] = bc[m] * bm.blk.X[m] + lc[m];
+  for (int m = 0; m < 4; ++m) {
+    int g = bc[m] * bm.core[m] - bm.ovl[m] + lc[m];
+    if (g < 0) { g += bm.nat.X[m]; sg *= bm.nat.bc[m]; }
+    else if (g >= bm.nat.X[m]) { g -= bm.nat.X[m]; sg *= bm.nat.bc[m]; }
+    mine = mine && lc[m] >= bm.ovl[m] && lc[m] < bm.ovl[m] + bm.core[m];
+    gc[m] = g;
+  }
+  if (own) *own = mine;
+  if (sign) *sign = sg;
   return coords_to_cb(bm.nat, gc);
 }
 
@@ -105,6 +126,7 @@ struct lqcd_ctx {
   lq::BlockMap bm;
   char* bgauge[3][3];
   int schwarz_group;      // blocks per launch group of the preconditioner (0 = all; lqcd_invert_params::schwarz_group)
+  int schwarz_overlap;    // overlap of the Schwarz domains (0 = none; lqcd_invert_params::schwarz_overlap)
   // clover
   bool have_clover;
   double c_sw;

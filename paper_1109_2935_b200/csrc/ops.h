@@ -14,7 +14,7 @@ void ws_put(lqcd_ctx* c, void* p, size_t bytes, cudaStream_t s);
 int get_gauge(lqcd_ctx* c, int prec, int recon, bool blocked, const char** out, cudaStream_t s);
 int get_clover(lqcd_ctx* c, int prec, double kappa, bool blocked, const char** A, const char** Ainv, cudaStream_t s);
 int get_tmp(lqcd_ctx* c, int prec, bool blocked, char** out);
-int set_blocks(lqcd_ctx* c, const int* blk, int cmaj = 0);   // cmaj: colour-major box order (multiplicative Schwarz)
+int set_blocks(lqcd_ctx* c, const int* blk, int cmaj = 0, int overlap = 0);   // cmaj: colour-major box order (multiplicative Schwarz); overlap: host.h
 int op_dslash(lqcd_ctx* c, char* out, const char* in, const char* y, int parity_out, int dagger, int prec, int recon,
               int epi, double a, double kappa, bool blocked, cudaStream_t s, int cb0 = 0, int cb1 = -1, int fin = 0,
               const char* q = nullptr, int box0 = 0, int nbox = 0);

@@ -35,7 +35,8 @@ cudaError_t run_pack_gauge(double* g64, const double* U, const Geom& nat, cudaSt
 template <class P, int RECON>
 __global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, const BlockMap bm, int blocked, unsigned* bad) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= bm.nat.ns) return;
+  const long long ns_d = blocked ? bm.blk.ns : bm.nat.ns;      // block-major copies have their own size with overlapping domains (host.h)
+  if (i >= ns_d) return;
   const int pm = blockIdx.y, parity = pm >> 2;
   long long is = i;
   if (blocked) is = block_to_natural(bm, (int)(i / bm.blk.vh), (int)(i % bm.blk.vh), parity);
@@ -45,7 +46,7 @@ __global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, 
   compress_link<RECON>(u, v);
   alignas(16) typename P::store_t q[RECON];
   quantize_link<P, RECON>(v, q);
-  Rec<typename P::store_t, RECON>::store(q, dst + (long long)pm * RECON * sizeof(typename P::store_t) * bm.nat.ns, bm.nat.ns, i);
+  Rec<typename P::store_t, RECON>::store(q, dst + (long long)pm * RECON * sizeof(typename P::store_t) * ns_d, ns_d, i);
   if (RECON != 18 && bad) {
     unsigned f = 0;
     // rows orthonormal, row2 = conj(row0 x row1)  <=>  U in SU(3)
@@ -85,7 +86,7 @@ __global__ void convert_gauge_kernel(char* dst, const double* __restrict__ g64, 
 
 template <class P>
 static cudaError_t convert_gauge_p(int recon, char* dst, const double* g64, const BlockMap& bm, int blocked, unsigned* bad, cudaStream_t s) {
-  dim3 grid((unsigned)((bm.nat.ns + 127) / 128), 8), block(128);
+  dim3 grid((unsigned)(((blocked ? bm.blk.ns : bm.nat.ns) + 127) / 128), 8), block(128);
   switch (recon) {
     case 18: convert_gauge_kernel<P, 18><<<grid, block, 0, s>>>(dst, g64, bm, blocked, bad); break;
     case 12: convert_gauge_kernel<P, 12><<<grid, block, 0, s>>>(dst, g64, bm, blocked, bad); break;

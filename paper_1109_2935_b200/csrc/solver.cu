@@ -553,14 +553,17 @@ int solve_gcr(lqcd_ctx* c, char* x, const char* b, const lqcd_invert_params& p, 
   }
   const bool sap = p.precondition && p.schwarz_type == LQCD_SCHWARZ_MULTIPLICATIVE;
   // the solve's group size must not outlive it (lqcd_set_schwarz_group is the context-level setting)
-  struct GroupGuard { lqcd_ctx* c; int saved; bool armed; ~GroupGuard() { if (armed) c->schwarz_group = saved; } } group_guard{c, c->schwarz_group, false};
+  struct GroupGuard { lqcd_ctx* c; int saved, saved_ovl; bool armed; ~GroupGuard() { if (armed) { c->schwarz_group = saved; c->schwarz_overlap = saved_ovl; } } }
+      group_guard{c, c->schwarz_group, c->schwarz_overlap, false};
   char *sr = nullptr, *sy = nullptr, *st = nullptr;
   if (p.precondition) {
     if (p.schwarz_group < 0) return fail(c, LQCD_EINVAL, "schwarz_group");
     group_guard.armed = true;
     c->schwarz_group = p.schwarz_group;
-    if ((rc = set_blocks(c, p.schwarz_block, sap ? 1 : 0))) return rc;
-    for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, ns)))) return rc;
+    if (p.schwarz_overlap < 0 || (sap && p.schwarz_overlap)) return fail(c, LQCD_EINVAL, "schwarz_overlap");
+    c->schwarz_overlap = p.schwarz_overlap;
+    if ((rc = set_blocks(c, p.schwarz_block, sap ? 1 : 0, c->schwarz_overlap))) return rc;
+    for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(pp, c->bm.blk.ns)))) return rc;   // block-major: grown domains
     if (sap) for (char** q : {&sr, &sy, &st}) if ((rc = wk.get(q, spinor_bytes(ps, ns)))) return rc;
   }
   double r0n;
@@ -823,11 +826,11 @@ int lqcd_schwarz(lqcd_ctx* c, void* out, const void* in, int parity, double kapp
     return fail(c, LQCD_EINVAL, "schwarz arguments");
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
-  int rc = set_blocks(c, block);
+  int rc = set_blocks(c, block, 0, c->schwarz_overlap);
   if (rc) return rc;
   Work wk(c, s);
   char *rho, *w, *xk;
-  for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->nat.ns)))) return rc;
+  for (char** q : {&rho, &w, &xk}) if ((rc = wk.get(q, spinor_bytes(prec, c->bm.blk.ns)))) return rc;     // block-major: grown domains
   rc = schwarz_apply(c, (char*)out, (const char*)in, parity, kappa, n_mr, omega_mr, prec, recon, prec_io, rho, w, xk, s);
   cudaStreamSynchronize(s);          // workspace is freed on return
   return rc;
@@ -856,6 +859,13 @@ int lqcd_set_schwarz_group(lqcd_ctx* c, int blocks_per_group) {
   if (!c) return LQCD_EINVAL;
   if (blocks_per_group < 0) return fail(c, LQCD_EINVAL, "schwarz group");
   c->schwarz_group = blocks_per_group;
+  return LQCD_OK;
+}
+
+int lqcd_set_schwarz_overlap(lqcd_ctx* c, int overlap) {
+  if (!c) return LQCD_EINVAL;
+  if (overlap < 0) return fail(c, LQCD_EINVAL, "schwarz overlap");
+  c->schwarz_overlap = overlap;
   return LQCD_OK;
 }
 

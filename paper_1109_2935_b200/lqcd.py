@@ -26,7 +26,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_last_error", "lqcd_release_workspace", "lqcd_load_gauge", "lqcd_build_clover",
     "lqcd_field_bytes", "lqcd_pack_spinor", "lqcd_unpack_spinor", "lqcd_dslash", "lqcd_clover",
-    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_apply_host_c64", "lqcd_invert_host",
+    "lqcd_matpc", "lqcd_matpc_sym", "lqcd_dslash_mrhs", "lqcd_matpc_mrhs", "lqcd_schwarz", "lqcd_schwarz_sap", "lqcd_set_schwarz_group", "lqcd_set_schwarz_overlap", "lqcd_invert", "lqcd_invert_mrhs", "lqcd_apply_host", "lqcd_apply_host_c64", "lqcd_invert_host",
     "lqcd_axpy_norm", "lqcd_cdot", "lqcd_cdot_static", "lqcd_launch_count",
     "lqcd_load_staggered_links", "lqcd_pack_staggered", "lqcd_unpack_staggered", "lqcd_staggered_dslash", "lqcd_staggered_mdagm", "lqcd_staggered_multishift",
 ]
@@ -42,7 +42,7 @@ class InvertParams(ctypes.Structure):
         ("mr_steps", ctypes.c_int), ("mr_omega", ctypes.c_double),
         ("use_initial_guess", ctypes.c_int), ("precondition", ctypes.c_int), ("matpc_type", ctypes.c_int),
         ("schwarz_group", ctypes.c_int), ("schwarz_type", ctypes.c_int), ("sap_cycles", ctypes.c_int), ("history_len", ctypes.c_int),
-        ("residual_history", ctypes.POINTER(ctypes.c_double)),
+        ("residual_history", ctypes.POINTER(ctypes.c_double)), ("schwarz_overlap", ctypes.c_int),
     ]
 
 
@@ -93,6 +93,7 @@ def load_library():
             "lqcd_matpc_mrhs": (i, [vp, vp, vp, i, i, i, d, i, i, vp]),
             "lqcd_schwarz": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, vp]),
             "lqcd_set_schwarz_group": (i, [vp, i]),
+            "lqcd_set_schwarz_overlap": (i, [vp, i]),
             "lqcd_schwarz_sap": (i, [vp, vp, vp, i, d, ctypes.POINTER(i), i, d, i, i, i, i, i, vp]),
             "lqcd_invert": (i, [vp, vp, vp, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
             "lqcd_invert_mrhs": (i, [vp, vp, vp, i, ctypes.POINTER(InvertParams), ctypes.POINTER(InvertResult), vp]),
@@ -223,6 +224,9 @@ class Context:
     def set_schwarz_group(self, blocks_per_group):
         self._check(self.lib.lqcd_set_schwarz_group(self.h, int(blocks_per_group)))
 
+    def set_schwarz_overlap(self, overlap):
+        self._check(self.lib.lqcd_set_schwarz_overlap(self.h, int(overlap)))
+
     def schwarz(self, out, inp, parity, kappa, block, n_mr, omega_mr, prec, recon, prec_io):
         self._check(self.lib.lqcd_schwarz(self.h, _ptr(out), _ptr(inp), parity, kappa, _i4(block), n_mr, omega_mr,
                                           prec, recon, prec_io, _stream()))
@@ -289,7 +293,7 @@ class Context:
     def make_params(kappa, c_sw, tol, solver=SOLVER_BICGSTAB, prec=(PREC_DOUBLE, PREC_SINGLE, PREC_HALF),
                     recon=(RECON_18, RECON_12, RECON_12), delta=0.1, max_iter=5000, parity=0, gcr_kmax=16,
                     schwarz_block=(0, 0, 0, 0), mr_steps=10, mr_omega=1.0, use_initial_guess=False, precondition=True,
-                    matpc_type=MATPC_ASYMMETRIC, schwarz_group=0, history_len=0, schwarz_type=0, sap_cycles=1):
+                    matpc_type=MATPC_ASYMMETRIC, schwarz_group=0, history_len=0, schwarz_type=0, sap_cycles=1, schwarz_overlap=0):
         p = InvertParams()
         p.kappa, p.c_sw, p.tol, p.delta = kappa, c_sw, tol, delta
         p.max_iter, p.solver = max_iter, solver
@@ -303,6 +307,7 @@ class Context:
         p.matpc_type = int(matpc_type)
         p.schwarz_group = int(schwarz_group)
         p.schwarz_type, p.sap_cycles = int(schwarz_type), int(sap_cycles)
+        p.schwarz_overlap = int(schwarz_overlap)
         if history_len > 0:                       # host buffer owned by the params object
             p._history = (ctypes.c_double * int(history_len))()
             p.history_len = int(history_len)

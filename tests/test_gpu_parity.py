@@ -300,6 +300,22 @@ def test_cfg5_full_size_operator_and_schwarz():
     assert float(torch.count_nonzero(got * ~even)) == 0
     err = float(torch.linalg.vector_norm(got - want_k) / torch.linalg.vector_norm(want_k))
     assert err <= 1e-2, ("schwarz_sap", err)
+    # overlapping domains (R18), 256 domains of 14^3x26: the GPU applies all of them, the oracle two of them
+    # (block 0, whose domain reaches through the wrap in every direction and holds the antiperiodic plane, and an
+    # interior one); compared on those blocks' own boxes, where nothing else contributes
+    ctx.set_schwarz_overlap(1)
+    fk = ctx.new_field(1)
+    ctx.schwarz(fk, ctx.pack_spinor(pt, 0, 1), 0, kappa, blk, 2, 1.0, 2, 12, 1)
+    ctx.set_schwarz_overlap(0)
+    got = torch.zeros_like(pt)
+    ctx.unpack_spinor(got, fk, 0, 1)
+    g = got.cpu().numpy()
+    for box in (0, 1 + 4 * (2 + 4 * (1 + 4 * 2))):
+        want = oracle.schwarz_ras(psi, U, T, BC, kappa, 0, blk, 1, n_mr=2, only_block=box)
+        own = np.abs(want).sum(axis=(-1, -2)) > 0
+        assert own.sum() == 12 * 12 * 12 * 24 // 2
+        err = np.linalg.norm((g - want)[own]) / np.linalg.norm(want[own])
+        assert err <= 1e-2, ("schwarz_ras", box, err)
     ctx.close()
 
 

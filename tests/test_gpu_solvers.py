@@ -475,3 +475,57 @@ def test_fused_reductions_are_bit_reproducible(mid, solver):
         assert runs[0][1] == runs[1][1]
         assert runs[0][2] == runs[1][2]
         assert np.array_equal(runs[0][0], runs[1][0])
+
+
+def test_overlapping_schwarz(mid):
+    """Overlapping (restricted additive) Schwarz domains (R18): K with every block grown by
+    one site on both sides of every direction against the oracle's block-by-block schwarz_ras, in every precision and
+    on both parities (antiperiodic t: domains at the t edges contain the sign plane); overlap 0 afterwards is the
+    non-overlapping K again; GCR-DD preconditioned by it reaches the oracle's solution; impossible overlaps are refused."""
+    c = mid
+    lq = c.lqcd
+    kappa, blk = 0.124, (4, 4, 4, 8)
+    r = inputs.gaussian_spinor(c.dims, 7)
+    d = torch.from_numpy(r).cuda()
+    try:
+        c.ctx.set_schwarz_overlap(1)
+        for prec, tol in ((0, 1e-11), (1, 5e-5), (2, 2e-2)):
+            for parity in (0, 1):
+                want = oracle.schwarz_ras(r, c.U, c.T, c.bc, kappa, parity, blk, 1, n_mr=4)
+                out = c.ctx.new_field(prec)
+                c.ctx.schwarz(out, c.ctx.pack_spinor(d, parity, prec), parity, kappa, blk, 4, 1.0, prec, 12, prec)
+                got = torch.zeros_like(d)
+                c.ctx.unpack_spinor(got, out, parity, prec)
+                g = got.cpu().numpy()
+                assert np.max(np.abs(g[c.par != parity])) == 0.0
+                assert _rel(g, want) <= tol, (prec, parity, _rel(g, want))
+        # the overlap is not silently ignored
+        assert _rel(want, oracle.schwarz(r, c.U, c.T, c.bc, kappa, 1, blk, n_mr=4)) > 1e-3
+        with pytest.raises(lq.LqcdError):                               # 4 + 2*2 = 8 = extent
+            c.ctx.set_schwarz_overlap(2)
+            c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 2), 0, kappa, blk, 4, 1.0, 2, 12, 2)
+        with pytest.raises(lq.LqcdError):                               # three partitioned directions x 1: odd
+            c.ctx.set_schwarz_overlap(1)
+            c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 2), 0, kappa, (8, 4, 4, 8), 4, 1.0, 2, 12, 2)
+    finally:
+        c.ctx.set_schwarz_overlap(0)
+    want = oracle.schwarz(r, c.U, c.T, c.bc, kappa, 0, blk, n_mr=4)
+    out = c.ctx.new_field(0)
+    c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 0), 0, kappa, blk, 4, 1.0, 0, 18, 0)
+    got = torch.zeros_like(d)
+    c.ctx.unpack_spinor(got, out, 0, 0)
+    assert _rel(got.cpu().numpy(), want) <= 1e-11
+    b = inputs.gaussian_spinor(c.dims, 2)
+    xo, io = oracle.invert(b, c.U, c.T, c.bc, kappa, parity=0, tol=1e-12)
+    its = {}
+    for ovl in (0, 1):
+        for prec in ((0, 0, 0), (0, 2, 2)):
+            p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, prec=prec, recon=(18, 12, 12), schwarz_block=blk,
+                                  mr_steps=4, schwarz_overlap=ovl)
+            x, info = _solve(c, b, p)
+            assert info["status"] == 0 and info["true_residual"] <= 1e-10 and _rel(x, xo) <= 1e-8
+            its[(ovl, prec)] = info["iterations"]
+    assert its[(1, (0, 0, 0))] <= its[(0, (0, 0, 0))]                  # the overlap does not cost outer iterations
+    p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, schwarz_block=blk, schwarz_type=lq.SCHWARZ_MULTIPLICATIVE, schwarz_overlap=1)
+    with pytest.raises(lq.LqcdError):
+        _solve(c, b, p)
