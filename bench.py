@@ -775,13 +775,14 @@ def config5(torch, lqcd, inputs, dev):
     rows = []
     B5 = (12, 12, 12, 24)
     # the paper's configuration (additive Schwarz, 10 MR steps) first, then the variants of SURVEY NEXT-1:
-    # fewer MR steps, the L2-sized block-group schedule, multiplicative Schwarz (SAP)
+    # fewer MR steps, the L2-sized block-group schedule, multiplicative Schwarz (SAP), overlapping domains
     runs = [("bicgstab", lqcd.SOLVER_BICGSTAB, (0, 1, 1), None, {}), ("bicgstab", lqcd.SOLVER_BICGSTAB, (0, 2, 2), None, {}),
             ("bicgstab_delta0.01", lqcd.SOLVER_BICGSTAB, (0, 2, 2), None, dict(delta=0.01)),
             ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 1, 2), B5, dict(mr_steps=10)), ("gcr_dd", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10)),
             ("gcr_dd_mr4", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=4)),
             ("gcr_dd_group5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10, schwarz_group=5)),
             ("gcr_sap_mr5", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=5, schwarz_type=lqcd.SCHWARZ_MULTIPLICATIVE, sap_cycles=1)),
+            ("gcr_dd_overlap1", lqcd.SOLVER_GCR_DD, (0, 2, 2), B5, dict(mr_steps=10, schwarz_overlap=1)),
             ("gcr_noprecond", lqcd.SOLVER_GCR_DD, (0, 2, 2), None, dict(gcr_kmax=16, precondition=False))]
     for name, solver, prec, blk, extra_kw in runs:
         kw = dict(gcr_kmax=16, schwarz_block=blk, **extra_kw) if blk else dict(extra_kw)
