@@ -281,6 +281,7 @@ def main():
     ap.add_argument("--solvers-only", action="store_true", help="headline + the config-4 solves only (for ncu launch lists of a solve)")
     ap.add_argument("--config5-only", action="store_true", help="headline + the config-5 solves only (for ncu launch lists of GCR-DD)")
     ap.add_argument("--schwarz-group", type=int, default=0, help="--op schwarz: blocks per launch group (0 = all)")
+    ap.add_argument("--schwarz-overlap", type=int, default=0, help="--op schwarz: sites by which every Schwarz domain is grown (0 = the paper's blocks)")
     ap.add_argument("--op", default="dslash", choices=["dslash", "staggered", "schwarz"],
                     help="dslash: the BASELINE metric (Wilson-clover Dslash); staggered: the improved staggered Dslash (SURVEY NEXT-3)")
     ap.add_argument("--long12", action="store_true", help="--op staggered: long links declared c3 x SU(3) and stored as 12 reals")
@@ -484,6 +485,7 @@ def run_schwarz(args, rank, world, local):
     del U
     ctx.build_clover(CSW)
     ctx.set_schwarz_group(args.schwarz_group)
+    ctx.set_schwarz_overlap(args.schwarz_overlap)
     fin, out = ctx.pack_spinor(b, 0, 2), ctx.new_field(2)
     step = lambda: ctx.schwarz(out, fin, 0, KAPPA, blk, n_mr, 1.0, 2, 12, 2)
     for _ in range(max(args.warmup, 3)):
@@ -498,7 +500,7 @@ def run_schwarz(args, rank, world, local):
         print(json.dumps({"metric": "schwarz_preconditioner_ms", "value": ms, "unit": "ms", "n_gpus": 1, "steps": args.steps,
                           "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
                           "vs_baseline": None, "dtype": "i16+f32", "data": "synthetic",
-                          "config": {"workload": "config 5 preconditioner: 48^3x96, 256 Schwarz blocks of 12^3x24, 10 MR steps, half", "schwarz_group": args.schwarz_group},
+                          "config": {"workload": "config 5 preconditioner: 48^3x96, 256 Schwarz blocks of 12^3x24, 10 MR steps, half", "schwarz_group": args.schwarz_group, "schwarz_overlap": args.schwarz_overlap},
                           "gpu_launches": launches,
                           "roofline": {"bound": "hbm", "achieved": by * Vh / (ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                        "frac": by * Vh / (ms * 1e-3) / 1e9 / pk["hbm_gbs"], "traffic": None, "peak_kind": pk_kind,
