@@ -501,6 +501,20 @@ def test_overlapping_schwarz(mid):
                 assert _rel(g, want) <= tol, (prec, parity, _rel(g, want))
         # the overlap is not silently ignored
         assert _rel(want, oracle.schwarz(r, c.U, c.T, c.bc, kappa, 1, blk, n_mr=4)) > 1e-3
+        # two partitioned directions (z, t), x and y keep their wrap; block groups give the same bits
+        blk2 = (8, 8, 4, 8)
+        want = oracle.schwarz_ras(r, c.U, c.T, c.bc, kappa, 0, blk2, 1, n_mr=3)
+        outs = []
+        for group in (0, 3):
+            c.ctx.set_schwarz_group(group)
+            out = c.ctx.new_field(0)
+            c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 0), 0, kappa, blk2, 3, 1.0, 0, 18, 0)
+            outs.append(out)
+        c.ctx.set_schwarz_group(0)
+        assert torch.equal(outs[0], outs[1])
+        got = torch.zeros_like(d)
+        c.ctx.unpack_spinor(got, outs[0], 0, 0)
+        assert _rel(got.cpu().numpy(), want) <= 1e-11
         with pytest.raises(lq.LqcdError):                               # 4 + 2*2 = 8 = extent
             c.ctx.set_schwarz_overlap(2)
             c.ctx.schwarz(out, c.ctx.pack_spinor(d, 0, 2), 0, kappa, blk, 4, 1.0, 2, 12, 2)
