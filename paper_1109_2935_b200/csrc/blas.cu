@@ -100,6 +100,14 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK, (sizeof(typename P::real) == 8 
 #pragma unroll
       for (int u = 0; u < U; ++u) site_caxpy<R>(nb[2 * (i0 + u)], nb[2 * (i0 + u) + 1], zi[u], zk);
     }
+    if (U > 2 && i0 + 2 <= m.k) {                // a tail of two: together as well
+      R zi[2][24];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) load_site<P, 24>(zi[u], m.z[i0 + u], a.ns, cb);
+#pragma unroll
+      for (int u = 0; u < 2; ++u) site_caxpy<R>(nb[2 * (i0 + u)], nb[2 * (i0 + u) + 1], zi[u], zk);
+      i0 += 2;
+    }
     for (; i0 < m.k; ++i0) {
       R zi[24];
       load_site<P, 24>(zi, m.z[i0], a.ns, cb);
@@ -226,6 +234,14 @@ __global__ void __launch_bounds__(LQ_BLAS_BLOCK) accumulate_kernel(char* y, cons
     for (int u = 0; u < U; ++u) load_site<PL_, 24>(x[u], m.z[j + u], m.b.ns, i);
 #pragma unroll
     for (int u = 0; u < U; ++u) add(x[u], j + u);
+  }
+  if (U > 2 && j + 2 <= m.n) {                   // a tail of two: together as well
+    typename PL_::real x[2][24];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) load_site<PL_, 24>(x[u], m.z[j + u], m.b.ns, i);
+#pragma unroll
+    for (int u = 0; u < 2; ++u) add(x[u], j + u);
+    j += 2;
   }
   for (; j < m.n; ++j) {
     typename PL_::real x[24];
