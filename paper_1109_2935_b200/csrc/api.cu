@@ -23,6 +23,8 @@ static Geom make_geom(const int* X, const int* bc, int nb) {
   g.vh = X[0] * X[1] * X[2] * X[3] / 2;
   g.nb = nb;
   g.ns = (long long)nb * g.vh;
+  auto magic = [](int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); };
+  g.mXh = magic(g.Xh); g.mY = magic(X[1]); g.mZ = magic(X[2]);
   return g;
 }
 
@@ -333,6 +335,11 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
     if (boundary[m] != 1 && boundary[m] != -1) return LQCD_EINVAL;
   }
   if ((long long)dims[0] * dims[1] * dims[2] * dims[3] / 2 > 0x7fffffffLL) return LQCD_EINVAL;
+  {   // the site index is decomposed with multiply-high divisions (core.cuh Geom): exact while Vh x max extent < 2^32
+    const long long vh = (long long)dims[0] * dims[1] * dims[2] * dims[3] / 2;
+    const int dmax = dims[0] / 2 > dims[1] ? (dims[0] / 2 > dims[2] ? dims[0] / 2 : dims[2]) : (dims[1] > dims[2] ? dims[1] : dims[2]);
+    if (vh * dmax >= (1ll << 32)) return LQCD_EINVAL;
+  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LQCD_ECUDA;
   if (cudaSetDevice(device) != cudaSuccess) return LQCD_ECUDA;

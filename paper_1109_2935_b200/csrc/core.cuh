@@ -19,11 +19,15 @@ namespace lq {
 struct Geom {
   int X[4];
   int Xh;          // X[0]/2
-  int bc[4];
+  signed char bc[4];   // +1 periodic, -1 antiperiodic, 0 open (Dirichlet) per direction
   int vh;          // sites of one parity in one box
   int nb;          // boxes in the batch
   long long ns;    // nb*vh = plane stride of every packed field
+  // ceil(2^32 / d) for d = Xh, X[1], X[2]: n / d = umulhi(n, m) exactly for n d < 2^32 (checked where a Geom is made);
+  // the three run-time divisions of the site index were ~50 instructions and 9 XU-pipe operations per thread
+  unsigned mXh, mY, mZ;
 };
+static_assert(sizeof(Geom) == 56, "Geom is part of DslashArgs, which must stay 128 bytes (dslash.cuh)");
 
 struct PrecD { typedef double store_t; typedef double real; static constexpr bool HALF = false; static constexpr int ID = 0; };
 struct PrecS { typedef float  store_t; typedef float  real; static constexpr bool HALF = false; static constexpr int ID = 1; };
@@ -398,11 +402,15 @@ LQ_DEV void quantize_link(const double* __restrict__ v, typename P::store_t* __r
 
 // ---------------------------------------------------------------- index arithmetic
 // Checkerboard index of one box: cb = xh + Xh*(y + Y*(z + Z*t)),  x = 2*xh + ((y+z+t+parity)&1).
+// n / d with the precomputed m = ceil(2^32 / d) (d = 1 has no 32-bit m)
+LQ_DEV int fast_div(int n, int d, unsigned m) { return d == 1 ? n : (int)__umulhi((unsigned)n, m); }
 LQ_DEV void cb_to_coords(const Geom& g, int cb, int parity, int c[4]) {
-  int xh = cb % g.Xh; int r = cb / g.Xh;
-  c[1] = r % g.X[1]; r /= g.X[1];
-  c[2] = r % g.X[2];
-  c[3] = r / g.X[2];
+  int r = fast_div(cb, g.Xh, g.mXh);
+  const int xh = cb - r * g.Xh;
+  int q = fast_div(r, g.X[1], g.mY);
+  c[1] = r - q * g.X[1];
+  c[3] = fast_div(q, g.X[2], g.mZ);
+  c[2] = q - c[3] * g.X[2];
   c[0] = 2 * xh + ((c[1] + c[2] + c[3] + parity) & 1);
 }
 LQ_DEV int coords_to_cb(const Geom& g, const int c[4]) {
