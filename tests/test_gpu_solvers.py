@@ -543,3 +543,24 @@ def test_overlapping_schwarz(mid):
     p = c.ctx.make_params(kappa, 1.0, 1e-10, solver=lq.SOLVER_GCR_DD, schwarz_block=blk, schwarz_type=lq.SCHWARZ_MULTIPLICATIVE, schwarz_overlap=1)
     with pytest.raises(lq.LqcdError):
         _solve(c, b, p)
+
+
+def test_overlapping_schwarz_three_blocks_in_x():
+    """An odd number of blocks in a direction (12 x 4 x 4 x 16, blocks 4 x 4 x 4 x 8: 3 x 1 x 1 x 2): every x domain
+    overlaps both its neighbours, block 0 and block 2 through the lattice's wrap; y and z are not partitioned."""
+    c = Case((12, 4, 4, 16), 0.3)
+    kappa, blk = 0.124, (4, 4, 4, 8)
+    r = inputs.gaussian_spinor(c.dims, 9)
+    d = torch.from_numpy(r).cuda()
+    try:
+        c.ctx.set_schwarz_overlap(1)
+        for prec, tol in ((0, 1e-11), (2, 2e-2)):
+            for parity in (0, 1):
+                want = oracle.schwarz_ras(r, c.U, c.T, c.bc, kappa, parity, blk, 1, n_mr=3)
+                out = c.ctx.new_field(prec)
+                c.ctx.schwarz(out, c.ctx.pack_spinor(d, parity, prec), parity, kappa, blk, 3, 1.0, prec, 12, prec)
+                got = torch.zeros_like(d)
+                c.ctx.unpack_spinor(got, out, parity, prec)
+                assert _rel(got.cpu().numpy(), want) <= tol, (prec, parity)
+    finally:
+        c.ctx.set_schwarz_overlap(0)
