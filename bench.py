@@ -45,7 +45,7 @@ def matpc_bytes(prec, recon):
 
 # ncu --set full captures of one launch at 32^3x64 (profiles/r2_dslash_*.md, commit named there): DRAM bytes read + written,
 # and executed warp instructions of the half-precision kernel (its math pipes are the second limiter)
-NCU_TRAFFIC = {("fp32", 12): 595.84e6, ("half", 12): 300.01e6, ("staggered", "fp32"): 1238.6e6}
+NCU_TRAFFIC = {("fp32", 12): 593.61e6, ("half", 12): 300.01e6, ("staggered", "fp32"): 1238.6e6}
 NCU_TRAFFIC_SRC = {("fp32", 12): "profiles/r2_dslash_fp32_r12.md", ("half", 12): "profiles/r2_dslash_half_r12_tile.md"}
 NCU_WARP_INST = {("half", 12): 47.62e6}
 N_SCHEDULERS = 148 * 4      # one warp instruction per scheduler per clock (B200: 148 SMs x 4 SMSPs)
