@@ -335,10 +335,9 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], const int boundary[4], int de
     if (boundary[m] != 1 && boundary[m] != -1) return LQCD_EINVAL;
   }
   if ((long long)dims[0] * dims[1] * dims[2] * dims[3] / 2 > 0x7fffffffLL) return LQCD_EINVAL;
-  {   // the site index is decomposed with multiply-high divisions (core.cuh Geom): exact while Vh x max extent < 2^32
-    const long long vh = (long long)dims[0] * dims[1] * dims[2] * dims[3] / 2;
-    const int dmax = dims[0] / 2 > dims[1] ? (dims[0] / 2 > dims[2] ? dims[0] / 2 : dims[2]) : (dims[1] > dims[2] ? dims[1] : dims[2]);
-    if (vh * dmax >= (1ll << 32)) return LQCD_EINVAL;
+  {   // the site index is decomposed with multiply-high divisions (core.cuh Geom): n / d is exact while n d < 2^32
+    const long long vh = (long long)dims[0] * dims[1] * dims[2] * dims[3] / 2, xh = dims[0] / 2;
+    if (vh * xh >= (1ll << 32) || (vh / xh) * dims[1] >= (1ll << 32) || (vh / xh / dims[1]) * dims[2] >= (1ll << 32)) return LQCD_EINVAL;
   }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LQCD_ECUDA;
