@@ -83,3 +83,28 @@ def test_random_staggered(seed):
     want = oracle.stag_MdagM(chi * mask, fat, lng, bc, mass, sigma) * mask
     assert _rel(got.cpu().numpy(), want) <= (1e-13 if prec == 0 else 1e-5), (dims, bc, prec, use12)
     ctx.close()
+
+
+@pytest.mark.parametrize("seed", [0, 1, 5, 6, 14, 16, 17, 22, 25, 27])
+def test_random_overlapping_schwarz(seed):
+    """Overlapping Schwarz domains (R18) on drawn shapes: directions of extent 8 or 12 are cut into blocks of 4
+    (an even number of them), the others stay whole; one site of overlap; random boundary signs, so that antiperiodic
+    planes fall inside grown domains in x, y, z as well as t; against the oracle's block-by-block schwarz_ras."""
+    rng, dims, bc = _draw(seed)
+    blk = [4 if d in (8, 12) else d for d in dims]
+    parts = [m for m in range(4) if blk[m] != dims[m]]
+    if len(parts) % 2:
+        blk[parts[0]] = dims[parts[0]]
+        parts = parts[1:]
+    assert len(parts) >= 2, "seed list and draw disagree"
+    c = Case(dims, float(rng.uniform(0.1, 0.6)), c_sw=float(rng.uniform(0.0, 1.5)), bc=bc, gauge_seed=seed)
+    kappa = float(rng.uniform(0.05, 0.11))
+    psi = inputs.gaussian_spinor(dims, 90 + seed)
+    prec, parity, n_mr = int(rng.integers(0, 3)), int(rng.integers(0, 2)), int(rng.integers(1, 4))
+    want = oracle.schwarz_ras(psi, c.U, c.T, c.bc, kappa, parity, tuple(blk), 1, n_mr=n_mr)
+    try:
+        c.ctx.set_schwarz_overlap(1)
+        got = c.gpu_parity_op(lambda o, i: c.ctx.schwarz(o, i, parity, kappa, tuple(blk), n_mr, 1.0, prec, 12, prec), psi, parity, parity, prec)
+    finally:
+        c.ctx.set_schwarz_overlap(0)
+    assert _rel(got, want) <= 3 * n_mr * TOL[prec], ("schwarz_ras", dims, bc, blk, prec, n_mr)
